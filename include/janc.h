@@ -1,0 +1,130 @@
+/* janc.h -- C ABI of libjanc: the per-time-step update of the compressible multi-species
+ * reacting Euler equations on uniform block-structured patches (arXiv 2504.13750, "JANC"),
+ * implemented as hand-written sm_100a CUDA kernels in fp64.
+ *
+ * Citations are PAPER.md:<line> (section / equation).  Readings of silent or garbled passages
+ * (A1..A24) are listed in DESIGN.md.
+ *
+ * Conventions
+ *  - Every call returns an int status (JANC_OK = 0, negative = error); nothing throws or aborts
+ *    across the ABI.  janc_last_error() gives a text for the last failure of a context.
+ *  - The caller owns every buffer it passes; the library copies what it keeps.  Device memory
+ *    for the state and all scratch comes from ONE caller-allocated workspace
+ *    (janc_workspace_bytes / janc_bind_workspace); the library never allocates the big arrays.
+ *  - All kernels are enqueued on the CUDA stream given to janc_create (a cudaStream_t passed as
+ *    void*; NULL = legacy default stream).  janc_step is asynchronous unless t_advanced != NULL.
+ *  - A device-side flag (non-finite value, T <= 0, Newton not converged, singular pivot) is
+ *    reported as JANC_ENONFINITE by the next synchronising call (janc_step with t_advanced,
+ *    janc_get_state, janc_status).
+ *  - There is no CPU fallback: without a CUDA device janc_create returns JANC_ECUDA.
+ *
+ * State layout (PAPER.md:232 eq 4.1; :83, :179 block data [N, n_U, n_x, n_y]):
+ *    U[np][nvar][nz][ny][nx], x fastest, interior cells only (no ghosts), fp64, with
+ *    nvar = ndim + 2 + (ns-1) in the paper's order  rho, rho*u[, rho*v[, rho*w]], E,
+ *    rho*Y_1 .. rho*Y_{ns-1};  np = max(1, n_patches).  T[np][nz][ny][nx] likewise.
+ */
+#ifndef JANC_H
+#define JANC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct janc_ctx janc_ctx; /* opaque, owned by the library */
+
+enum { JANC_OK = 0, JANC_EINVAL = -1, JANC_ENOMEM = -2, JANC_ECUDA = -3, JANC_ESTATE = -4, JANC_ENONFINITE = -5 };
+
+/* Physical boundary kinds (readings A14, A15):
+ * PERIODIC copies the opposite interior layers (uniform grid only; in block mode periodicity is
+ * expressed through the neighbour lists), REFLECT mirrors about the face and negates the normal
+ * momentum (slip wall), OUTFLOW copies the nearest interior cell (zero gradient,
+ * the paper's "non-reflecting"). */
+enum { JANC_BC_PERIODIC = 0, JANC_BC_REFLECT = 1, JANC_BC_OUTFLOW = 2 };
+
+typedef struct {
+  int ndim;               /* 1, 2 or 3 (paper: 2; reading A18)                     */
+  int n[3];               /* interior cells per direction (per patch in block mode)              */
+  double dx[3];           /* level-0 spacing (m); level l uses dx / ratio^l                      */
+  int bc_lo[3], bc_hi[3]; /* physical boundary kind per face                                     */
+  int n_patches;          /* 0 = one uniform grid; > 0 = block-list mode        */
+  int n_levels, ratio;    /* block mode: 1 or 2 levels, refine ratio 2          */
+} janc_grid;
+
+/* Reaction mechanism (eq 4.3-4.9).  Host arrays, copied by the call. */
+typedef struct {
+  int ns, nr;                /* species (>= 1), reactions (>= 0); ns <= 32, nr <= 128             */
+  const double *W;           /* [ns] molar mass, kg/mol                                           */
+  const double *nasa;        /* [ns][7] a0..a6 of eq 4.3-4.5, single range (reading A7)           */
+  const int32_t *nu_f, *nu_b;/* [nr][ns] integer stoichiometry 0..3 (eq 4.6)                      */
+  const double *A, *b, *Ta;  /* [nr] Arrhenius in SI (mol, m^3, s); Ta = Ea/Ru in K (eq 4.8)      */
+  const int32_t *reversible; /* [nr] 0 => k_b = 0 (reading A10)                                   */
+  const int32_t *third_body; /* [nr] 1 => rate multiplied by sum_j a_ij X_j (eq 4.7, reading A9)  */
+  const double *eff;         /* [nr][ns] a_ij; NULL => all 1                                      */
+} janc_mech;
+
+/* Create a context for one grid on CUDA device `device`; kernels go to `cuda_stream`. */
+int janc_create(const janc_grid *grid, int device, void *cuda_stream, janc_ctx **out);
+
+/* Mechanism must be set before the workspace is sized (nvar depends on ns). */
+int janc_set_mechanism(janc_ctx *, const janc_mech *);
+
+/* Bytes of device memory the context needs (state with ghosts, RK registers, primitives,
+ * reduction slots).  The caller allocates (e.g. torch.empty(..., device='cuda')) and binds a
+ * 256-byte aligned device pointer; it must stay alive until janc_destroy. */
+size_t janc_workspace_bytes(const janc_ctx *);
+int janc_bind_workspace(janc_ctx *, void *dev_ptr, size_t bytes);
+
+/* Block lists: level[np]; nbr[np][2*ndim] same-level neighbour patch ids in the
+ * order lo-x, hi-x, lo-y, hi-y, lo-z, hi-z, -1 = none; parent[np][1+ndim] = (parent patch id,
+ * sub-region index along x, y[, z] in 0..ratio-1), -1 on level 0.  Host arrays, copied.
+ * A face without neighbour is filled from the physical BC on level 0; on level 1 by
+ * piecewise-constant injection from the coarse parent unless the face lies on
+ * the domain boundary (reading A19). */
+int janc_set_blocks(janc_ctx *, const int32_t *level, const int32_t *nbr, const int32_t *parent);
+
+/* Load the state.  U as laid out above; T_guess (nullable: 1000 K) seeds the Newton iteration
+ * (reading A6).  on_device != 0: pointers are device pointers on the same device. */
+int janc_set_state(janc_ctx *, const double *U, const double *T_guess, int on_device);
+
+/* Advance nsteps of advance_one_step: cfl() -> advance_flux (TVD-RK3 over
+ * rhs: ghost fill, update_aux, LF-split WENO5 fluxes, divergence) -> advance_source_term
+ * (point-implicit chemistry, eq 4.12-4.13) [-> average-down in 2-level block mode, PAPER.md:188].
+ * cfl > 0: dt = cfl * min_d dx_d(finest) / max(|u_d| + c) each step (reading A16);
+ * cfl <= 0: dt = dt_fixed.  flags: bit 0 set => skip chemistry (explicit variant).
+ * t_advanced (host, nullable): receives the sum of dt; forces a stream synchronise. */
+int janc_step(janc_ctx *, int nsteps, double cfl, double dt_fixed, int flags, double *t_advanced);
+
+/* Read the state back (U and/or T nullable).  Synchronises.  Returns JANC_ENONFINITE if the
+ * device flag was raised since the last janc_set_state. */
+int janc_get_state(janc_ctx *, double *U, double *T, int on_device);
+
+/* Synchronise and return JANC_OK / JANC_ENONFINITE / JANC_ECUDA. */
+int janc_status(janc_ctx *);
+
+/* Number of kernel launches enqueued by this context since creation (diagnostic). */
+long long janc_launch_count(const janc_ctx *);
+
+/* Diagnostic: run the fused cons->prim + thermo kernel on the current
+ * state and return T, p, c per interior cell ([np][nz][ny][nx] each, device or host). */
+int janc_debug_cons2prim(janc_ctx *, double *T, double *p, double *c, int on_device);
+
+/* Diagnostic: per-phase device time (ms, CUDA events on the context's stream) of ONE step at the
+ * current state: out[0]=cons2prim+reduce, [1]=ghost fill, [2]=flux sweeps+divergence+RK,
+ * [3]=chemistry, [4]=average-down, [5]=whole step; launches of each in n_out[0..5] (nullable).
+ * Advances the state by one step with the given cfl/dt_fixed. */
+int janc_profile_step(janc_ctx *, double cfl, double dt_fixed, float *ms_out, int *n_out);
+
+/* Diagnostic: measured register-resident DFMA rate of the device, in DFMA/s (the FP64 ALU peak
+ * used as roofline denominator for "bound":"alu"). */
+int janc_measure_dfma_peak(int device, void *cuda_stream, double *dfma_per_s);
+
+const char *janc_last_error(const janc_ctx *);
+void janc_destroy(janc_ctx *);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JANC_H */

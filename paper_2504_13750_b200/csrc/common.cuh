@@ -1,0 +1,61 @@
+// common.cuh -- shared definitions of the libjanc CUDA path (sm_100a, fp64).
+// Independent of oracle/: nothing here is included by, or includes, the CPU oracle.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define JANC_NG 3            // ghost layers
+#define JANC_MAX_NS 32
+#define JANC_MAX_NR 128
+#define JANC_MAX_ORDER 6     // sum of stoichiometric coefficients on one side of a reaction
+#define JANC_RU 8.314472
+#define JANC_PATM 101325.0   // eq 4.9
+
+enum { FK_NEIGHBOUR = 0, FK_PHYSICAL = 1, FK_COARSE = 2 };
+
+// Mechanism in constant memory (eq 4.3-4.9).  Reactant / product lists are expanded with
+// multiplicity: prod_j X_j^nu_ij = prod_e X[sp[e]].
+struct MechC {
+  int ns, nr;
+  double W[JANC_MAX_NS], invW[JANC_MAX_NS], Rk[JANC_MAX_NS];
+  double nasa[JANC_MAX_NS][7];
+  double lnA[JANC_MAX_NR], b[JANC_MAX_NR], Ta[JANC_MAX_NR];
+  double Asign[JANC_MAX_NR];                 // sign(A) (A may not be <= 0; kept for safety: +1)
+  signed char rev[JANC_MAX_NR], tb[JANC_MAX_NR], dn[JANC_MAX_NR];
+  unsigned char nreac[JANC_MAX_NR], nprod[JANC_MAX_NR];
+  unsigned char reac[JANC_MAX_NR][JANC_MAX_ORDER], prod[JANC_MAX_NR][JANC_MAX_ORDER];
+  double eff[JANC_MAX_NR][JANC_MAX_NS];
+};
+
+// Geometry + device pointers handed to every kernel by value.
+struct Params {
+  int ndim, nvar, ns, np, nlev, ratio;
+  int n[3];          // interior cells per patch
+  int P[3];          // padded dims
+  int G[3];          // ghost width per dim (3 or 0)
+  long long st[3];   // strides in doubles
+  long long pc;      // padded cells per patch
+  double invdx[2][3];
+  double dxmin;
+  int bc_lo[3], bc_hi[3];
+  // device arrays
+  double *T, *p, *vel;        // [np][pc], [np][pc], [ndim][np][pc]
+  const int *level, *nbr, *parent, *fkind;
+  unsigned long long *slots;  // [2 parity][3 stage][2 lev][3 dir] ordered-int max(|u_d|+c)
+  double *scal;               // [0]=dt, [1]=t accumulated
+  int *flag;                  // device error flag
+};
+
+#define SLOT(par, stage, lev, d) ((((par) * 3 + (stage)) * 2 + (lev)) * 3 + (d))
+
+__device__ __forceinline__ long long cell_index(const Params &P, int i, int j, int k) {
+  return (long long)(i + P.G[0]) * P.st[0] + (long long)(j + P.G[1]) * P.st[1] + (long long)(k + P.G[2]) * P.st[2];
+}
+
+// non-negative doubles order like their bit patterns: exact, order-independent max
+__device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, double v) {
+  atomicMax(addr, (unsigned long long)__double_as_longlong(v));
+}
+__device__ __forceinline__ double slot_value(const unsigned long long *addr) {
+  return __longlong_as_double((long long)*addr);
+}

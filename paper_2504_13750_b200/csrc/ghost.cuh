@@ -1,0 +1,93 @@
+// ghost.cuh -- batched ghost fill over block lists + average-down.
+// PAPER.md:295 (3 ghost layers), :329 (boundary_conditions), :97, :117, :213 (get_ghost_block),
+// :215 (update_physical_boundary), :115 (one-to-four injection), :116/:188 (four-to-one mean).
+// Readings A14, A15, A19, A21.  Fills U (nvar fields) and the primitives T, p, vel.
+#pragma once
+#include "common.cuh"
+
+__device__ __forceinline__ int floordiv_i(int a, int b) {
+  int q = a / b;
+  if ((a % b != 0) && ((a < 0) != (b < 0))) q--;
+  return q;
+}
+
+// grid: (ceil(nf*3*amax / 256), np); only patches with level == lev act (level 0 must be complete
+// before level 1 injects from its padded parent).
+__global__ void __launch_bounds__(256) k_ghost(Params P, double *__restrict__ U, int lev, int amax) {
+  const int patch = blockIdx.y;
+  if (P.level[patch] != lev) return;
+  const int nf = 2 * P.ndim;
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)nf * JANC_NG * amax) return;
+  const int t = (int)(idx % amax);
+  const int g = (int)((idx / amax) % JANC_NG) + 1;
+  const int f = (int)(idx / ((long long)amax * JANC_NG));
+  const int d = f >> 1, side = f & 1;
+  const int e1 = d == 0 ? 1 : 0;            // fastest tangential dim
+  const int e2 = d == 2 ? 1 : 2;            // slowest tangential dim
+  if (t >= P.n[e1] * P.n[e2]) return;
+  int dst[3], src[3];
+  dst[e1] = t % P.n[e1];
+  dst[e2] = t / P.n[e1];
+  dst[d] = side == 0 ? -g : P.n[d] - 1 + g;
+  src[0] = dst[0]; src[1] = dst[1]; src[2] = dst[2];
+  const int kind = P.fkind[patch * nf + f];
+  const int bc = side == 0 ? P.bc_lo[d] : P.bc_hi[d];
+  int q = patch;
+  bool flip = false;
+  if (kind == FK_NEIGHBOUR || (kind == FK_PHYSICAL && bc == 0 /*periodic*/)) {
+    if (kind == FK_NEIGHBOUR) q = P.nbr[patch * nf + f];
+    src[d] = side == 0 ? P.n[d] - g : g - 1;
+  } else if (kind == FK_PHYSICAL && bc == 1 /*reflect*/) {
+    src[d] = side == 0 ? g - 1 : P.n[d] - g;
+    flip = true;
+  } else if (kind == FK_PHYSICAL) {       /*outflow*/
+    src[d] = side == 0 ? 0 : P.n[d] - 1;
+  } else {                                  /*coarse parent, piecewise-constant injection*/
+    const int *par = P.parent + patch * (1 + P.ndim);
+    q = par[0];
+    for (int e = 0; e < P.ndim; e++) src[e] = floordiv_i(par[1 + e] * P.n[e] + dst[e], P.ratio);
+  }
+  const long long di = (long long)patch * P.pc + cell_index(P, dst[0], dst[1], dst[2]);
+  const long long si = (long long)q * P.pc + cell_index(P, src[0], src[1], src[2]);
+  const long long dU = di + (long long)patch * (P.nvar - 1) * P.pc;   // = patch*nvar*pc + cell
+  const long long sU = si + (long long)q * (P.nvar - 1) * P.pc;
+  for (int v = 0; v < P.nvar; v++) {
+    double val = U[sU + (long long)v * P.pc];
+    if (flip && v == 1 + d) val = -val;
+    U[dU + (long long)v * P.pc] = val;
+  }
+  P.T[di] = P.T[si];
+  P.p[di] = P.p[si];
+  for (int e = 0; e < P.ndim; e++) {
+    double val = P.vel[(long long)e * P.np * P.pc + si];
+    if (flip && e == d) val = -val;
+    P.vel[(long long)e * P.np * P.pc + di] = val;
+  }
+}
+
+// Average-down: every level-1 patch writes the mean of its ratio^ndim children cells into the covered
+// cells of its parent.  grid: (ceil(nvar*coarse cells per fine patch / 256), np).
+__global__ void __launch_bounds__(256) k_average_down(Params P, double *__restrict__ U) {
+  const int patch = blockIdx.y;
+  if (P.level[patch] == 0) return;
+  const int r = P.ratio;
+  const int rr[3] = {r, P.ndim > 1 ? r : 1, P.ndim > 2 ? r : 1};
+  const int m[3] = {P.n[0] / rr[0], P.n[1] / rr[1], P.n[2] / rr[2]};
+  const int nc = m[0] * m[1] * m[2];
+  int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= nc * P.nvar) return;
+  const int v = idx / nc;
+  int c = idx % nc;
+  const int i = c % m[0], j = (c / m[0]) % m[1], k = c / (m[0] * m[1]);
+  const int *par = P.parent + patch * (1 + P.ndim);
+  const int q = par[0];
+  int off[3] = {0, 0, 0};
+  for (int e = 0; e < P.ndim; e++) off[e] = par[1 + e] * m[e];
+  const double *src = U + ((long long)patch * P.nvar + v) * P.pc;
+  double s = 0.0;
+  for (int kk = 0; kk < rr[2]; kk++)
+    for (int jj = 0; jj < rr[1]; jj++)
+      for (int ii = 0; ii < rr[0]; ii++) s += src[cell_index(P, i * rr[0] + ii, j * rr[1] + jj, k * rr[2] + kk)];
+  U[((long long)q * P.nvar + v) * P.pc + cell_index(P, off[0] + i, off[1] + j, off[2] + k)] = s * (1.0 / (rr[0] * rr[1] * rr[2]));
+}
