@@ -1,0 +1,563 @@
+// janc.cu -- host side of libjanc (C ABI declared in include/janc.h) + small utility kernels.
+// No CPU fallback: every step of the path runs in the kernels of prim/ghost/flux/chem.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/janc.h"
+#include "chem.cuh"
+#include "flux.cuh"
+#include "ghost.cuh"
+#include "prim.cuh"
+
+struct janc_ctx {
+  janc_grid g;
+  int device;
+  cudaStream_t stream;
+  int np, nvar, ns, nr;
+  bool have_mech, have_ws, have_state, have_blocks;
+  MechC mech;
+  Params P;
+  long long ncell;       // interior cells per patch
+  // workspace carve-up
+  size_t ws_bytes;
+  double *A, *B, *C;     // RK registers (A holds the state between steps)
+  double *dbgc, *stageU, *stageT;
+  int *d_level, *d_nbr, *d_parent, *d_fkind;
+  std::vector<int> level, nbr, parent, fkind;
+  int parity;
+  long long launches;
+  unsigned long long id;
+  std::string err;
+};
+
+static unsigned long long g_next_id = 1;
+static unsigned long long g_mech_owner = 0;   // which context's mechanism sits in c_mech
+
+#define CK(call)                                                                         \
+  do {                                                                                   \
+    cudaError_t e_ = (call);                                                             \
+    if (e_ != cudaSuccess) {                                                             \
+      c->err = std::string(#call) + ": " + cudaGetErrorString(e_);                       \
+      return JANC_ECUDA;                                                                 \
+    }                                                                                    \
+  } while (0)
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ------------------------------------------------------------------ utility kernels
+// interior layout [np][nf][ncell]  <->  padded layout [np][nf][pc]
+__global__ void __launch_bounds__(256) k_pack(Params P, const double *__restrict__ src, double *__restrict__ dst,
+                                              int nf, int unpack, double fill) {
+  const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ncell) return;
+  const int f = blockIdx.y % nf, patch = blockIdx.y / nf;
+  const int i = (int)(t % P.n[0]);
+  const long long r = t / P.n[0];
+  const int j = (int)(r % P.n[1]), k = (int)(r / P.n[1]);
+  const long long pi = ((long long)patch * nf + f) * P.pc + cell_index(P, i, j, k);
+  const long long ii = ((long long)patch * nf + f) * ncell + t;
+  if (unpack) dst[ii] = src[pi];
+  else dst[pi] = src ? src[ii] : fill;
+}
+
+__global__ void k_dfma(double *out, int iters) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const double m = 1.0000001, b = 1e-9;
+#pragma unroll 1
+  for (int i = 0; i < iters; i++) {
+#pragma unroll
+    for (int u = 0; u < 8; u++) {
+      a0 = fma(a0, m, b); a1 = fma(a1, m, b); a2 = fma(a2, m, b); a3 = fma(a3, m, b);
+      a4 = fma(a4, m, b); a5 = fma(a5, m, b); a6 = fma(a6, m, b); a7 = fma(a7, m, b);
+    }
+  }
+  double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+  if (s == 123.456) out[0] = s;
+}
+
+// ------------------------------------------------------------------ create / destroy
+extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream, janc_ctx **out) {
+  if (!grid || !out) return JANC_EINVAL;
+  if (grid->ndim < 1 || grid->ndim > 3) return JANC_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return JANC_ECUDA;
+  if (cudaSetDevice(device) != cudaSuccess) return JANC_ECUDA;
+  janc_ctx *c = new (std::nothrow) janc_ctx();
+  if (!c) return JANC_ENOMEM;
+  c->g = *grid;
+  c->device = device;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->np = grid->n_patches > 0 ? grid->n_patches : 1;
+  if (grid->n_patches <= 0) { c->g.n_levels = 1; c->g.ratio = 2; }
+  if (c->g.n_levels < 1 || c->g.n_levels > 2 || (c->g.n_levels == 2 && c->g.ratio != 2)) { delete c; return JANC_EINVAL; }
+  Params &P = c->P;
+  memset(&P, 0, sizeof P);
+  P.ndim = grid->ndim; P.np = c->np; P.nlev = c->g.n_levels; P.ratio = c->g.ratio;
+  P.pc = 1; c->ncell = 1;
+  double dxmin = 1e300;
+  for (int d = 0; d < 3; d++) {
+    if (d < grid->ndim) {
+      if (grid->n[d] < 1 || !(grid->dx[d] > 0.0)) { delete c; return JANC_EINVAL; }
+      if (c->g.n_levels == 2 && grid->n[d] % 2) { delete c; return JANC_EINVAL; }
+      P.n[d] = grid->n[d]; P.G[d] = JANC_NG; P.P[d] = grid->n[d] + 2 * JANC_NG;
+      double dx = grid->dx[d];
+      P.invdx[0][d] = 1.0 / dx; P.invdx[1][d] = 1.0 / (dx / c->g.ratio);
+      double dxf = c->g.n_levels == 2 ? dx / c->g.ratio : dx;
+      if (dxf < dxmin) dxmin = dxf;
+      P.bc_lo[d] = grid->bc_lo[d]; P.bc_hi[d] = grid->bc_hi[d];
+      if (P.bc_lo[d] < 0 || P.bc_lo[d] > 2 || P.bc_hi[d] < 0 || P.bc_hi[d] > 2) { delete c; return JANC_EINVAL; }
+    } else {
+      c->g.n[d] = 1; P.n[d] = 1; P.G[d] = 0; P.P[d] = 1; P.invdx[0][d] = P.invdx[1][d] = 0.0;
+    }
+    P.st[d] = P.pc; P.pc *= P.P[d]; c->ncell *= P.n[d];
+  }
+  P.dxmin = dxmin;
+  int nf = 2 * grid->ndim;
+  c->level.assign(c->np, 0);
+  c->nbr.assign((size_t)c->np * nf, -1);
+  c->parent.assign((size_t)c->np * (1 + grid->ndim), -1);
+  c->fkind.assign((size_t)c->np * nf, FK_PHYSICAL);
+  c->id = g_next_id++;
+  *out = c;
+  return JANC_OK;
+}
+
+extern "C" void janc_destroy(janc_ctx *c) {
+  if (!c) return;
+  if (g_mech_owner == c->id) g_mech_owner = 0;
+  delete c;
+}
+
+extern "C" const char *janc_last_error(const janc_ctx *c) { return c ? c->err.c_str() : "null context"; }
+extern "C" long long janc_launch_count(const janc_ctx *c) { return c ? c->launches : 0; }
+
+// ------------------------------------------------------------------ mechanism
+extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
+  if (!c || !m) return JANC_EINVAL;
+  if (m->ns < 1 || m->ns > JANC_MAX_NS || m->nr < 0 || m->nr > JANC_MAX_NR) { c->err = "ns/nr out of range"; return JANC_EINVAL; }
+  if (!m->W || !m->nasa) return JANC_EINVAL;
+  MechC &M = c->mech;
+  memset(&M, 0, sizeof M);
+  M.ns = m->ns; M.nr = m->nr;
+  for (int k = 0; k < m->ns; k++) {
+    if (!(m->W[k] > 0.0)) return JANC_EINVAL;
+    M.W[k] = m->W[k]; M.invW[k] = 1.0 / m->W[k]; M.Rk[k] = JANC_RU / m->W[k];
+    for (int q = 0; q < 7; q++) M.nasa[k][q] = m->nasa[k * 7 + q];
+  }
+  for (int i = 0; i < m->nr; i++) {
+    if (!(m->A[i] > 0.0)) { c->err = "A must be > 0"; return JANC_EINVAL; }
+    M.lnA[i] = log(m->A[i]); M.b[i] = m->b[i]; M.Ta[i] = m->Ta[i]; M.Asign[i] = 1.0;
+    M.rev[i] = m->reversible ? (m->reversible[i] != 0) : 1;
+    M.tb[i] = m->third_body ? (m->third_body[i] != 0) : 0;
+    int nre = 0, npr = 0, dn = 0;
+    for (int k = 0; k < m->ns; k++) {
+      int f = m->nu_f[i * m->ns + k], b = m->nu_b[i * m->ns + k];
+      if (f < 0 || b < 0) return JANC_EINVAL;
+      if (nre + f > JANC_MAX_ORDER || npr + b > JANC_MAX_ORDER) { c->err = "reaction order too large"; return JANC_EINVAL; }
+      for (int q = 0; q < f; q++) M.reac[i][nre++] = (unsigned char)k;
+      for (int q = 0; q < b; q++) M.prod[i][npr++] = (unsigned char)k;
+      dn += b - f;
+    }
+    M.nreac[i] = (unsigned char)nre; M.nprod[i] = (unsigned char)npr; M.dn[i] = (signed char)dn;
+    for (int k = 0; k < m->ns; k++) M.eff[i][k] = m->eff ? m->eff[i * m->ns + k] : 1.0;
+  }
+  c->ns = m->ns; c->nr = m->nr;
+  c->nvar = c->g.ndim + 2 + m->ns - 1;
+  c->P.nvar = c->nvar; c->P.ns = m->ns;
+  c->have_mech = true; c->have_ws = false; c->have_state = false;
+  if (g_mech_owner == c->id) g_mech_owner = 0;
+  return JANC_OK;
+}
+
+static int upload_mech(janc_ctx *c) {
+  if (g_mech_owner == c->id) return JANC_OK;
+  CK(cudaMemcpyToSymbolAsync(c_mech, &c->mech, sizeof(MechC), 0, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));   // c->mech is pageable host memory
+  g_mech_owner = c->id;
+  return JANC_OK;
+}
+
+// ------------------------------------------------------------------ workspace
+struct Carve { size_t off; size_t take(size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; } };
+
+static void carve(janc_ctx *c, char *base, size_t *total) {
+  Carve cv{0};
+  const size_t cells = (size_t)c->np * c->P.pc, nf = 2 * c->g.ndim;
+  size_t oA = cv.take(cells * c->nvar * 8), oB = cv.take(cells * c->nvar * 8), oC = cv.take(cells * c->nvar * 8);
+  size_t oT = cv.take(cells * 8), op = cv.take(cells * 8), ov = cv.take(cells * c->g.ndim * 8), oc = cv.take(cells * 8);
+  size_t osU = cv.take((size_t)c->np * c->ncell * c->nvar * 8), osT = cv.take((size_t)c->np * c->ncell * 8);
+  size_t oslots = cv.take(36 * 8), oscal = cv.take(4 * 8), oflag = cv.take(16);
+  size_t olev = cv.take(c->np * 4), onbr = cv.take(c->np * nf * 4), opar = cv.take(c->np * (1 + c->g.ndim) * 4), ofk = cv.take(c->np * nf * 4);
+  if (total) *total = cv.off;
+  if (base) {
+    c->A = (double *)(base + oA); c->B = (double *)(base + oB); c->C = (double *)(base + oC);
+    c->P.T = (double *)(base + oT); c->P.p = (double *)(base + op); c->P.vel = (double *)(base + ov);
+    c->dbgc = (double *)(base + oc); c->stageU = (double *)(base + osU); c->stageT = (double *)(base + osT);
+    c->P.slots = (unsigned long long *)(base + oslots); c->P.scal = (double *)(base + oscal); c->P.flag = (int *)(base + oflag);
+    c->d_level = (int *)(base + olev); c->d_nbr = (int *)(base + onbr); c->d_parent = (int *)(base + opar); c->d_fkind = (int *)(base + ofk);
+    c->P.level = c->d_level; c->P.nbr = c->d_nbr; c->P.parent = c->d_parent; c->P.fkind = c->d_fkind;
+  }
+}
+
+extern "C" size_t janc_workspace_bytes(const janc_ctx *c) {
+  if (!c || !c->have_mech) return 0;
+  size_t total = 0;
+  carve(const_cast<janc_ctx *>(c), nullptr, &total);
+  return total;
+}
+
+static int upload_lists(janc_ctx *c) {
+  CK(cudaMemcpyAsync(c->d_level, c->level.data(), c->level.size() * 4, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->d_nbr, c->nbr.data(), c->nbr.size() * 4, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->d_parent, c->parent.data(), c->parent.size() * 4, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->d_fkind, c->fkind.data(), c->fkind.size() * 4, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return JANC_OK;
+}
+
+extern "C" int janc_bind_workspace(janc_ctx *c, void *dev_ptr, size_t bytes) {
+  if (!c || !c->have_mech || !dev_ptr) return JANC_EINVAL;
+  size_t need = janc_workspace_bytes(c);
+  if (bytes < need || ((uintptr_t)dev_ptr & 255)) { c->err = "workspace too small or misaligned"; return JANC_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  carve(c, (char *)dev_ptr, nullptr);
+  c->ws_bytes = need;
+  CK(cudaMemsetAsync(dev_ptr, 0, need, c->stream));
+  c->have_ws = true; c->have_state = false; c->parity = 0;
+  return upload_lists(c);
+}
+
+// ------------------------------------------------------------------ block lists
+extern "C" int janc_set_blocks(janc_ctx *c, const int32_t *level, const int32_t *nbr, const int32_t *parent) {
+  if (!c || c->g.n_patches <= 0 || !level || !nbr) return JANC_EINVAL;
+  const int nd = c->g.ndim, nf = 2 * nd, np = c->np;
+  for (int p = 0; p < np; p++) {
+    if (level[p] < 0 || level[p] >= c->g.n_levels) { c->err = "level out of range"; return JANC_EINVAL; }
+    for (int f = 0; f < nf; f++) {
+      int q = nbr[p * nf + f];
+      if (q >= np || (q >= 0 && level[q] != level[p])) { c->err = "bad neighbour id"; return JANC_EINVAL; }
+    }
+    if (level[p] > 0) {
+      if (!parent) return JANC_EINVAL;
+      int k = parent[p * (1 + nd)];
+      if (k < 0 || k >= np || level[k] != level[p] - 1) { c->err = "bad parent id"; return JANC_EINVAL; }
+      for (int e = 0; e < nd; e++) {
+        int s = parent[p * (1 + nd) + 1 + e];
+        if (s < 0 || s >= c->g.ratio) { c->err = "bad sub-region index"; return JANC_EINVAL; }
+      }
+    }
+  }
+  for (int p = 0; p < np; p++) {
+    c->level[p] = level[p];
+    for (int f = 0; f < nf; f++) c->nbr[p * nf + f] = nbr[p * nf + f];
+    for (int e = 0; e <= nd; e++) c->parent[p * (1 + nd) + e] = parent ? parent[p * (1 + nd) + e] : -1;
+  }
+  // which source fills each face: neighbour, physical BC, or the coarse parent
+  for (int p = 0; p < np; p++)
+    for (int f = 0; f < nf; f++) {
+      int kind;
+      if (c->nbr[p * nf + f] >= 0) kind = FK_NEIGHBOUR;
+      else if (c->level[p] == 0) kind = FK_PHYSICAL;
+      else {
+        const int k = c->parent[p * (1 + nd)], d = f / 2, side = f % 2;
+        const int s = c->parent[p * (1 + nd) + 1 + d];
+        const bool at_parent_edge = side == 0 ? (s == 0) : (s == c->g.ratio - 1);
+        kind = (at_parent_edge && c->nbr[k * nf + f] < 0) ? FK_PHYSICAL : FK_COARSE;
+      }
+      c->fkind[p * nf + f] = kind;
+    }
+  c->have_blocks = true;
+  if (c->have_ws) return upload_lists(c);
+  return JANC_OK;
+}
+
+// ------------------------------------------------------------------ state in / out
+static dim3 cell_grid(const janc_ctx *c, int threads, int ny) {
+  return dim3((unsigned)((c->ncell + threads - 1) / threads), (unsigned)ny, 1);
+}
+
+extern "C" int janc_set_state(janc_ctx *c, const double *U, const double *Tg, int on_device) {
+  if (!c || !U) return JANC_EINVAL;
+  if (!c->have_ws) { c->err = "bind a workspace first"; return JANC_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  const size_t nU = (size_t)c->np * c->nvar * c->ncell, nT = (size_t)c->np * c->ncell;
+  const double *dU = U, *dT = Tg;
+  if (!on_device) {
+    CK(cudaMemcpyAsync(c->stageU, U, nU * 8, cudaMemcpyHostToDevice, c->stream));
+    dU = c->stageU;
+    if (Tg) { CK(cudaMemcpyAsync(c->stageT, Tg, nT * 8, cudaMemcpyHostToDevice, c->stream)); dT = c->stageT; }
+  }
+  k_pack<<<cell_grid(c, 256, c->np * c->nvar), 256, 0, c->stream>>>(c->P, dU, c->A, c->nvar, 0, 0.0);
+  k_pack<<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, dT, c->P.T, 1, 0, 1000.0);
+  c->launches += 2;
+  CK(cudaMemsetAsync(c->P.flag, 0, 4, c->stream));
+  CK(cudaMemsetAsync(c->P.slots, 0, 36 * 8, c->stream));
+  CK(cudaMemsetAsync(c->P.scal, 0, 4 * 8, c->stream));
+  c->parity = 0;
+  CK(cudaGetLastError());
+  if (!on_device) CK(cudaStreamSynchronize(c->stream));   // host buffers may be reused by the caller
+  c->have_state = true;
+  return JANC_OK;
+}
+
+static int read_flag(janc_ctx *c) {
+  int flag = 0;
+  CK(cudaMemcpyAsync(&flag, c->P.flag, 4, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  CK(cudaGetLastError());
+  return flag ? JANC_ENONFINITE : JANC_OK;
+}
+
+extern "C" int janc_status(janc_ctx *c) {
+  if (!c) return JANC_EINVAL;
+  if (!c->have_ws) return JANC_ESTATE;
+  return read_flag(c);
+}
+
+extern "C" int janc_get_state(janc_ctx *c, double *U, double *T, int on_device) {
+  if (!c) return JANC_EINVAL;
+  if (!c->have_state) { c->err = "no state"; return JANC_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  const size_t nU = (size_t)c->np * c->nvar * c->ncell, nT = (size_t)c->np * c->ncell;
+  if (U) {
+    double *dst = on_device ? U : c->stageU;
+    k_pack<<<cell_grid(c, 256, c->np * c->nvar), 256, 0, c->stream>>>(c->P, c->A, dst, c->nvar, 1, 0.0);
+    c->launches++;
+    if (!on_device) CK(cudaMemcpyAsync(U, c->stageU, nU * 8, cudaMemcpyDeviceToHost, c->stream));
+  }
+  if (T) {
+    double *dst = on_device ? T : c->stageT;
+    k_pack<<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, c->P.T, dst, 1, 1, 0.0);
+    c->launches++;
+    if (!on_device) CK(cudaMemcpyAsync(T, c->stageT, nT * 8, cudaMemcpyDeviceToHost, c->stream));
+  }
+  return read_flag(c);
+}
+
+// ------------------------------------------------------------------ the step
+struct Prof {                       // optional per-phase timing of one step (CUDA events on the stream)
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> phase;
+};
+
+static void prof_mark(janc_ctx *c, Prof *pf, int phase) {
+  if (!pf) return;
+  cudaEvent_t e;
+  cudaEventCreate(&e);
+  cudaEventRecord(e, c->stream);
+  pf->ev.push_back(e);
+  pf->phase.push_back(phase);
+}
+
+template <int NS>
+static void launch_prim(janc_ctx *c, const double *U, int reduce, int slot_base, double *dbgc) {
+  k_prim<NS><<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, U, reduce, slot_base, dbgc);
+}
+static void do_prim(janc_ctx *c, const double *U, int reduce, int slot_base, double *dbgc, Prof *pf) {
+  switch (c->ns) {
+    case 1: launch_prim<1>(c, U, reduce, slot_base, dbgc); break;
+    case 2: launch_prim<2>(c, U, reduce, slot_base, dbgc); break;
+    case 9: launch_prim<9>(c, U, reduce, slot_base, dbgc); break;
+    case 20: launch_prim<20>(c, U, reduce, slot_base, dbgc); break;
+    default: launch_prim<0>(c, U, reduce, slot_base, dbgc); break;
+  }
+  c->launches++;
+  prof_mark(c, pf, 0);
+}
+
+static void do_ghost(janc_ctx *c, double *U, Prof *pf) {
+  const int nd = c->g.ndim;
+  int amax = 1;
+  for (int d = 0; d < nd; d++) {
+    int a = 1;
+    for (int e = 0; e < nd; e++) if (e != d) a *= c->P.n[e];
+    if (a > amax) amax = a;
+  }
+  const long long total = (long long)2 * nd * JANC_NG * amax;
+  dim3 grid((unsigned)((total + 255) / 256), (unsigned)c->np, 1);
+  for (int lev = 0; lev < c->g.n_levels; lev++) {
+    k_ghost<<<grid, 256, 0, c->stream>>>(c->P, U, lev, amax);
+    c->launches++;
+  }
+  prof_mark(c, pf, 1);
+}
+
+static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef, Prof *pf) {
+  const Params &P = c->P;
+  if (c->g.ndim == 1) {
+    constexpr int TX = 256;
+    dim3 grid((unsigned)((P.n[0] + TX - 1) / TX), (unsigned)c->np, 1);
+    k_flux_rk<1, TX, 1, 1, 256><<<grid, 256, 0, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
+  } else if (c->g.ndim == 2) {
+    constexpr int TX = 32, TY = 16;
+    dim3 grid((unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY)), (unsigned)c->np, 1);
+    k_flux_rk<2, TX, TY, 1, 512><<<grid, 512, 0, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
+  } else {
+    constexpr int TX = 16, TY = 8, TZ = 8;
+    dim3 grid((unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY) * ((P.n[2] + TZ - 1) / TZ)), (unsigned)c->np, 1);
+    k_flux_rk<3, TX, TY, TZ, 512><<<grid, 512, 0, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
+  }
+  c->launches++;
+  prof_mark(c, pf, 2);
+}
+
+template <int NS>
+static void launch_chem(janc_ctx *c, double *U) {
+  k_chem<NS><<<cell_grid(c, 128, c->np), 128, 0, c->stream>>>(c->P, U);
+}
+static void do_chem(janc_ctx *c, double *U, Prof *pf) {
+  switch (c->ns) {
+    case 2: launch_chem<2>(c, U); break;
+    case 9: launch_chem<9>(c, U); break;
+    case 20: launch_chem<20>(c, U); break;
+    default: launch_chem<0>(c, U); break;
+  }
+  c->launches++;
+  prof_mark(c, pf, 3);
+}
+
+// advance_one_step: cfl -> advance_flux (RK3 over rhs) -> advance_source_term
+static void step_once(janc_ctx *c, double cfl, double dt_fixed, int flags, Prof *pf) {
+  const int par = c->parity;
+  prof_mark(c, pf, -1);
+  // stage 0: update_aux on U^n (also the cfl() evaluation), dt, ghost fill, fluxes
+  do_prim(c, c->A, 1, SLOT(par, 0, 0, 0), nullptr, pf);
+  k_dt<<<1, 32, 0, c->stream>>>(c->P, par, cfl, dt_fixed);
+  c->launches++;
+  prof_mark(c, pf, 0);
+  do_ghost(c, c->A, pf);
+  do_flux(c, c->A, c->A, c->B, SLOT(par, 0, 0, 0), 1.0, pf);
+  // stage 1
+  do_prim(c, c->B, 1, SLOT(par, 1, 0, 0), nullptr, pf);
+  do_ghost(c, c->B, pf);
+  do_flux(c, c->B, c->A, c->C, SLOT(par, 1, 0, 0), 0.25, pf);
+  // stage 2 (writes U* over U^n in place: each cell reads its own U^n before writing)
+  do_prim(c, c->C, 1, SLOT(par, 2, 0, 0), nullptr, pf);
+  do_ghost(c, c->C, pf);
+  do_flux(c, c->C, c->A, c->A, SLOT(par, 2, 0, 0), 2.0 / 3.0, pf);
+  // advance_source_term: T* inside the chemistry kernel; explicit variant: only refresh aux
+  const bool chem = !(flags & 1) && c->ns > 1 && c->nr > 0;
+  if (chem) do_chem(c, c->A, pf);
+  else do_prim(c, c->A, 0, 0, nullptr, pf);
+  if (c->g.n_levels > 1) {
+    const int r = c->g.ratio, nd = c->g.ndim;
+    long long nc = c->ncell;
+    for (int d = 0; d < nd; d++) nc /= r;
+    dim3 grid((unsigned)((nc * c->nvar + 255) / 256), (unsigned)c->np, 1);
+    k_average_down<<<grid, 256, 0, c->stream>>>(c->P, c->A);
+    c->launches++;
+    prof_mark(c, pf, 4);
+  }
+  c->parity = 1 - par;
+}
+
+static int check_ready(janc_ctx *c) {
+  if (!c) return JANC_EINVAL;
+  if (!c->have_state) { c->err = "no state"; return JANC_ESTATE; }
+  if (c->g.n_patches > 0 && !c->have_blocks) { c->err = "block mode needs janc_set_blocks"; return JANC_ESTATE; }
+  return JANC_OK;
+}
+
+extern "C" int janc_step(janc_ctx *c, int nsteps, double cfl, double dt_fixed, int flags, double *t_advanced) {
+  int rc = check_ready(c);
+  if (rc) return rc;
+  if (nsteps < 0 || (!(cfl > 0.0) && !(dt_fixed > 0.0))) { c->err = "need cfl > 0 or dt_fixed > 0"; return JANC_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  rc = upload_mech(c);
+  if (rc) return rc;
+  double t0 = 0.0;
+  if (t_advanced) {
+    CK(cudaMemcpyAsync(&t0, c->P.scal + 1, 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+  }
+  for (int s = 0; s < nsteps; s++) step_once(c, cfl, dt_fixed, flags, nullptr);
+  CK(cudaGetLastError());
+  if (t_advanced) {
+    double t1 = 0.0;
+    CK(cudaMemcpyAsync(&t1, c->P.scal + 1, 8, cudaMemcpyDeviceToHost, c->stream));
+    rc = read_flag(c);
+    *t_advanced = t1 - t0;
+    return rc;
+  }
+  return JANC_OK;
+}
+
+extern "C" int janc_profile_step(janc_ctx *c, double cfl, double dt_fixed, float *ms_out, int *n_out) {
+  int rc = check_ready(c);
+  if (rc) return rc;
+  if (!ms_out) return JANC_EINVAL;
+  CK(cudaSetDevice(c->device));
+  rc = upload_mech(c);
+  if (rc) return rc;
+  Prof pf;
+  step_once(c, cfl, dt_fixed, 0, &pf);
+  CK(cudaStreamSynchronize(c->stream));
+  for (int q = 0; q < 6; q++) { ms_out[q] = 0.f; if (n_out) n_out[q] = 0; }
+  for (size_t e = 1; e < pf.ev.size(); e++) {
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, pf.ev[e - 1], pf.ev[e]);
+    ms_out[pf.phase[e]] += ms;
+    if (n_out) n_out[pf.phase[e]]++;
+  }
+  float tot = 0.f;
+  cudaEventElapsedTime(&tot, pf.ev.front(), pf.ev.back());
+  ms_out[5] = tot;
+  if (n_out) n_out[5] = (int)pf.ev.size() - 1;
+  for (auto e : pf.ev) cudaEventDestroy(e);
+  return read_flag(c);
+}
+
+extern "C" int janc_debug_cons2prim(janc_ctx *c, double *T, double *p, double *cs, int on_device) {
+  int rc = check_ready(c);
+  if (rc) return rc;
+  CK(cudaSetDevice(c->device));
+  rc = upload_mech(c);
+  if (rc) return rc;
+  do_prim(c, c->A, 0, 0, c->dbgc, nullptr);
+  const size_t nT = (size_t)c->np * c->ncell;
+  double *srcs[3] = {c->P.T, c->P.p, c->dbgc};
+  double *dsts[3] = {T, p, cs};
+  for (int q = 0; q < 3; q++) {
+    if (!dsts[q]) continue;
+    double *dst = on_device ? dsts[q] : c->stageT;
+    k_pack<<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, srcs[q], dst, 1, 1, 0.0);
+    c->launches++;
+    if (!on_device) {
+      CK(cudaMemcpyAsync(dsts[q], c->stageT, nT * 8, cudaMemcpyDeviceToHost, c->stream));
+      CK(cudaStreamSynchronize(c->stream));
+    }
+  }
+  return read_flag(c);
+}
+
+extern "C" int janc_measure_dfma_peak(int device, void *cuda_stream, double *dfma_per_s) {
+  if (!dfma_per_s) return JANC_EINVAL;
+  if (cudaSetDevice(device) != cudaSuccess) return JANC_ECUDA;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return JANC_ECUDA;
+  double *d = nullptr;
+  if (cudaMalloc(&d, 64) != cudaSuccess) return JANC_ECUDA;
+  const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 4096;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  double best = 0.0;
+  for (int rep = 0; rep < 6; rep++) {
+    cudaEventRecord(e0, st);
+    k_dfma<<<blocks, threads, 0, st>>>(d, iters);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return JANC_ECUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    double rate = (double)blocks * threads * iters * 64.0 / (ms * 1e-3);
+    if (rep > 0 && rate > best) best = rate;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  *dfma_per_s = best;
+  return JANC_OK;
+}
