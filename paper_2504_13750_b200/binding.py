@@ -1,0 +1,225 @@
+"""Thin ctypes binding of libjanc.so (include/janc.h): argument marshalling only.
+
+PyTorch supplies device memory (the workspace, device-resident state tensors) and the CUDA
+stream; every step of the path runs in the library's kernels.  There is no CPU fallback: if the
+library is missing, or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libjanc.so")
+_lib = None
+
+JANC_OK, JANC_EINVAL, JANC_ENOMEM, JANC_ECUDA, JANC_ESTATE, JANC_ENONFINITE = 0, -1, -2, -3, -4, -5
+FLAG_NO_CHEM = 1
+
+EXPORTS = ["janc_create", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
+           "janc_set_blocks", "janc_set_state", "janc_step", "janc_get_state", "janc_status",
+           "janc_launch_count", "janc_debug_cons2prim", "janc_profile_step",
+           "janc_measure_dfma_peak", "janc_last_error", "janc_destroy"]
+
+
+class JancError(RuntimeError):
+    def __init__(self, code, msg=""):
+        super().__init__(f"libjanc error {code}: {msg}")
+        self.code = code
+
+
+class _Grid(C.Structure):
+    _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("dx", C.c_double * 3),
+                ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3),
+                ("n_patches", C.c_int), ("n_levels", C.c_int), ("ratio", C.c_int)]
+
+
+class _Mech(C.Structure):
+    _fields_ = [("ns", C.c_int), ("nr", C.c_int),
+                ("W", C.c_void_p), ("nasa", C.c_void_p), ("nu_f", C.c_void_p), ("nu_b", C.c_void_p),
+                ("A", C.c_void_p), ("b", C.c_void_p), ("Ta", C.c_void_p),
+                ("reversible", C.c_void_p), ("third_body", C.c_void_p), ("eff", C.c_void_p)]
+
+
+def lib():
+    """Load libjanc.so (built in-tree by paper_2504_13750_b200.build); fail loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2504_13750_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.janc_workspace_bytes.restype = C.c_size_t
+        L.janc_workspace_bytes.argtypes = [C.c_void_p]
+        L.janc_bind_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
+        L.janc_create.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.janc_set_mechanism.argtypes = [C.c_void_p, C.c_void_p]
+        L.janc_set_blocks.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.janc_set_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.janc_step.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int, C.c_void_p]
+        L.janc_get_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.janc_status.argtypes = [C.c_void_p]
+        L.janc_launch_count.argtypes = [C.c_void_p]
+        L.janc_launch_count.restype = C.c_longlong
+        L.janc_debug_cons2prim.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.janc_profile_step.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
+        L.janc_measure_dfma_peak.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
+        L.janc_last_error.argtypes = [C.c_void_p]
+        L.janc_last_error.restype = C.c_char_p
+        L.janc_destroy.argtypes = [C.c_void_p]
+        L.janc_destroy.restype = None
+        _lib = L
+    return _lib
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def measure_dfma_peak(device=0, stream=None):
+    out = C.c_double(0.0)
+    rc = lib().janc_measure_dfma_peak(int(device), C.c_void_p(stream or 0), C.byref(out))
+    if rc:
+        raise JancError(rc, "janc_measure_dfma_peak")
+    return out.value
+
+
+class Solver:
+    """janc_* context: create -> set_mechanism -> bind_workspace (torch) -> [set_blocks] -> set_state
+    -> step -> get_state -> destroy.  Same call names as the C ABI."""
+
+    def __init__(self, grid, mech, blocks=None, device=0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise JancError(JANC_ECUDA, "no CUDA device (libjanc has no CPU fallback)")
+        L = lib()
+        self._torch = torch
+        self.device = int(device)
+        torch.cuda.set_device(self.device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        g = _Grid(grid.ndim, (C.c_int * 3)(*grid.n), (C.c_double * 3)(*grid.dx),
+                  (C.c_int * 3)(*grid.bc_lo), (C.c_int * 3)(*grid.bc_hi),
+                  grid.n_patches, grid.n_levels, grid.ratio)
+        self._h = C.c_void_p()
+        rc = L.janc_create(C.byref(g), self.device, C.c_void_p(stream.cuda_stream), C.byref(self._h))
+        if rc:
+            raise JancError(rc, "janc_create")
+        self._keep = dict(W=_f64(mech.W), nasa=_f64(mech.nasa), nu_f=_i32(mech.nu_f), nu_b=_i32(mech.nu_b),
+                          A=_f64(mech.A), b=_f64(mech.b), Ta=_f64(mech.Ta), reversible=_i32(mech.reversible),
+                          third_body=_i32(mech.third_body), eff=_f64(mech.eff))
+        m = _Mech(mech.ns, mech.nr, *[_ptr(self._keep[k]) for k in
+                                      ("W", "nasa", "nu_f", "nu_b", "A", "b", "Ta", "reversible", "third_body", "eff")])
+        self._check(L.janc_set_mechanism(self._h, C.byref(m)), "janc_set_mechanism")
+        nbytes = L.janc_workspace_bytes(self._h)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{self.device}")
+        base = (self.workspace.data_ptr() + 255) // 256 * 256
+        self._check(L.janc_bind_workspace(self._h, C.c_void_p(base), nbytes), "janc_bind_workspace")
+        if blocks is not None:
+            self._check(L.janc_set_blocks(self._h, _ptr(_i32(blocks.level)), _ptr(_i32(blocks.nbr)),
+                                          _ptr(_i32(blocks.parent))), "janc_set_blocks")
+        self.np_ = max(1, grid.n_patches)
+        self.nvar = grid.ndim + 2 + mech.ns - 1
+        self.shape = (self.np_, self.nvar, grid.n[2] if grid.ndim > 2 else 1,
+                      grid.n[1] if grid.ndim > 1 else 1, grid.n[0])
+        self.tshape = (self.shape[0],) + self.shape[2:]
+
+    def _check(self, rc, what):
+        if rc:
+            msg = lib().janc_last_error(self._h)
+            raise JancError(rc, f"{what}: {msg.decode() if msg else ''}")
+
+    # -- state ------------------------------------------------------------------------------
+    def set_state(self, U, T=None):
+        """U, T: numpy arrays (host) or torch CUDA tensors (device), interior layout."""
+        torch = self._torch
+        if isinstance(U, torch.Tensor):
+            assert U.is_cuda and U.dtype == torch.float64 and U.is_contiguous() and U.numel() == int(np.prod(self.shape))
+            Tp = None
+            if T is not None:
+                assert T.is_cuda and T.dtype == torch.float64 and T.is_contiguous()
+                Tp = C.c_void_p(T.data_ptr())
+            self._check(lib().janc_set_state(self._h, C.c_void_p(U.data_ptr()), Tp, 1), "janc_set_state")
+        else:
+            U = _f64(U)
+            assert U.size == int(np.prod(self.shape)), (U.shape, self.shape)
+            Tn = _f64(T) if T is not None else None
+            self._check(lib().janc_set_state(self._h, _ptr(U), _ptr(Tn) if Tn is not None else None, 0),
+                        "janc_set_state")
+
+    def step(self, nsteps, cfl=0.0, dt=0.0, chem=True, sync=True):
+        """Returns the time advanced (sync=True) or None (asynchronous enqueue)."""
+        flags = 0 if chem else FLAG_NO_CHEM
+        if sync:
+            t = C.c_double(0.0)
+            rc = lib().janc_step(self._h, int(nsteps), float(cfl), float(dt), flags, C.byref(t))
+            self.status = rc
+            if rc not in (JANC_OK, JANC_ENONFINITE):
+                self._check(rc, "janc_step")
+            return t.value
+        self._check(lib().janc_step(self._h, int(nsteps), float(cfl), float(dt), flags, None), "janc_step")
+        return None
+
+    def get_state(self, device=False):
+        if device:
+            torch = self._torch
+            U = torch.empty(self.shape, dtype=torch.float64, device=f"cuda:{self.device}")
+            T = torch.empty(self.tshape, dtype=torch.float64, device=f"cuda:{self.device}")
+            rc = lib().janc_get_state(self._h, C.c_void_p(U.data_ptr()), C.c_void_p(T.data_ptr()), 1)
+        else:
+            U = np.empty(self.shape); T = np.empty(self.tshape)
+            rc = lib().janc_get_state(self._h, _ptr(U), _ptr(T), 0)
+        self.status = rc
+        if rc not in (JANC_OK, JANC_ENONFINITE):
+            self._check(rc, "janc_get_state")
+        return U, T
+
+    def get_state_into(self, U_host):
+        """Device -> caller's (pinned) host array; returns status."""
+        rc = lib().janc_get_state(self._h, _ptr(U_host), None, 0)
+        self.status = rc
+        return rc
+
+    def status_sync(self):
+        return lib().janc_status(self._h)
+
+    def launch_count(self):
+        return lib().janc_launch_count(self._h)
+
+    def debug_cons2prim(self):
+        T = np.empty(self.tshape); p = np.empty(self.tshape); c = np.empty(self.tshape)
+        rc = lib().janc_debug_cons2prim(self._h, _ptr(T), _ptr(p), _ptr(c), 0)
+        if rc not in (JANC_OK, JANC_ENONFINITE):
+            self._check(rc, "janc_debug_cons2prim")
+        return T, p, c
+
+    def profile_step(self, cfl=0.0, dt=0.0):
+        ms = (C.c_float * 6)(); n = (C.c_int * 6)()
+        rc = lib().janc_profile_step(self._h, float(cfl), float(dt), ms, n)
+        if rc not in (JANC_OK, JANC_ENONFINITE):
+            self._check(rc, "janc_profile_step")
+        names = ["cons2prim", "ghost", "flux_rk", "chem", "average_down", "step"]
+        return {k: (ms[i], n[i]) for i, k in enumerate(names)}
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().janc_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

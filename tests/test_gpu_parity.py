@@ -1,0 +1,231 @@
+"""GPU parity: libjanc (through the C ABI binding) vs the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's: <= 1e-10 relative L-inf per field after one
+step, <= 1e-6 after 100 steps (fp64).  Run with -m gpu on a B200."""
+import numpy as np
+import pytest
+
+from paper_2504_13750_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+TOL1, TOL100 = 1e-10, 1e-6
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2504_13750_b200 import binding, build
+    build.build()
+    binding.lib()
+    return binding
+
+
+def field_errors(case, Ug, Ur):
+    """relative L-inf per conserved field; momentum components share one scale."""
+    nd = case.grid.ndim
+    errs = []
+    mom_scale = max(np.abs(Ur[:, 1:1 + nd]).max(), 1e-300)
+    rho_c = np.abs(Ur[:, 0]).max() * np.sqrt(np.abs(Ur[:, nd + 1]).max() / np.abs(Ur[:, 0]).max())
+    mom_scale = max(mom_scale, 1e-3 * rho_c)
+    for v in range(Ur.shape[1]):
+        if 1 <= v <= nd:
+            scale = mom_scale
+        elif v > nd + 1:
+            scale = max(np.abs(Ur[:, v]).max(), 1e-6 * np.abs(Ur[:, 0]).max())   # species vs density
+        else:
+            scale = np.abs(Ur[:, v]).max()
+        errs.append(np.abs(Ug[:, v] - Ur[:, v]).max() / scale)
+    return np.array(errs)
+
+
+def both(B, ref, case, nsteps, chem=True, cfl=None, dt=0.0):
+    cfl = case.cfl if cfl is None else cfl
+    g = B.Solver(case.grid, case.mech, case.blocks)
+    g.set_state(case.U, case.T)
+    tg = g.step(nsteps, cfl=cfl, dt=dt, chem=chem)
+    Ug, Tg = g.get_state()
+    assert g.status == 0, "device flag raised"
+    g.close()
+    r = ref.RefSolver(case.grid, case.mech, case.blocks)
+    r.set_state(case.U, case.T)
+    tr = r.step(nsteps, cfl=cfl, dt=dt, chem=chem)
+    Ur, Tr = r.get_state()
+    assert r.status == 0
+    assert abs(tg - tr) <= 1e-12 * tr, (tg, tr)
+    return Ug, Tg, Ur, Tr
+
+
+def check(B, ref, case, nsteps, tol, **kw):
+    Ug, Tg, Ur, Tr = both(B, ref, case, nsteps, **kw)
+    e = field_errors(case, Ug, Ur)
+    assert e.max() <= tol, (case.name, nsteps, e)
+    assert np.abs(Tg - Tr).max() <= max(tol, 1e-11) * np.abs(Tr).max()
+    assert np.abs(Ug - case.U).max() > 0          # something happened
+    return e
+
+
+# ------------------------------------------------------------------ cons->prim kernel alone
+def test_cons2prim_kernel(B, ref, mech9):
+    case = I.config1(nx=70, ny=20)
+    g = B.Solver(case.grid, case.mech)
+    g.set_state(case.U, np.full_like(case.T, 900.0))
+    T, p, c = g.debug_cons2prim()
+    g.close()
+    for (j, i) in [(0, 0), (3, 2), (19, 69), (7, 33), (12, 5)]:
+        rc, out = ref.cons2prim(mech9, 2, case.U[0, :, 0, j, i], 900.0)
+        assert rc == 0
+        assert abs(T[0, 0, j, i] - out[0]) <= 1e-12 * out[0]
+        assert abs(p[0, 0, j, i] - out[1]) <= 1e-12 * out[1]
+        assert abs(c[0, 0, j, i] - out[3]) <= 1e-12 * out[3]
+    assert np.abs(T - case.T).max() <= 1e-9 * case.T.max()
+
+
+# ------------------------------------------------------------------ config 0 (1-D, 2 species)
+def test_cfg0_one_step(B, ref):
+    check(B, ref, I.config0(), 1, TOL1)
+
+
+def test_cfg0_full_200_steps(B, ref):
+    check(B, ref, I.config0(), 200, TOL100)
+
+
+def test_cfg0_ragged_and_tiny(B, ref):
+    check(B, ref, I.config0(n=300), 1, TOL1)      # tile of 256 + ragged tail
+    check(B, ref, I.config0(n=7), 3, TOL1 * 10)   # smaller than the stencil's reach into ghosts
+
+
+def test_sod_inert_single_species(B, ref):
+    from tests.test_oracle_pins import _sod_case
+    case, x = _sod_case(400)
+    check(B, ref, case, 1, TOL1, chem=False)
+    check(B, ref, case, 100, TOL100, chem=False)
+
+
+# ------------------------------------------------------------------ configs 1, 2 (2-D, 9 species)
+def test_cfg1_scaled_one_step_and_100(B, ref):
+    case = I.config1(nx=100, ny=40)               # 4 x 3 tiles of 32x16, ragged in both directions
+    check(B, ref, case, 1, TOL1)
+    check(B, ref, case, 100, TOL100)
+
+
+def test_cfg2_scaled_outflow(B, ref):
+    case = I.config2(nx=160, ny=48)
+    check(B, ref, case, 1, TOL1)
+    check(B, ref, case, 30, TOL100)
+
+
+def test_periodic_2d_smooth(B, ref, mech9):
+    from tests.test_oracle_pins import _random_smooth_2d
+    case = _random_smooth_2d(mech9, 48, 40, 3, I.BC_PERIODIC)
+    check(B, ref, case, 1, TOL1)
+    check(B, ref, case, 10, TOL100)
+    check(B, ref, case, 2, TOL1 * 10, cfl=0.0, dt=1.5e-9)     # fixed-dt mode
+
+
+def test_explicit_variant_no_chem(B, ref):
+    case = I.config1(nx=64, ny=32)
+    check(B, ref, case, 5, TOL100, chem=False)
+
+
+# ------------------------------------------------------------------ config 3 (block list, 2 levels)
+def test_cfg3_scaled_block_list(B, ref):
+    case = I.config3(pcols=16, prows=8, npc=16)
+    assert case.blocks.level.sum() > 0
+    check(B, ref, case, 1, TOL1)
+    check(B, ref, case, 10, TOL100)
+
+
+def test_block_tiling_equals_uniform_on_gpu(B, ref, mech9):
+    from tests.test_oracle_pins import _random_smooth_2d
+    case = _random_smooth_2d(mech9, 32, 32, 8, I.BC_REFLECT)
+    g = B.Solver(case.grid, case.mech); g.set_state(case.U, case.T); g.step(3, cfl=case.cfl); U1, _ = g.get_state(); g.close()
+    tiled = I.tile_uniform(case, 16, 16)
+    g = B.Solver(tiled.grid, tiled.mech, tiled.blocks); g.set_state(tiled.U, tiled.T); g.step(3, cfl=case.cfl)
+    U2, _ = g.get_state(); g.close()
+    U2 = I.untile(tiled, U2, 2, 2)
+    assert np.abs(U1 - U2).max() <= 1e-12 * np.abs(U1).max()
+
+
+# ------------------------------------------------------------------ config 4 (3-D, 20 species)
+def test_cfg4_scaled_3d(B, ref):
+    case = I.config4(n=24, nspheres=3, radius=5)
+    check(B, ref, case, 1, TOL1)
+    check(B, ref, case, 5, TOL100)
+
+
+def test_3d_ragged_nonperiodic(B, ref):
+    c1 = I.config4(n=20, nspheres=2, radius=4)
+    g = c1.grid
+    U = c1.U[:, :, :18, :13, :].copy(); T = c1.T[:, :18, :13, :].copy()
+    g2 = I.Grid(3, (20, 13, 18), g.dx, (I.BC_REFLECT, I.BC_OUTFLOW, I.BC_PERIODIC), (I.BC_OUTFLOW, I.BC_REFLECT, I.BC_PERIODIC))
+    check(B, ref, I.Case("3d_ragged", g2, c1.mech, U, T, 0.2, 2), 2, TOL1 * 10)
+
+
+# ------------------------------------------------------------------ generic species count (run-time ns path)
+def test_generic_ns_path(B, ref):
+    m2 = I.single_step_mechanism()
+    W = np.array([0.029, 0.029, 0.040]); nasa = np.zeros((3, 7)); nasa[:, 0] = [3.5, 3.5, 2.5]; nasa[0, 5] = m2.nasa[0, 5]
+    m3 = I.Mechanism(3, 1, W, nasa, np.array([[1, 0, 0]], dtype=np.int32), np.array([[0, 1, 0]], dtype=np.int32),
+                     m2.A, m2.b, np.array([8000.0]), np.array([1], dtype=np.int32), np.array([1], dtype=np.int32),
+                     np.array([[1.0, 2.0, 0.5]]))
+    n = 96
+    x = np.arange(n)
+    p = np.where(x < 48, 8e5, 1e5); T = np.where(x < 48, 1800.0, 400.0)
+    Y = np.zeros((n, 3)); Y[:, 0] = 0.6; Y[:, 1] = 0.1; Y[:, 2] = 0.3
+    U = I.prim_to_cons(m3, 1, p, T, Y, [np.zeros(n)])
+    g = I.Grid(1, (n, 1, 1), (1e-4, 1, 1), (I.BC_REFLECT, 0, 0), (I.BC_OUTFLOW, 0, 0))
+    case = I.Case("ns3", g, m3, U.reshape(1, 5, 1, 1, n), T.reshape(1, 1, 1, n).astype(float), 0.3, 10)
+    check(B, ref, case, 1, TOL1)
+    check(B, ref, case, 10, TOL100)
+
+
+# ------------------------------------------------------------------ invariants on the GPU path itself
+def test_uniform_state_bitwise_on_gpu(B, mech9):
+    nx, ny = 70, 37
+    Y = I.hot_Y(9); z = np.zeros((ny, nx))
+    U = I.prim_to_cons(mech9, 2, z + 2.5e5, z + 1234.5, np.broadcast_to(Y, (ny, nx, 9)), [z + 310.0, z - 95.0])
+    U = np.broadcast_to(U[:, :1, :1], U.shape).copy()
+    g = I.Grid(2, (nx, ny, 1), (1e-4, 2e-4, 1), (0, 0, 0), (0, 0, 0))
+    s = B.Solver(g, mech9); s.set_state(U.reshape(1, -1, 1, ny, nx), np.full((1, 1, ny, nx), 1234.5))
+    s.step(5, cfl=0.4, chem=False)
+    U1, _ = s.get_state(); s.close()
+    assert np.array_equal(U1.reshape(U.shape), U)
+
+
+def test_device_resident_state_and_async(B, ref):
+    import torch
+    case = I.config1(nx=64, ny=32)
+    s = B.Solver(case.grid, case.mech)
+    Ud = torch.from_numpy(case.U).cuda(); Td = torch.from_numpy(case.T).cuda()
+    s.set_state(Ud, Td)
+    s.step(2, cfl=case.cfl, sync=False)
+    U1, T1 = s.get_state(device=True)
+    s2 = B.Solver(case.grid, case.mech); s2.set_state(case.U, case.T); s2.step(2, cfl=case.cfl); U2, _ = s2.get_state()
+    assert np.array_equal(U1.cpu().numpy(), U2)
+    assert s.launch_count() > 20
+    s.close(); s2.close()
+
+
+def test_error_flag_and_arguments(B):
+    case = I.config0(n=64)
+    s = B.Solver(case.grid, case.mech)
+    with pytest.raises(B.JancError):
+        s.step(1, cfl=0.0, dt=0.0)                 # neither cfl nor dt
+    U = case.U.copy(); U[0, 2, 0, 0, 10] = -1e9    # negative energy => T <= 0 => device flag
+    s.set_state(U, case.T)
+    s.step(1, cfl=0.4)
+    assert s.status == B.JANC_ENONFINITE
+    s.set_state(case.U, case.T)                    # flag is cleared by set_state
+    s.step(1, cfl=0.4)
+    assert s.status == 0
+    s.close()
+
+
+# ------------------------------------------------------------------ full-size bench workload (config 2)
+def test_cfg2_full_size_one_step(B, ref):
+    """The configuration bench.py times (4096 x 512, 9 species): one full step against the oracle."""
+    case = I.config2()
+    e = check(B, ref, case, 1, TOL1)
+    print("cfg2 full-size per-field rel err", e)
