@@ -105,3 +105,190 @@ def oracle_throughput(case, budget_s=15.0):
     s.close()
     return {"value": cells * n / tn, "unit": UNIT, "cores": ref.threads(), "kind": "oracle",
             "sample": f"{desc}, {n} steps after 1 warm-up, {tn:.1f} s"}, cells, tn / n
+
+
+# ------------------------------------------------------------------------------------------------
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle as it stands on a bounded sample per step (tier contract)."""
+    if rank != 0:
+        return
+    case = make_case(args.workload)
+    from oracle import ref
+    ref.build()
+    g = case.grid
+    if g.n_patches == 0 and g.ndim == 2:
+        nx, ny = min(g.n[0], 512), min(g.n[1], 128)
+        U = np.ascontiguousarray(case.U[:, :, :, :ny, :nx]); T = np.ascontiguousarray(case.T[:, :, :ny, :nx])
+        crop = I.Case(case.name + "_crop", I.Grid(2, (nx, ny, 1), g.dx, g.bc_lo, g.bc_hi), case.mech, U, T, case.cfl, 1)
+        desc = f"{case.name} cropped to {nx}x{ny} cells per step"
+    elif g.n_patches == 0 and g.ndim == 3:
+        n = min(g.n[0], 32)
+        U = np.ascontiguousarray(case.U[:, :, :n, :n, :n]); T = np.ascontiguousarray(case.T[:, :n, :n, :n])
+        crop = I.Case(case.name + "_crop", I.Grid(3, (n, n, n), g.dx, g.bc_lo, g.bc_hi), case.mech, U, T, case.cfl, 1)
+        desc = f"{case.name} cropped to {n}^3 cells per step"
+    else:
+        crop, desc = case, f"{case.name} (whole)"
+    s = ref.RefSolver(crop.grid, crop.mech, crop.blocks)
+    s.set_state(crop.U, crop.T)
+    for _ in range(args.warmup):
+        s.step(1, cfl=crop.cfl)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        s.step(1, cfl=crop.cfl)
+    dt = time.perf_counter() - t0
+    s.close()
+    val = crop.cells * args.steps / dt
+    cores = ref.threads()
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": case.name, "cells": case.cells, "ns": case.mech.ns, "nr": case.mech.nr,
+                       "sample": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2504_13750_b200 import binding, build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libjanc has no CPU fallback")
+    if rank == 0:
+        build.build()
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        dist.barrier()
+    binding.lib()
+
+    # replicas only (DESIGN.md "Multi-GPU"): every rank advances its own independent problem
+    case = make_case(args.workload, rank)
+    cells = case.cells
+    K, W = args.steps, max(args.warmup, 3)
+    s = binding.Solver(case.grid, case.mech, case.blocks, device=local)
+    dev = f"cuda:{local}"
+    Ud = torch.from_numpy(case.U).to(dev); Td = torch.from_numpy(case.T).to(dev)
+    s.set_state(Ud, Td)
+    for _ in range(W):
+        s.step(1, cfl=case.cfl, sync=False)
+    assert s.status_sync() == 0, "device flag raised during warm-up"
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    # ---- timed region 1: device-resident (inputs already in HBM)
+    l0 = s.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(K):
+        s.step(1, cfl=case.cfl, sync=False)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = s.launch_count() - l0
+    assert s.status_sync() == 0, "device flag raised during the timed region"
+
+    # ---- per-kernel-phase device time over K more steps (CUDA events on the library's stream)
+    phases = {}
+    for _ in range(K):
+        pr = s.profile_step(cfl=case.cfl)
+        for k, (t, n) in pr.items():
+            a = phases.setdefault(k, [0.0, 0]); a[0] += t; a[1] += n
+    if sampler:
+        sampler.stop_flag = True
+        sampler.join()
+
+    # ---- timed region 2: end to end through the C ABI with HOST buffers (pinned), copies inside
+    Uh = torch.from_numpy(case.U).pin_memory(); Th = torch.from_numpy(case.T).pin_memory()
+    Uo = torch.empty_like(Uh).pin_memory()
+    Ke = max(1, min(K, 5))
+    s.set_state(Uh.numpy(), Th.numpy()); s.step(1, cfl=case.cfl, sync=False); s.get_state_into(Uo.numpy())
+    barrier()
+    e0.record()
+    for _ in range(Ke):
+        s.set_state(Uh.numpy(), Th.numpy())
+        s.step(1, cfl=case.cfl, sync=False)
+        rc = s.get_state_into(Uo.numpy())
+    e1.record()
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    assert rc == 0
+
+    t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, ms_e2e = float(t[0]), float(t[1])
+    s.close()
+
+    if rank == 0:
+        g = case.grid
+        nd, nvar = g.ndim, case.nvar
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        hbm_peak = peaks.get("hbm_gbs", 6650.0)
+        hbm_src = "measured (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback"
+        dfma = binding.measure_dfma_peak(local)                      # DP instructions/s, measured now
+        # dominant kernel: the fused flux+divergence+RK kernel, 3 launches per step
+        fl_ms, fl_n = phases["flux_rk"]
+        fl_avg = fl_ms / max(fl_n, 1) * 1e-3
+        ops = flux_ops_per_cell_stage(nd, nvar) * cells
+        byt = flux_bytes_per_cell_stage(nd, nvar) * cells
+        roof = {"kernel": "k_flux_rk", "bound": "alu", "achieved": ops / fl_avg / 1e12, "peak": dfma / 1e12,
+                "unit": "T fp64-instr/s (FMA=1)", "frac": ops / fl_avg / dfma, "traffic": None,
+                "peak_source": "measured: register-resident DFMA microbenchmark in this run",
+                "avg_launch_ms": fl_avg * 1e3, "launches_timed": fl_n,
+                "hbm": {"achieved": byt / fl_avg / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": byt / fl_avg / 1e9 / hbm_peak, "peak_source": hbm_src}}
+        line = {"metric": METRIC, "value": cells * world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+                "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": case.name, "cells": cells, "ns": case.mech.ns, "nr": case.mech.nr,
+                           "nvar": nvar, "cfl": case.cfl, "parallelism": f"replicas x{world}",
+                           "l2": "state %.0f MB per register > 126 MB L2" % (cells * nvar * 8 / 1e6)
+                                 if cells * nvar * 8 > 126e6 else "state fits L2 (no flush; noted)"},
+                "clocks": sampler.summary(),
+                "e2e": {"value": cells * world * Ke / (ms_e2e * 1e-3), "unit": UNIT,
+                        "h2d_bytes_per_step": int(Uh.numel() * 8 + Th.numel() * 8), "d2h_bytes_per_step": int(Uo.numel() * 8),
+                        "steps": Ke},
+                "gpu_launches": int(launches),
+                "roofline": roof,
+                "phases_ms_per_step": {k: v[0] / K for k, v in phases.items()},
+                "context": {"paper_a100_cell_updates_per_s": 2.0e7, "note": "PAPER.md:448, other hardware and mechanism"}}
+        if not args.no_cpu_baseline and world >= 1:
+            cb, _, _ = oracle_throughput(case)
+            line["cpu_baseline"] = cb
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
