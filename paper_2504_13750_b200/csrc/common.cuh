@@ -11,7 +11,17 @@
 #define JANC_RU 8.314472
 #define JANC_PATM 101325.0   // eq 4.9
 
+#define JANC_MAX_TB 32       // third-body reactions
+#define JANC_MAX_ENT 768     // sum over reactions of (reactant + product entries with multiplicity)
+
 enum { FK_NEIGHBOUR = 0, FK_PHYSICAL = 1, FK_COARSE = 2 };
+
+// One term of dq_i/dX_j (product rule on eq 4.7): +-(M k) * prod of the other species of that side.
+struct DqEntry {
+  unsigned char rx, side, nother, pad;
+  unsigned char other[JANC_MAX_ORDER - 1];
+  unsigned char pad2[3];
+};
 
 // Mechanism in constant memory (eq 4.3-4.9).  Reactant / product lists are expanded with
 // multiplicity: prod_j X_j^nu_ij = prod_e X[sp[e]].
@@ -24,7 +34,14 @@ struct MechC {
   signed char rev[JANC_MAX_NR], tb[JANC_MAX_NR], dn[JANC_MAX_NR];
   unsigned char nreac[JANC_MAX_NR], nprod[JANC_MAX_NR];
   unsigned char reac[JANC_MAX_NR][JANC_MAX_ORDER], prod[JANC_MAX_NR][JANC_MAX_ORDER];
-  double eff[JANC_MAX_NR][JANC_MAX_NS];
+  unsigned char tbi[JANC_MAX_NR];            // row of eff[] for a third-body reaction
+  int ntb;
+  double eff[JANC_MAX_TB][JANC_MAX_NS];      // a_ij of eq 4.7, third-body reactions only
+  // tables of the register-resident chemistry kernel (chem.cuh, k_chem_reg)
+  double dnu[JANC_MAX_NR][JANC_MAX_NS];      // nu^b - nu^f as doubles (dense rows, static row index)
+  int col_start[JANC_MAX_NS + 1];            // derivative entries grouped by species column
+  int nent;
+  DqEntry ent[JANC_MAX_ENT];
 };
 
 // Geometry + device pointers handed to every kernel by value.

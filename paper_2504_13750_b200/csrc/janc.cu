@@ -164,8 +164,33 @@ extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
       dn += b - f;
     }
     M.nreac[i] = (unsigned char)nre; M.nprod[i] = (unsigned char)npr; M.dn[i] = (signed char)dn;
-    for (int k = 0; k < m->ns; k++) M.eff[i][k] = m->eff ? m->eff[i * m->ns + k] : 1.0;
+    if (M.tb[i]) {
+      if (M.ntb >= JANC_MAX_TB) { c->err = "too many third-body reactions"; return JANC_EINVAL; }
+      M.tbi[i] = (unsigned char)M.ntb;
+      for (int k = 0; k < m->ns; k++) M.eff[M.ntb][k] = m->eff ? m->eff[i * m->ns + k] : 1.0;
+      M.ntb++;
+    }
+    for (int k = 0; k < m->ns; k++) M.dnu[i][k] = (double)(m->nu_b[i * m->ns + k] - m->nu_f[i * m->ns + k]);
   }
+  // derivative entries of eq 4.7 grouped by the species (column) they differentiate
+  M.nent = 0;
+  for (int j = 0; j < m->ns; j++) {
+    M.col_start[j] = M.nent;
+    for (int i = 0; i < m->nr; i++)
+      for (int side = 0; side < 2; side++) {
+        if (side == 1 && !M.rev[i]) continue;
+        const unsigned char *lst = side == 0 ? M.reac[i] : M.prod[i];
+        const int cnt = side == 0 ? M.nreac[i] : M.nprod[i];
+        for (int e = 0; e < cnt; e++) {
+          if (lst[e] != j) continue;
+          if (M.nent >= JANC_MAX_ENT) { c->err = "mechanism has too many derivative entries"; return JANC_EINVAL; }
+          DqEntry &E = M.ent[M.nent++];
+          E.rx = (unsigned char)i; E.side = (unsigned char)side; E.nother = 0;
+          for (int e2 = 0; e2 < cnt; e2++) if (e2 != e) E.other[E.nother++] = lst[e2];
+        }
+      }
+  }
+  for (int j = m->ns; j <= JANC_MAX_NS; j++) M.col_start[j] = M.nent;
   c->ns = m->ns; c->nr = m->nr;
   c->nvar = c->g.ndim + 2 + m->ns - 1;
   c->P.nvar = c->nvar; c->P.ns = m->ns;
@@ -410,10 +435,18 @@ template <int NS>
 static void launch_chem(janc_ctx *c, double *U) {
   k_chem<NS><<<cell_grid(c, 128, c->np), 128, 0, c->stream>>>(c->P, U);
 }
+template <int NS>
+static void launch_chem_reg(janc_ctx *c, double *U) {
+  constexpr int NT = 64;
+  const size_t smem = (size_t)(NS + 2 * c->nr + c->mech.ntb) * NT * sizeof(double);
+  static bool attr_done = false;
+  if (!attr_done) { cudaFuncSetAttribute(k_chem_reg<NS, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); attr_done = true; }
+  k_chem_reg<NS, NT><<<cell_grid(c, NT, c->np), NT, smem, c->stream>>>(c->P, U);
+}
 static void do_chem(janc_ctx *c, double *U, Prof *pf) {
   switch (c->ns) {
-    case 2: launch_chem<2>(c, U); break;
-    case 9: launch_chem<9>(c, U); break;
+    case 2: launch_chem_reg<2>(c, U); break;
+    case 9: launch_chem_reg<9>(c, U); break;
     case 20: launch_chem<20>(c, U); break;
     default: launch_chem<0>(c, U); break;
   }

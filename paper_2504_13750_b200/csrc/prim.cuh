@@ -5,6 +5,7 @@
 #include "common.cuh"
 
 __constant__ MechC c_mech;
+static_assert(sizeof(MechC) <= 65536, "MechC must fit constant memory");
 
 // cp_k/R_k and h_k/R_k (eq 4.3, 4.4), Horner form
 __device__ __forceinline__ double cp_R(int k, double T) {
