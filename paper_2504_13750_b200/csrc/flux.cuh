@@ -4,140 +4,310 @@
 // Readings A1 (WENO5-JS, eps 1e-6, p 2), A2 (component-wise), A3/A20 (alpha per direction per
 // level, from the stage state), A4 (increment form of SSP-RK3), A24 (x, y, z order).
 //
-// Work decomposition ("pair" form): the thread at cell c forms, for one component and one direction,
-// the split fluxes f+ and f- on the window c-2..c+2 ONCE and reconstructs from it both
-//     G(c) = Fhat+_{c+1/2}   (WENO5 on f+_{c-2..c+2})
-//     H(c) = Fhat-_{c-1/2}   (WENO5 on f-_{c+2..c-2}, the mirror image)
-// so that  Fhat_{c+1/2} = G(c) + H(c+1).  G and H go through shared memory; the divergence of cell c
-// is  -(G(c) + H(c+1) - G(c-1) - H(c)) / dx.  Per tile and direction the items are the tile cells
-// plus one rim cell at each end: every face is reconstructed exactly once, no flux array in HBM.
+// Work decomposition ("pencil walk"): a CTA owns a TX x TY x TZ tile of one patch and loops over the
+// nvar components.  For each direction every thread walks a pencil of SEG consecutive cells along
+// that direction and produces the SEG+1 face fluxes of the pencil from the SEG+6 cells it touches;
+// first and second differences of the split fluxes are shared between neighbouring faces, so one
+// face costs ~2 x 38 fp64 instructions and each split flux is evaluated once per pencil.
+//   x: the tile rows (+3 ghosts each side) of 2f+- = F +- alpha U are staged once in shared memory
+//      with coalesced loads; pencils then read them row-wise (odd pitch, conflict-free).
+//   y, z: lanes run along x, so the strided pencil loads are already coalesced; no staging.
+// Pencil results (-dF/dx_d) are summed per cell in shared memory; a coalesced pass applies the RK
+// stage.  No flux array ever goes to HBM: per stage the kernel reads U^(k) (+ U^n) and writes U^(k+1).
+//
+// WENO5 in difference form.  With D_k = v_{k+1} - v_k (k = 0..3 over v_{-2..+2}):
+//   beta_0 = 13/12 (D1-D0)^2 + 1/4 (3 D1 - D0)^2,  beta_1 = 13/12 (D2-D1)^2 + 1/4 (D1+D2)^2,
+//   beta_2 = 13/12 (D3-D2)^2 + 1/4 (D3 - 3 D2)^2,
+//   q_0 = v_0 + (5 D1 - 2 D0)/6,  q_1 = v_0 + (D1 + 2 D2)/6,  q_2 = v_0 + (4 D2 - D3)/6
+// which is the Jiang-Shu formula of SURVEY 8(c) step 5 re-grouped (identical in exact arithmetic).
+// The kernel reconstructs 2f+- (not f+-): beta scales by 4, so eps -> 4 eps keeps the weights
+// bit-for-bit those of f+-; beta is further carried as 12 beta (eps -> 48 eps); the 1/2 is folded
+// into 1/dx.  a_k = d_k/(eps+beta_k)^2 is evaluated as d_k prod_{l!=k}(eps+beta_l)^2 over the common
+// denominator: one reciprocal per reconstruction.
 #pragma once
 #include "common.cuh"
 
-// WENO5-JS value at +1/2 from v_{-2..+2}, one division:
-//   a_k = d_k / (eps + beta_k)^2  ==  d_k * prod_{l != k} (eps + beta_l)^2 / prod_l (eps+beta_l)^2
-__device__ __forceinline__ double weno5_js(double v0, double v1, double v2, double v3, double v4) {
-  const double eps = 1e-6, c1312 = 13.0 / 12.0;
-  double t1, t2;
-  t1 = (v0 - 2.0 * v1) + v2; t2 = (v0 - 4.0 * v1) + 3.0 * v2;
-  double b0 = fma(c1312 * t1, t1, fma(0.25 * t2, t2, eps));
-  t1 = (v1 - 2.0 * v2) + v3; t2 = v1 - v3;
-  double b1 = fma(c1312 * t1, t1, fma(0.25 * t2, t2, eps));
-  t1 = (v2 - 2.0 * v3) + v4; t2 = (3.0 * v2 - 4.0 * v3) + v4;
-  double b2 = fma(c1312 * t1, t1, fma(0.25 * t2, t2, eps));
-  b0 *= b0; b1 *= b1; b2 *= b2;
-  const double a0 = 0.1 * (b1 * b2), a1 = 0.6 * (b0 * b2), a2 = 0.3 * (b0 * b1);
-  const double q0 = fma(2.0, v0, fma(-7.0, v1, 11.0 * v2));
-  const double q1 = fma(5.0, v2, fma(2.0, v3, -v1));
-  const double q2 = fma(2.0, v2, fma(5.0, v3, -v4));
-  const double num = fma(a0, q0, fma(a1, q1, a2 * q2));
-  const double den = 6.0 * ((a0 + a1) + a2);
-  return num / den;
+#define JANC_WENO_EPS48 4.8e-5   // 48 * 1e-6, see above
+
+// 1/x to full fp64 precision for normal, finite x > 0 (MUFU seed + 2 Newton steps, no slow path).
+__device__ __forceinline__ double rcp_pos(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  r = fma(fma(-x, r, 1.0), r, r);
+  r = fma(fma(-x, r, 1.0), r, r);
+  return r;
 }
 
-template <int NDIM, int TX, int TY, int TZ, int NT>
-__global__ void __launch_bounds__(NT)
-k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uout, int slot_base, double coef) {
-  constexpr int T_[3] = {TX, TY, TZ};
-  constexpr int NOUT = TX * TY * TZ;
-  constexpr int OPT = (NOUT + NT - 1) / NT;                 // outputs per thread
-  constexpr int MAXI = NDIM == 1 ? (TX + 2) * TY * TZ
-                     : NDIM == 2 ? ((TX + 2) * TY > TX * (TY + 2) ? (TX + 2) * TY : TX * (TY + 2)) * TZ
-                     : ((TX + 2) * TY * TZ > TX * (TY + 2) * TZ
-                            ? ((TX + 2) * TY * TZ > TX * TY * (TZ + 2) ? (TX + 2) * TY * TZ : TX * TY * (TZ + 2))
-                            : (TX * (TY + 2) * TZ > TX * TY * (TZ + 2) ? TX * (TY + 2) * TZ : TX * TY * (TZ + 2)));
-  __shared__ double sG[2][MAXI], sH[2][MAXI];
+// value at the face from centre value v and differences D0..D3; S_k = 48 eps + 13 (D_{k+1}-D_k)^2
+__device__ __forceinline__ double weno5_diff(double v, double D0, double D1, double D2, double D3,
+                                             double S0, double S1, double S2) {
+  const double t0 = fma(3.0, D1, -D0), t1 = D1 + D2, t2 = fma(-3.0, D2, D3);
+  double b0 = fma(3.0 * t0, t0, S0), b1 = fma(3.0 * t1, t1, S1), b2 = fma(3.0 * t2, t2, S2);
+  b0 *= b0; b1 *= b1; b2 *= b2;
+  const double a0 = 0.1 * (b1 * b2), a1 = 0.6 * (b0 * b2), a2 = 0.3 * (b0 * b1);
+  const double c0 = fma(5.0, D1, -2.0 * D0), c1 = fma(2.0, D2, D1), c2 = fma(4.0, D2, -D3);
+  const double num = fma(a0, c0, fma(a1, c1, a2 * c2));
+  const double den = (a0 + a1) + a2;
+  return fma(num * rcp_pos(den), 1.0 / 6.0, v);
+}
 
+// Face fluxes of one pencil, streamed: ld(k, fp2, fm2) returns 2f+ and 2f- of pencil cell k-3
+// (k = 0..SEG+5); Fh[q], q = 0..SEG, is twice the numerical flux at the face between cells q-1 and q.
+// Cell k is fetched just before the first face that needs it, so only a 6-cell window is live.
+template <int SEG, class Load>
+__device__ __forceinline__ void weno_faces(Load &&ld, double (&Fh)[SEG + 1]) {
+  double P[SEG + 6], M[SEG + 6], dP[SEG + 5], dM[SEG + 5], sP[SEG + 4], sM[SEG + 4];
+#pragma unroll
+  for (int k = 0; k < 5; k++) ld(k, P[k], M[k]);
+#pragma unroll
+  for (int k = 0; k < 4; k++) { dP[k] = P[k + 1] - P[k]; dM[k] = M[k + 1] - M[k]; }
+#pragma unroll
+  for (int k = 0; k < 3; k++) {
+    const double s = dP[k + 1] - dP[k], r = dM[k + 1] - dM[k];
+    sP[k] = fma(13.0 * s, s, JANC_WENO_EPS48);
+    sM[k] = fma(13.0 * r, r, JANC_WENO_EPS48);
+  }
+#pragma unroll
+  for (int q = 0; q <= SEG; q++) {
+    ld(q + 5, P[q + 5], M[q + 5]);
+    dP[q + 4] = P[q + 5] - P[q + 4]; dM[q + 4] = M[q + 5] - M[q + 4];
+    const double s = dP[q + 4] - dP[q + 3], r = dM[q + 4] - dM[q + 3];
+    sP[q + 3] = fma(13.0 * s, s, JANC_WENO_EPS48);
+    sM[q + 3] = fma(13.0 * r, r, JANC_WENO_EPS48);
+    // plus part: stencil cells q-3..q+1 (array q..q+4), upwind centre = array q+2
+    const double fp = weno5_diff(P[q + 2], dP[q], dP[q + 1], dP[q + 2], dP[q + 3], sP[q], sP[q + 1], sP[q + 2]);
+    // minus part: mirror image, cells q+2..q-2 (array q+5..q+1), centre = array q+3
+    const double fm = weno5_diff(M[q + 3], -dM[q + 4], -dM[q + 3], -dM[q + 2], -dM[q + 1], sM[q + 3], sM[q + 2], sM[q + 1]);
+    Fh[q] = fp + fm;
+  }
+}
+
+// physical flux component m of direction d from (U_m, u_d, p):  F = (U_m + cE p) u_d + cM p  with
+// (cE, cM) = (0,1) for the normal momentum, (1,0) for the energy, (0,0) otherwise.
+__device__ __forceinline__ void split2(double Um, double ud, double p, double cE, double cM, double alpha,
+                                       double &fp2, double &fm2) {
+  const double F = fma(fma(cE, p, Um), ud, cM * p);
+  fp2 = fma(alpha, Um, F);
+  fm2 = fma(-alpha, Um, F);
+}
+
+template <int NDIM, int TX, int TY, int TZ, int SEG>
+struct FluxCfg {
+  static constexpr int NT = TX * TY * TZ / SEG;          // threads per CTA = pencils per direction
+  static constexpr int ROWS = TY * TZ;
+  static constexpr int XP = ((TX + 6) | 1);              // odd pitch of the staged x rows
+  static constexpr int LP = TX | 1;                      // odd pitch of the per-cell accumulator
+  static constexpr int NOUT = TX * TY * TZ;
+  static constexpr size_t SMEM = (size_t)(2 * ROWS * XP + ROWS * LP) * sizeof(double);
+  static_assert(TX % SEG == 0 && (NDIM < 2 || TY % SEG == 0) && (NDIM < 3 || TZ % SEG == 0), "tile % SEG");
+  static_assert(NT >= 32 && NT <= 1024, "threads");
+};
+
+// grid: (tiles of one patch, np).  Uout = U0 + coef * ((Uk - U0) + dt * L(Uk)).
+template <int NDIM, int TX, int TY, int TZ, int SEG>
+__global__ void __launch_bounds__(TX * TY * TZ / SEG, 512 / (TX * TY * TZ / SEG) > 0 ? 512 / (TX * TY * TZ / SEG) : 1)
+k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uout, int slot_base, double coef) {
+  using C = FluxCfg<NDIM, TX, TY, TZ, SEG>;
+  constexpr int NT = C::NT;
+  extern __shared__ double flux_smem[];
+  double *sFp = flux_smem, *sFm = sFp + C::ROWS * C::XP, *sL = sFm + C::ROWS * C::XP;
+
+  const int tid = threadIdx.x;
   const int patch = blockIdx.y;
   const int lev = P.level[patch];
   const int ntx = (P.n[0] + TX - 1) / TX, nty = (P.n[1] + TY - 1) / TY;
-  const int bx = blockIdx.x % ntx, by = (blockIdx.x / ntx) % nty, bz = blockIdx.x / (ntx * nty);
-  const int o0[3] = {bx * TX, by * TY, bz * TZ};
+  const int o0 = (blockIdx.x % ntx) * TX, o1 = ((blockIdx.x / ntx) % nty) * TY, o2 = (blockIdx.x / (ntx * nty)) * TZ;
   const double dt = P.scal[0];
-  const double *Ukp = Uk + (long long)patch * P.nvar * P.pc;
-  const double *U0p = U0 + (long long)patch * P.nvar * P.pc;
-  double *Uop = Uout + (long long)patch * P.nvar * P.pc;
-  const double *pp = P.p + (long long)patch * P.pc;
+  const long long pbase = (long long)patch * P.pc;
+  const double *Ukp = Uk + pbase * P.nvar;
+  const double *U0p = U0 + pbase * P.nvar;
+  double *Uop = Uout + pbase * P.nvar;
+  const double *pp = P.p + pbase;
+  const long long st1 = P.st[1], st2 = P.st[2];
+  double alpha[3], hidx[3];
+#pragma unroll
+  for (int d = 0; d < NDIM; d++) {
+    alpha[d] = slot_value(P.slots + slot_base + lev * 3 + d);
+    hidx[d] = 0.5 * P.invdx[lev][d];
+  }
+  // last loadable index along each dim (keeps ragged tiles inside the padded array)
+  const int mx0 = P.n[0] + 2, mx1 = NDIM > 1 ? P.n[1] + 2 : 0, mx2 = NDIM > 2 ? P.n[2] + 2 : 0;
+  const int in1 = NDIM > 1 ? P.n[1] - 1 : 0, in2 = NDIM > 2 ? P.n[2] - 1 : 0;
 
-  int q = 0;
 #pragma unroll 1
   for (int m = 0; m < P.nvar; m++) {
     const double *Um = Ukp + (long long)m * P.pc;
-    double Lacc[OPT];
-#pragma unroll
-    for (int r = 0; r < OPT; r++) Lacc[r] = 0.0;
-#pragma unroll
-    for (int d = 0; d < NDIM; d++, q++) {
-      const int buf = q & 1;
-      const int B0 = TX + (d == 0 ? 2 : 0), B1 = TY + (d == 1 ? 2 : 0), B2 = TZ + (d == 2 ? 2 : 0);
-      const int nitems = B0 * B1 * B2;
-      const long long sd = P.st[d];
-      const double alpha = slot_value(P.slots + slot_base + lev * 3 + d);
-      const double *ud = P.vel + ((long long)d * P.np + patch) * P.pc;
-      const double *Umom = Ukp + (long long)(1 + d) * P.pc;
-      const int kindm = m == 0 ? 0 : (m == 1 + d ? 1 : (m == NDIM + 1 ? 2 : 3));
+    const double cEn = m == NDIM + 1 ? 1.0 : 0.0;
+    // ---------------- x: stage 2f+- rows, then walk
+    {
+      const double cM = m == 1 ? 1.0 : 0.0;
+      const double *ux = P.vel + pbase;
 #pragma unroll 1
-      for (int it = threadIdx.x; it < nitems; it += NT) {
-        int l[3] = {it % B0, (it / B0) % B1, it / (B0 * B1)};
-        l[d] -= 1;
-        const int g0 = o0[0] + l[0], g1 = o0[1] + l[1], g2 = o0[2] + l[2];
-        const int gd = d == 0 ? g0 : (d == 1 ? g1 : g2);
-        bool valid = gd <= P.n[d];
-        if (d != 0) valid = valid && g0 < P.n[0];
-        if (d != 1) valid = valid && g1 < P.n[1];
-        if (d != 2) valid = valid && g2 < P.n[2];
-        double G = 0.0, H = 0.0;
-        if (valid) {
-          const long long id = cell_index(P, g0, g1, g2);
-          double fp[5], fm[5];
-#pragma unroll
-          for (int s = 0; s < 5; s++) {
-            const long long c = id + (long long)(s - 2) * sd;
-            const double Uv = Um[c];
-            double F;
-            if (kindm == 0) F = Umom[c];                       // rho u_d
-            else if (kindm == 1) F = fma(Uv, ud[c], pp[c]);    // rho u_d u_d + p
-            else if (kindm == 2) F = ud[c] * (Uv + pp[c]);     // u_d (E + p)
-            else F = Uv * ud[c];                               // rho u_j u_d, rho Y_k u_d
-            const double aU = alpha * Uv;
-            fp[s] = 0.5 * (F + aU);
-            fm[s] = 0.5 * (F - aU);
-          }
-          G = weno5_js(fp[0], fp[1], fp[2], fp[3], fp[4]);
-          H = weno5_js(fm[4], fm[3], fm[2], fm[1], fm[0]);
-        }
-        sG[buf][it] = G;
-        sH[buf][it] = H;
+      for (int it = tid; it < C::ROWS * (TX + 6); it += NT) {
+        const int xi = it % (TX + 6), r = it / (TX + 6);
+        const int gx = min(o0 + xi - 3, mx0), gy = min(o1 + r % TY, in1), gz = min(o2 + r / TY, in2);
+        const long long id = cell_index(P, gx, gy, gz);
+        double a, b;
+        split2(Um[id], ux[id], pp[id], cEn, cM, alpha[0], a, b);
+        sFp[r * C::XP + xi] = a;
+        sFm[r * C::XP + xi] = b;
       }
       __syncthreads();
-      const double idx = P.invdx[lev][d];
+      const int r = tid % C::ROWS, xs = (tid / C::ROWS) * SEG;
+      double Fh[SEG + 1];
+      const double *rp = sFp + r * C::XP + xs, *rm = sFm + r * C::XP + xs;
+      weno_faces<SEG>([&](int k, double &a, double &b) { a = rp[k]; b = rm[k]; }, Fh);
 #pragma unroll
-      for (int r = 0; r < OPT; r++) {
-        const int o = threadIdx.x + r * NT;
-        if (o < NOUT) {
-          int l[3] = {o % TX, (o / TX) % TY, o / (TX * TY)};
-          l[d] += 1;
-          const int c = (l[2] * B1 + l[1]) * B0 + l[0];
-          const int sI = d == 0 ? 1 : (d == 1 ? B0 : B0 * B1);
-          const double Fr = sG[buf][c] + sH[buf][c + sI];
-          const double Fl = sG[buf][c - sI] + sH[buf][c];
-          Lacc[r] -= (Fr - Fl) * idx;
-        }
+      for (int i = 0; i < SEG; i++) sL[r * C::LP + xs + i] = (Fh[i] - Fh[i + 1]) * hidx[0];
+      __syncthreads();
+    }
+    // ---------------- y and z: strided pencils straight from global memory
+#pragma unroll
+    for (int d = 1; d < NDIM; d++) {
+      const double cM = m == 1 + d ? 1.0 : 0.0;
+      const double *ud = P.vel + (long long)d * P.np * P.pc + pbase;
+      const int x = tid % TX, rest = tid / TX;
+      // d == 1: pencils along y, the other index is z;  d == 2: pencils along z, the other index is y
+      const int other = d == 1 ? rest % TZ : rest % TY;
+      const int seg = (d == 1 ? rest / TZ : rest / TY) * SEG;
+      const int ly = d == 1 ? seg : other, lz = d == 1 ? other : seg;
+      const int gx = min(o0 + x, P.n[0] - 1);
+      const int gy = d == 1 ? o1 + ly : min(o1 + ly, in1);
+      const int gz = d == 2 ? o2 + lz : min(o2 + lz, in2);
+      const long long sd = d == 1 ? st1 : st2;
+      const int gd = d == 1 ? gy : gz, mxd = d == 1 ? mx1 : mx2;
+      const long long id0 = cell_index(P, gx, gy, gz);
+      double Fh[SEG + 1];
+      const double al = alpha[d];
+      weno_faces<SEG>([&](int k, double &a, double &b) {
+        const long long id = id0 + (long long)(min(gd + k - 3, mxd) - gd) * sd;
+        split2(Um[id], ud[id], pp[id], cEn, cM, al, a, b);
+      }, Fh);
+      double *acc = sL + (lz * TY + ly) * C::LP + x;
+      const int sa = d == 1 ? C::LP : TY * C::LP;
+#pragma unroll
+      for (int i = 0; i < SEG; i++) acc[i * sa] += (Fh[i] - Fh[i + 1]) * hidx[d];
+      __syncthreads();
+    }
+    // ---------------- RK stage (increment form), coalesced
+#pragma unroll
+    for (int o = tid; o < C::NOUT; o += NT) {
+      const int lx = o % TX, ly = (o / TX) % TY, lz = o / (TX * TY);
+      const int g0 = o0 + lx, g1 = o1 + ly, g2 = o2 + lz;
+      if (g0 < P.n[0] && g1 < P.n[1] && g2 < P.n[2]) {
+        const long long id = cell_index(P, g0, g1, g2) + (long long)m * P.pc;
+        const double u0 = U0p[id];
+        Uop[id] = u0 + coef * ((Ukp[id] - u0) + dt * sL[(lz * TY + ly) * C::LP + lx]);
       }
     }
-    // RK stage (increment form): Uout = U0 + coef * ((Uk - U0) + dt * L)
-#pragma unroll
-    for (int r = 0; r < OPT; r++) {
-      const int o = threadIdx.x + r * NT;
-      if (o < NOUT) {
-        const int g0 = o0[0] + o % TX, g1 = o0[1] + (o / TX) % TY, g2 = o0[2] + o / (TX * TY);
-        if (g0 < P.n[0] && g1 < P.n[1] && g2 < P.n[2]) {
-          const long long id = cell_index(P, g0, g1, g2) + (long long)m * P.pc;
-          const double u0 = U0p[id];
-          Uop[id] = u0 + coef * ((Ukp[id] - u0) + dt * Lacc[r]);
-        }
-      }
-    }
+    // the next component's x pencils overwrite sL only after its staging barrier
   }
-  (void)T_;
+}
+
+// ------------------------------------------------------------------------------------------------
+// 2-D variant with the tile resident in shared memory.  p, u, v of the tile + 3 ghost layers are
+// copied once per CTA and U_m (same box) is double-buffered with cp.async: the copy of component
+// m+1 runs while the pencils of component m are computed, so the walks only ever wait on shared
+// memory.  Odd row pitch: x pencils (lanes = rows) and y pencils (lanes = columns) are both
+// conflict-free, so no transposed staging pass is needed.
+__device__ __forceinline__ void cp_async8(double *dst_smem, const double *src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <int TX, int TY, int SEG>
+struct Flux2Cfg {
+  static constexpr int NT = TX * TY / SEG;
+  static constexpr int BX = TX + 6, BY = TY + 6;
+  static constexpr int PIT = BX | 1;
+  static constexpr int BOX = PIT * BY;
+  static constexpr int LP = TX | 1;
+  static constexpr size_t SMEM = (size_t)(5 * BOX + TY * LP) * sizeof(double);
+  static constexpr int MINB = 512 / NT > 0 ? 512 / NT : 1;      // keeps the kernel at <= 128 registers
+  static_assert(TX % SEG == 0 && TY % SEG == 0, "tile % SEG");
+};
+
+template <int TX, int TY, int SEG>
+__global__ void __launch_bounds__(Flux2Cfg<TX, TY, SEG>::NT, Flux2Cfg<TX, TY, SEG>::MINB)
+k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uout, int slot_base, double coef) {
+  using C = Flux2Cfg<TX, TY, SEG>;
+  constexpr int NT = C::NT, PIT = C::PIT;
+  extern __shared__ double flux_smem[];
+  double *sp = flux_smem, *su = sp + C::BOX, *sv = su + C::BOX, *sU = sv + C::BOX, *sL = sU + 2 * C::BOX;
+
+  const int tid = threadIdx.x;
+  const int patch = blockIdx.y;
+  const int lev = P.level[patch];
+  const int ntx = (P.n[0] + TX - 1) / TX;
+  const int o0 = (blockIdx.x % ntx) * TX, o1 = (blockIdx.x / ntx) * TY;
+  const double dt = P.scal[0];
+  const long long pbase = (long long)patch * P.pc;
+  const double *Ukp = Uk + pbase * P.nvar;
+  const double *U0p = U0 + pbase * P.nvar;
+  double *Uop = Uout + pbase * P.nvar;
+  const long long st1 = P.st[1];
+  const double ax = slot_value(P.slots + slot_base + lev * 3 + 0), ay = slot_value(P.slots + slot_base + lev * 3 + 1);
+  const double hx = 0.5 * P.invdx[lev][0], hy = 0.5 * P.invdx[lev][1];
+  const int mxp = P.P[0] - 1, myp = P.P[1] - 1;     // last padded index (ragged tiles stay in the array)
+
+  auto load_box = [&](double *dst, const double *src) {
+#pragma unroll 4
+    for (int it = tid; it < C::BX * C::BY; it += NT) {
+      const int bx = it % C::BX, by = it / C::BX;
+      const int gx = min(o0 + bx, mxp), gy = min(o1 + by, myp);
+      cp_async8(dst + by * PIT + bx, src + (long long)gy * st1 + gx);
+    }
+  };
+  load_box(sp, P.p + pbase);
+  load_box(su, P.vel + pbase);
+  load_box(sv, P.vel + (long long)P.np * P.pc + pbase);
+  load_box(sU, Ukp);
+  cp_async_commit();
+  if (P.nvar > 1) load_box(sU + C::BOX, Ukp + P.pc);
+  cp_async_commit();
+
+#pragma unroll 1
+  for (int m = 0; m < P.nvar; m++) {
+    const double *sUm = sU + (m & 1) * C::BOX;
+    const double cEn = m == 3 ? 1.0 : 0.0;
+    cp_async_wait<1>();
+    __syncthreads();
+    {  // x pencils: lanes run over rows
+      const double cM = m == 1 ? 1.0 : 0.0;
+      const int r = tid % TY, xs = (tid / TY) * SEG;
+      const int base = (r + 3) * PIT + xs;
+      double Fh[SEG + 1];
+      weno_faces<SEG>([&](int k, double &a, double &b) { split2(sUm[base + k], su[base + k], sp[base + k], cEn, cM, ax, a, b); }, Fh);
+#pragma unroll
+      for (int i = 0; i < SEG; i++) sL[r * C::LP + xs + i] = (Fh[i] - Fh[i + 1]) * hx;
+    }
+    __syncthreads();
+    {  // y pencils: lanes run over columns
+      const double cM = m == 2 ? 1.0 : 0.0;
+      const int x = tid % TX, ys = (tid / TX) * SEG;
+      const int base = ys * PIT + x + 3;
+      double Fh[SEG + 1];
+      weno_faces<SEG>([&](int k, double &a, double &b) { split2(sUm[base + k * PIT], sv[base + k * PIT], sp[base + k * PIT], cEn, cM, ay, a, b); }, Fh);
+#pragma unroll
+      for (int i = 0; i < SEG; i++) sL[(ys + i) * C::LP + x] += (Fh[i] - Fh[i + 1]) * hy;
+    }
+    __syncthreads();
+    // RK stage (increment form), coalesced
+#pragma unroll
+    for (int o = tid; o < TX * TY; o += NT) {
+      const int lx = o % TX, ly = o / TX;
+      const int g0 = o0 + lx, g1 = o1 + ly;
+      if (g0 < P.n[0] && g1 < P.n[1]) {
+        const long long id = cell_index(P, g0, g1, 0) + (long long)m * P.pc;
+        const double u0 = U0p[id];
+        Uop[id] = u0 + coef * ((sUm[(ly + 3) * PIT + lx + 3] - u0) + dt * sL[ly * C::LP + lx]);
+      }
+    }
+    __syncthreads();   // everyone is done with sU[m & 1] and sL
+    if (m + 2 < P.nvar) load_box(sU + (m & 1) * C::BOX, Ukp + (long long)(m + 2) * P.pc);
+    cp_async_commit();
+  }
 }

@@ -412,21 +412,39 @@ static void do_ghost(janc_ctx *c, double *U, Prof *pf) {
   prof_mark(c, pf, 1);
 }
 
+template <int NDIM, int TX, int TY, int TZ, int SEG>
+static void launch_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef) {
+  using C = FluxCfg<NDIM, TX, TY, TZ, SEG>;
+  const Params &P = c->P;
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(k_flux_rk<NDIM, TX, TY, TZ, SEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    attr_done = true;
+  }
+  const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY) * ((P.n[2] + TZ - 1) / TZ));
+  k_flux_rk<NDIM, TX, TY, TZ, SEG><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
+}
+
+template <int TX, int TY, int SEG>
+static void launch_flux2(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef) {
+  using C = Flux2Cfg<TX, TY, SEG>;
+  const Params &P = c->P;
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(k_flux_rk2<TX, TY, SEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    attr_done = true;
+  }
+  const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY));
+  k_flux_rk2<TX, TY, SEG><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
+}
+
 static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef, Prof *pf) {
   const Params &P = c->P;
-  if (c->g.ndim == 1) {
-    constexpr int TX = 256;
-    dim3 grid((unsigned)((P.n[0] + TX - 1) / TX), (unsigned)c->np, 1);
-    k_flux_rk<1, TX, 1, 1, 256><<<grid, 256, 0, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
-  } else if (c->g.ndim == 2) {
-    constexpr int TX = 32, TY = 16;
-    dim3 grid((unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY)), (unsigned)c->np, 1);
-    k_flux_rk<2, TX, TY, 1, 512><<<grid, 512, 0, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
-  } else {
-    constexpr int TX = 16, TY = 8, TZ = 8;
-    dim3 grid((unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY) * ((P.n[2] + TZ - 1) / TZ)), (unsigned)c->np, 1);
-    k_flux_rk<3, TX, TY, TZ, 512><<<grid, 512, 0, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
-  }
+  if (c->g.ndim == 1) launch_flux<1, 128, 1, 1, 4>(c, Uk, U0, Uout, slot_base, coef);
+  else if (c->g.ndim == 2) {
+    if (P.n[0] <= 16 && P.n[1] <= 16) launch_flux2<16, 16, 8>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches
+    else launch_flux2<64, 16, 8>(c, Uk, U0, Uout, slot_base, coef);
+  } else launch_flux<3, 32, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);
   c->launches++;
   prof_mark(c, pf, 2);
 }
