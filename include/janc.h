@@ -121,6 +121,19 @@ int janc_profile_step(janc_ctx *, double cfl, double dt_fixed, float *ms_out, in
  * used as roofline denominator for "bound":"alu"). */
 int janc_measure_dfma_peak(int device, void *cuda_stream, double *dfma_per_s);
 
+/* Which chemistry kernel the context runs: "jit" = the mechanism-specialised kernel generated and
+ * compiled with NVRTC by janc_set_mechanism (csrc/chemgen.h; the counterpart of the paper's XLA JIT,
+ * PAPER.md:24, :39), "reg" / "generic" = the table-driven kernels of csrc/chem.cuh (mechanisms with
+ * more than 12 unknowns, NVRTC missing, or JANC_DISABLE_JIT=1 in the environment), "none" before a
+ * mechanism is set.  janc_jit_log returns the NVRTC log / the reason the specialised kernel is not used. */
+const char *janc_chem_kernel(const janc_ctx *);
+const char *janc_jit_log(const janc_ctx *);
+
+/* Diagnostic, needs no device: write the specialised CUDA source of a mechanism (NUL-terminated,
+ * truncated to cap) to src_out (nullable), its length to src_len (nullable), and, if cubin_bytes is
+ * non-NULL, compile it for sm_100a and return the cubin size.  JANC_ESTATE if NVRTC fails. */
+int janc_jit_probe(const janc_mech *, int ndim, char *src_out, size_t cap, size_t *src_len, size_t *cubin_bytes);
+
 const char *janc_last_error(const janc_ctx *);
 void janc_destroy(janc_ctx *);
 

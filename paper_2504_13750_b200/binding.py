@@ -21,7 +21,8 @@ FLAG_NO_CHEM = 1
 EXPORTS = ["janc_create", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
            "janc_set_blocks", "janc_set_state", "janc_step", "janc_get_state", "janc_status",
            "janc_launch_count", "janc_debug_cons2prim", "janc_profile_step",
-           "janc_measure_dfma_peak", "janc_last_error", "janc_destroy"]
+           "janc_measure_dfma_peak", "janc_chem_kernel", "janc_jit_log", "janc_jit_probe",
+           "janc_last_error", "janc_destroy"]
 
 
 class JancError(RuntimeError):
@@ -68,6 +69,11 @@ def lib():
         L.janc_measure_dfma_peak.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
         L.janc_last_error.argtypes = [C.c_void_p]
         L.janc_last_error.restype = C.c_char_p
+        L.janc_chem_kernel.argtypes = [C.c_void_p]
+        L.janc_chem_kernel.restype = C.c_char_p
+        L.janc_jit_log.argtypes = [C.c_void_p]
+        L.janc_jit_log.restype = C.c_char_p
+        L.janc_jit_probe.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p]
         L.janc_destroy.argtypes = [C.c_void_p]
         L.janc_destroy.restype = None
         _lib = L
@@ -84,6 +90,30 @@ def _i32(a):
 
 def _ptr(a):
     return a.ctypes.data_as(C.c_void_p)
+
+
+def _mech_struct(mech):
+    keep = dict(W=_f64(mech.W), nasa=_f64(mech.nasa), nu_f=_i32(mech.nu_f), nu_b=_i32(mech.nu_b),
+                A=_f64(mech.A), b=_f64(mech.b), Ta=_f64(mech.Ta), reversible=_i32(mech.reversible),
+                third_body=_i32(mech.third_body), eff=_f64(mech.eff))
+    m = _Mech(mech.ns, mech.nr, *[_ptr(keep[k]) for k in
+                                  ("W", "nasa", "nu_f", "nu_b", "A", "b", "Ta", "reversible", "third_body", "eff")])
+    return m, keep
+
+
+def jit_probe(mech, ndim, compile=True):
+    """janc_jit_probe: (specialised CUDA source, cubin size or None).  Needs no GPU."""
+    m, keep = _mech_struct(mech)
+    n = C.c_size_t(0)
+    rc = lib().janc_jit_probe(C.byref(m), int(ndim), None, 0, C.byref(n), None)
+    if rc:
+        raise JancError(rc, "janc_jit_probe")
+    buf = C.create_string_buffer(n.value + 1)
+    nb = C.c_size_t(0)
+    rc = lib().janc_jit_probe(C.byref(m), int(ndim), buf, n.value + 1, None, C.byref(nb) if compile else None)
+    if rc:
+        raise JancError(rc, "janc_jit_probe (NVRTC)")
+    return buf.value.decode(), (nb.value if compile else None)
 
 
 def measure_dfma_peak(device=0, stream=None):
@@ -116,11 +146,7 @@ class Solver:
         rc = L.janc_create(C.byref(g), self.device, C.c_void_p(stream.cuda_stream), C.byref(self._h))
         if rc:
             raise JancError(rc, "janc_create")
-        self._keep = dict(W=_f64(mech.W), nasa=_f64(mech.nasa), nu_f=_i32(mech.nu_f), nu_b=_i32(mech.nu_b),
-                          A=_f64(mech.A), b=_f64(mech.b), Ta=_f64(mech.Ta), reversible=_i32(mech.reversible),
-                          third_body=_i32(mech.third_body), eff=_f64(mech.eff))
-        m = _Mech(mech.ns, mech.nr, *[_ptr(self._keep[k]) for k in
-                                      ("W", "nasa", "nu_f", "nu_b", "A", "b", "Ta", "reversible", "third_body", "eff")])
+        m, self._keep = _mech_struct(mech)
         self._check(L.janc_set_mechanism(self._h, C.byref(m)), "janc_set_mechanism")
         nbytes = L.janc_workspace_bytes(self._h)
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{self.device}")
@@ -134,6 +160,13 @@ class Solver:
         self.shape = (self.np_, self.nvar, grid.n[2] if grid.ndim > 2 else 1,
                       grid.n[1] if grid.ndim > 1 else 1, grid.n[0])
         self.tshape = (self.shape[0],) + self.shape[2:]
+
+    def chem_kernel(self):
+        """'jit' (mechanism-specialised, NVRTC), 'reg' or 'generic' (table-driven kernels)."""
+        return lib().janc_chem_kernel(self._h).decode()
+
+    def jit_log(self):
+        return lib().janc_jit_log(self._h).decode()
 
     def _check(self, rc, what):
         if rc:

@@ -7,8 +7,13 @@
 #include <string>
 #include <vector>
 
+#include <dlfcn.h>
+#include <map>
+#include <nvrtc.h>
+
 #include "../../include/janc.h"
 #include "chem.cuh"
+#include "chemgen.h"
 #include "flux.cuh"
 #include "ghost.cuh"
 #include "prim.cuh"
@@ -30,6 +35,8 @@ struct janc_ctx {
   std::vector<int> level, nbr, parent, fkind;
   int parity;
   long long launches;
+  cudaKernel_t jit_kernel;   // mechanism-specialised chemistry kernel (chemgen.h), null if not in use
+  std::string jit_log;
   unsigned long long id;
   std::string err;
 };
@@ -123,6 +130,7 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
   c->parent.assign((size_t)c->np * (1 + grid->ndim), -1);
   c->fkind.assign((size_t)c->np * nf, FK_PHYSICAL);
   c->id = g_next_id++;
+  c->jit_kernel = nullptr;
   *out = c;
   return JANC_OK;
 }
@@ -137,11 +145,12 @@ extern "C" const char *janc_last_error(const janc_ctx *c) { return c ? c->err.c_
 extern "C" long long janc_launch_count(const janc_ctx *c) { return c ? c->launches : 0; }
 
 // ------------------------------------------------------------------ mechanism
-extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
-  if (!c || !m) return JANC_EINVAL;
-  if (m->ns < 1 || m->ns > JANC_MAX_NS || m->nr < 0 || m->nr > JANC_MAX_NR) { c->err = "ns/nr out of range"; return JANC_EINVAL; }
+// janc_mech (host arrays) -> MechC tables; err receives a text on failure
+static int fill_mech(const janc_mech *m, MechC &M, std::string &err) {
+  if (!m) return JANC_EINVAL;
+  if (m->ns < 1 || m->ns > JANC_MAX_NS || m->nr < 0 || m->nr > JANC_MAX_NR) { err = "ns/nr out of range"; return JANC_EINVAL; }
   if (!m->W || !m->nasa) return JANC_EINVAL;
-  MechC &M = c->mech;
+  if (m->nr > 0 && (!m->nu_f || !m->nu_b || !m->A || !m->b || !m->Ta)) return JANC_EINVAL;
   memset(&M, 0, sizeof M);
   M.ns = m->ns; M.nr = m->nr;
   for (int k = 0; k < m->ns; k++) {
@@ -150,7 +159,7 @@ extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
     for (int q = 0; q < 7; q++) M.nasa[k][q] = m->nasa[k * 7 + q];
   }
   for (int i = 0; i < m->nr; i++) {
-    if (!(m->A[i] > 0.0)) { c->err = "A must be > 0"; return JANC_EINVAL; }
+    if (!(m->A[i] > 0.0)) { err = "A must be > 0"; return JANC_EINVAL; }
     M.lnA[i] = log(m->A[i]); M.b[i] = m->b[i]; M.Ta[i] = m->Ta[i]; M.Asign[i] = 1.0;
     M.rev[i] = m->reversible ? (m->reversible[i] != 0) : 1;
     M.tb[i] = m->third_body ? (m->third_body[i] != 0) : 0;
@@ -158,14 +167,14 @@ extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
     for (int k = 0; k < m->ns; k++) {
       int f = m->nu_f[i * m->ns + k], b = m->nu_b[i * m->ns + k];
       if (f < 0 || b < 0) return JANC_EINVAL;
-      if (nre + f > JANC_MAX_ORDER || npr + b > JANC_MAX_ORDER) { c->err = "reaction order too large"; return JANC_EINVAL; }
+      if (nre + f > JANC_MAX_ORDER || npr + b > JANC_MAX_ORDER) { err = "reaction order too large"; return JANC_EINVAL; }
       for (int q = 0; q < f; q++) M.reac[i][nre++] = (unsigned char)k;
       for (int q = 0; q < b; q++) M.prod[i][npr++] = (unsigned char)k;
       dn += b - f;
     }
     M.nreac[i] = (unsigned char)nre; M.nprod[i] = (unsigned char)npr; M.dn[i] = (signed char)dn;
     if (M.tb[i]) {
-      if (M.ntb >= JANC_MAX_TB) { c->err = "too many third-body reactions"; return JANC_EINVAL; }
+      if (M.ntb >= JANC_MAX_TB) { err = "too many third-body reactions"; return JANC_EINVAL; }
       M.tbi[i] = (unsigned char)M.ntb;
       for (int k = 0; k < m->ns; k++) M.eff[M.ntb][k] = m->eff ? m->eff[i * m->ns + k] : 1.0;
       M.ntb++;
@@ -183,7 +192,7 @@ extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
         const int cnt = side == 0 ? M.nreac[i] : M.nprod[i];
         for (int e = 0; e < cnt; e++) {
           if (lst[e] != j) continue;
-          if (M.nent >= JANC_MAX_ENT) { c->err = "mechanism has too many derivative entries"; return JANC_EINVAL; }
+          if (M.nent >= JANC_MAX_ENT) { err = "mechanism has too many derivative entries"; return JANC_EINVAL; }
           DqEntry &E = M.ent[M.nent++];
           E.rx = (unsigned char)i; E.side = (unsigned char)side; E.nother = 0;
           for (int e2 = 0; e2 < cnt; e2++) if (e2 != e) E.other[E.nother++] = lst[e2];
@@ -191,6 +200,124 @@ extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
       }
   }
   for (int j = m->ns; j <= JANC_MAX_NS; j++) M.col_start[j] = M.nent;
+  return JANC_OK;
+}
+
+// ------------------------------------------------------------------ run-time specialised chemistry
+// NVRTC is reached through dlopen so that libjanc.so loads (and the generic kernels run) where it is
+// absent; the cubin is loaded with the runtime's cudaLibrary API (no link against libcuda).
+struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; };
+
+struct NvrtcApi {
+  void *h = nullptr;
+  nvrtcResult (*create)(nvrtcProgram *, const char *, const char *, int, const char *const *, const char *const *) = nullptr;
+  nvrtcResult (*compile)(nvrtcProgram, int, const char *const *) = nullptr;
+  nvrtcResult (*cubin_size)(nvrtcProgram, size_t *) = nullptr;
+  nvrtcResult (*cubin)(nvrtcProgram, char *) = nullptr;
+  nvrtcResult (*log_size)(nvrtcProgram, size_t *) = nullptr;
+  nvrtcResult (*log)(nvrtcProgram, char *) = nullptr;
+  nvrtcResult (*destroy)(nvrtcProgram *) = nullptr;
+  bool ok = false;
+};
+
+static NvrtcApi &nvrtc_api() {
+  static NvrtcApi a;
+  static bool tried = false;
+  if (tried) return a;
+  tried = true;
+  const char *names[] = {"libnvrtc.so.12", "libnvrtc.so", "/usr/local/cuda/lib64/libnvrtc.so.12", "/usr/local/cuda/lib64/libnvrtc.so"};
+  for (const char *n : names) { a.h = dlopen(n, RTLD_NOW | RTLD_LOCAL); if (a.h) break; }
+  if (!a.h) return a;
+  a.create = (decltype(a.create))dlsym(a.h, "nvrtcCreateProgram");
+  a.compile = (decltype(a.compile))dlsym(a.h, "nvrtcCompileProgram");
+  a.cubin_size = (decltype(a.cubin_size))dlsym(a.h, "nvrtcGetCUBINSize");
+  a.cubin = (decltype(a.cubin))dlsym(a.h, "nvrtcGetCUBIN");
+  a.log_size = (decltype(a.log_size))dlsym(a.h, "nvrtcGetProgramLogSize");
+  a.log = (decltype(a.log))dlsym(a.h, "nvrtcGetProgramLog");
+  a.destroy = (decltype(a.destroy))dlsym(a.h, "nvrtcDestroyProgram");
+  a.ok = a.create && a.compile && a.cubin_size && a.cubin && a.log_size && a.log && a.destroy;
+  return a;
+}
+
+// CUDA C -> sm_100a cubin.  Needs no device.
+static bool jit_compile(const std::string &src, std::vector<char> &cubin, std::string &log) {
+  NvrtcApi &a = nvrtc_api();
+  if (!a.ok) { log = "NVRTC not available (dlopen libnvrtc.so.12 failed)"; return false; }
+  nvrtcProgram prog;
+  if (a.create(&prog, src.c_str(), "k_chem_jit.cu", 0, nullptr, nullptr) != NVRTC_SUCCESS) { log = "nvrtcCreateProgram failed"; return false; }
+  const char *opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo"};
+  const nvrtcResult r = a.compile(prog, 3, opts);
+  size_t ls = 0;
+  a.log_size(prog, &ls);
+  if (ls > 1) { log.resize(ls); a.log(prog, &log[0]); }
+  bool ok = r == NVRTC_SUCCESS;
+  if (ok) {
+    size_t n = 0;
+    ok = a.cubin_size(prog, &n) == NVRTC_SUCCESS && n > 0;
+    if (ok) { cubin.resize(n); ok = a.cubin(prog, cubin.data()) == NVRTC_SUCCESS; }
+  }
+  a.destroy(&prog);
+  return ok;
+}
+
+// Generate + compile + load the chemistry kernel of c->mech; on any failure the generic kernels stay.
+static void jit_setup(janc_ctx *c) {
+  c->jit_kernel = nullptr;
+  c->jit_log.clear();
+  const MechC &M = c->mech;
+  if (M.ns < 2 || M.nr < 1 || M.ns - 1 > JANC_JIT_MAX_N1) { c->jit_log = "mechanism outside the specialised range"; return; }
+  const char *off = getenv("JANC_DISABLE_JIT");
+  if (off && off[0] && off[0] != '0') { c->jit_log = "disabled by JANC_DISABLE_JIT"; return; }
+  const std::string src = chemgen::generate(M, c->g.ndim);
+  static std::map<std::string, cudaKernel_t> cache;          // per process; one device per process
+  const std::string key = std::to_string(c->device) + "\n" + src;
+  auto it = cache.find(key);
+  if (it != cache.end()) { c->jit_kernel = it->second; return; }
+  std::vector<char> cubin;
+  if (!jit_compile(src, cubin, c->jit_log)) return;
+  cudaLibrary_t lib;
+  cudaError_t e = cudaLibraryLoadData(&lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+  if (e != cudaSuccess) { c->jit_log = std::string("cudaLibraryLoadData: ") + cudaGetErrorString(e); cudaGetLastError(); return; }
+  cudaKernel_t k;
+  e = cudaLibraryGetKernel(&k, lib, "k_chem_jit");
+  if (e != cudaSuccess) { c->jit_log = std::string("cudaLibraryGetKernel: ") + cudaGetErrorString(e); cudaGetLastError(); return; }
+  cache[key] = k;
+  c->jit_kernel = k;
+}
+
+extern "C" const char *janc_chem_kernel(const janc_ctx *c) {
+  if (!c || !c->have_mech) return "none";
+  if (c->jit_kernel) return "jit";
+  return (c->ns == 2 || c->ns == 9) ? "reg" : "generic";
+}
+extern "C" const char *janc_jit_log(const janc_ctx *c) { return c ? c->jit_log.c_str() : ""; }
+
+// Diagnostic, needs no device: emit the specialised source for a mechanism and compile it for sm_100a.
+extern "C" int janc_jit_probe(const janc_mech *m, int ndim, char *src_out, size_t cap, size_t *src_len, size_t *cubin_bytes) {
+  if (!m || ndim < 1 || ndim > 3) return JANC_EINVAL;
+  static MechC M;
+  std::string err;
+  int rc = fill_mech(m, M, err);
+  if (rc) return rc;
+  if (M.ns < 2 || M.nr < 1 || M.ns - 1 > JANC_JIT_MAX_N1) return JANC_EINVAL;
+  const std::string src = chemgen::generate(M, ndim);
+  if (src_len) *src_len = src.size();
+  if (src_out && cap > 0) { size_t n = src.size() < cap - 1 ? src.size() : cap - 1; memcpy(src_out, src.data(), n); src_out[n] = 0; }
+  if (cubin_bytes) {
+    std::vector<char> cubin;
+    std::string log;
+    *cubin_bytes = 0;
+    if (!jit_compile(src, cubin, log)) { fprintf(stderr, "janc_jit_probe: %s\n", log.c_str()); return JANC_ESTATE; }
+    *cubin_bytes = cubin.size();
+  }
+  return JANC_OK;
+}
+
+extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
+  if (!c || !m) return JANC_EINVAL;
+  int rc = fill_mech(m, c->mech, c->err);
+  if (rc) return rc;
+  jit_setup(c);
   c->ns = m->ns; c->nr = m->nr;
   c->nvar = c->g.ndim + 2 + m->ns - 1;
   c->P.nvar = c->nvar; c->P.ns = m->ns;
@@ -462,6 +589,15 @@ static void launch_chem_reg(janc_ctx *c, double *U) {
   k_chem_reg<NS, NT><<<cell_grid(c, NT, c->np), NT, smem, c->stream>>>(c->P, U);
 }
 static void do_chem(janc_ctx *c, double *U, Prof *pf) {
+  if (c->jit_kernel) {
+    const Params &P = c->P;
+    ChemArgs a{U, P.T, P.scal, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc};
+    void *args[] = {&a};
+    cudaLaunchKernel((const void *)c->jit_kernel, cell_grid(c, JANC_JIT_NT, c->np), dim3(JANC_JIT_NT, 1, 1), args, 0, c->stream);
+    c->launches++;
+    prof_mark(c, pf, 3);
+    return;
+  }
   switch (c->ns) {
     case 2: launch_chem_reg<2>(c, U); break;
     case 9: launch_chem_reg<9>(c, U); break;
