@@ -229,3 +229,52 @@ def test_cfg2_full_size_one_step(B, ref):
     case = I.config2()
     e = check(B, ref, case, 1, TOL1)
     print("cfg2 full-size per-field rel err", e)
+
+
+# ------------------------------------------------------------------ chemistry kernel selection
+def test_specialised_chemistry_kernel_is_the_one_running(B, mech9, mech20):
+    """janc_set_mechanism compiles the mechanism-specialised kernel (chemgen.h) for <= 12 unknowns;
+    larger mechanisms run the table-driven kernel.  Both are CUDA: there is no CPU path."""
+    c = I.config1(nx=32, ny=16)
+    s = B.Solver(c.grid, mech9)
+    assert s.chem_kernel() == "jit", s.jit_log()
+    s.close()
+    c0 = I.config0(n=64)
+    s = B.Solver(c0.grid, c0.mech)
+    assert s.chem_kernel() == "jit", s.jit_log()
+    s.close()
+    c4 = I.config4(n=16, nspheres=2, radius=3)
+    s = B.Solver(c4.grid, mech20)
+    assert s.chem_kernel() == "generic"
+    s.close()
+
+
+def test_table_driven_chemistry_fallback_parity(B, ref, monkeypatch):
+    """Same parity bar with the specialised kernel switched off (JANC_DISABLE_JIT=1): the table-driven
+    kernels of chem.cuh remain correct."""
+    monkeypatch.setenv("JANC_DISABLE_JIT", "1")
+    case = I.config1(nx=96, ny=40)
+    s = B.Solver(case.grid, case.mech)
+    assert s.chem_kernel() == "reg"
+    s.close()
+    check(B, ref, case, 1, TOL1)
+    check(B, ref, case, 20, TOL100)
+    case0 = I.config0(n=130)
+    check(B, ref, case0, 5, TOL100)
+
+
+def test_chemistry_pivoting_path(B, ref, mech9):
+    """Large dt makes off-diagonal entries of I - dt J dominate, so partial pivoting actually swaps rows
+    (the warp-wide skip must not change the answer): one fixed-dt step of pure chemistry on hot gas."""
+    nx, ny = 40, 24
+    rng = np.random.default_rng(7)
+    z = np.zeros((ny, nx))
+    Y = np.broadcast_to(I.hot_Y(9), (ny, nx, 9)).copy()
+    Y[..., :8] *= rng.uniform(0.2, 1.8, size=(ny, nx, 8)); Y[..., 8] = 1.0 - Y[..., :8].sum(-1)
+    T = 1500.0 + 1500.0 * rng.random((ny, nx))
+    U = I.prim_to_cons(mech9, 2, z + 2.0e6, T, Y, [z, z])
+    g = I.Grid(2, (nx, ny, 1), (1e-3, 1e-3, 1), (0, 0, 0), (0, 0, 0))
+    case = I.Case("chem_big_dt", g, mech9, U.reshape(1, -1, 1, ny, nx), T.reshape(1, 1, ny, nx), 0.2, 1)
+    Ug, Tg, Ur, Tr = both(B, ref, case, 1, cfl=0.0, dt=2e-7)
+    e = field_errors(case, Ug, Ur)
+    assert e.max() <= 1e-8, e
