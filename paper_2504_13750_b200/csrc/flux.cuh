@@ -252,6 +252,7 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
   const double ax = slot_value(P.slots + slot_base + lev * 3 + 0), ay = slot_value(P.slots + slot_base + lev * 3 + 1);
   const double hx = 0.5 * P.invdx[lev][0], hy = 0.5 * P.invdx[lev][1];
   const int mxp = P.P[0] - 1, myp = P.P[1] - 1;     // last padded index (ragged tiles stay in the array)
+  const bool same = Uk == U0;                        // stage 0: U^n is the stage state, already in smem
 
   auto load_box = [&](double *dst, const double *src) {
 #pragma unroll 4
@@ -285,6 +286,16 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
       for (int i = 0; i < SEG; i++) sL[r * C::LP + xs + i] = (Fh[i] - Fh[i + 1]) * hx;
     }
     __syncthreads();
+    // U^n of this thread's output cells: requested before the y pencils, consumed after them
+    double u0v[SEG];
+    if (!same) {
+#pragma unroll
+      for (int q = 0; q < SEG; q++) {
+        const int o = tid + q * NT;
+        const int g0 = min(o0 + o % TX, P.n[0] - 1), g1 = min(o1 + o / TX, P.n[1] - 1);
+        u0v[q] = U0p[cell_index(P, g0, g1, 0) + (long long)m * P.pc];
+      }
+    }
     {  // y pencils: lanes run over columns
       const double cM = m == 2 ? 1.0 : 0.0;
       const int x = tid % TX, ys = (tid / TX) * SEG;
@@ -297,13 +308,15 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
     __syncthreads();
     // RK stage (increment form), coalesced
 #pragma unroll
-    for (int o = tid; o < TX * TY; o += NT) {
+    for (int q = 0; q < SEG; q++) {
+      const int o = tid + q * NT;
       const int lx = o % TX, ly = o / TX;
       const int g0 = o0 + lx, g1 = o1 + ly;
       if (g0 < P.n[0] && g1 < P.n[1]) {
         const long long id = cell_index(P, g0, g1, 0) + (long long)m * P.pc;
-        const double u0 = U0p[id];
-        Uop[id] = u0 + coef * ((sUm[(ly + 3) * PIT + lx + 3] - u0) + dt * sL[ly * C::LP + lx]);
+        const double uk = sUm[(ly + 3) * PIT + lx + 3];
+        const double u0 = same ? uk : u0v[q];
+        Uop[id] = u0 + coef * ((uk - u0) + dt * sL[ly * C::LP + lx]);
       }
     }
     __syncthreads();   // everyone is done with sU[m & 1] and sL

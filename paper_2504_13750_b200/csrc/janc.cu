@@ -35,6 +35,7 @@ struct janc_ctx {
   std::vector<int> level, nbr, parent, fkind;
   int parity;
   long long launches;
+  cudaKernel_t jit_prim;     // mechanism-specialised cons->prim kernel, null if not in use
   cudaKernel_t jit_kernel;   // mechanism-specialised chemistry kernel (chemgen.h), null if not in use
   std::string jit_log;
   unsigned long long id;
@@ -131,6 +132,7 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
   c->fkind.assign((size_t)c->np * nf, FK_PHYSICAL);
   c->id = g_next_id++;
   c->jit_kernel = nullptr;
+  c->jit_prim = nullptr;
   *out = c;
   return JANC_OK;
 }
@@ -260,29 +262,42 @@ static bool jit_compile(const std::string &src, std::vector<char> &cubin, std::s
   return ok;
 }
 
-// Generate + compile + load the chemistry kernel of c->mech; on any failure the generic kernels stay.
+struct PrimArgs { const double *U; double *T; double *p; double *vel; double *dbgc; unsigned long long *slots;
+                  const int *level; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np, reduce, slot_base; };
+struct JitKernels { cudaKernel_t chem = nullptr, prim = nullptr; };
+
+static bool jit_chem_eligible(const MechC &M) { return M.ns >= 2 && M.nr >= 1 && M.ns - 1 <= JANC_JIT_MAX_N1; }
+
+// Generate + compile + load the kernels specialised for c->mech (cons->prim for any mechanism, chemistry
+// for <= JANC_JIT_MAX_N1 unknowns); on any failure the table-driven kernels stay.
 static void jit_setup(janc_ctx *c) {
   c->jit_kernel = nullptr;
+  c->jit_prim = nullptr;
   c->jit_log.clear();
   const MechC &M = c->mech;
-  if (M.ns < 2 || M.nr < 1 || M.ns - 1 > JANC_JIT_MAX_N1) { c->jit_log = "mechanism outside the specialised range"; return; }
   const char *off = getenv("JANC_DISABLE_JIT");
   if (off && off[0] && off[0] != '0') { c->jit_log = "disabled by JANC_DISABLE_JIT"; return; }
-  const std::string src = chemgen::generate(M, c->g.ndim);
-  static std::map<std::string, cudaKernel_t> cache;          // per process; one device per process
+  const bool chem = jit_chem_eligible(M);
+  std::string src = chemgen::generate_prim(M, c->g.ndim);
+  if (chem) src += chemgen::generate(M, c->g.ndim);
+  else c->jit_log = "chemistry: mechanism outside the specialised range; ";
+  static std::map<std::string, JitKernels> cache;          // per process; one device per process
   const std::string key = std::to_string(c->device) + "\n" + src;
   auto it = cache.find(key);
-  if (it != cache.end()) { c->jit_kernel = it->second; return; }
+  if (it != cache.end()) { c->jit_kernel = it->second.chem; c->jit_prim = it->second.prim; return; }
   std::vector<char> cubin;
-  if (!jit_compile(src, cubin, c->jit_log)) return;
+  std::string log;
+  if (!jit_compile(src, cubin, log)) { c->jit_log += log; return; }
   cudaLibrary_t lib;
   cudaError_t e = cudaLibraryLoadData(&lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
-  if (e != cudaSuccess) { c->jit_log = std::string("cudaLibraryLoadData: ") + cudaGetErrorString(e); cudaGetLastError(); return; }
-  cudaKernel_t k;
-  e = cudaLibraryGetKernel(&k, lib, "k_chem_jit");
-  if (e != cudaSuccess) { c->jit_log = std::string("cudaLibraryGetKernel: ") + cudaGetErrorString(e); cudaGetLastError(); return; }
+  if (e != cudaSuccess) { c->jit_log += std::string("cudaLibraryLoadData: ") + cudaGetErrorString(e); cudaGetLastError(); return; }
+  JitKernels k;
+  e = cudaLibraryGetKernel(&k.prim, lib, "k_prim_jit");
+  if (e == cudaSuccess && chem) e = cudaLibraryGetKernel(&k.chem, lib, "k_chem_jit");
+  if (e != cudaSuccess) { c->jit_log += std::string("cudaLibraryGetKernel: ") + cudaGetErrorString(e); cudaGetLastError(); return; }
   cache[key] = k;
-  c->jit_kernel = k;
+  c->jit_kernel = k.chem;
+  c->jit_prim = k.prim;
 }
 
 extern "C" const char *janc_chem_kernel(const janc_ctx *c) {
@@ -299,8 +314,8 @@ extern "C" int janc_jit_probe(const janc_mech *m, int ndim, char *src_out, size_
   std::string err;
   int rc = fill_mech(m, M, err);
   if (rc) return rc;
-  if (M.ns < 2 || M.nr < 1 || M.ns - 1 > JANC_JIT_MAX_N1) return JANC_EINVAL;
-  const std::string src = chemgen::generate(M, ndim);
+  std::string src = chemgen::generate_prim(M, ndim);
+  if (jit_chem_eligible(M)) src += chemgen::generate(M, ndim);
   if (src_len) *src_len = src.size();
   if (src_out && cap > 0) { size_t n = src.size() < cap - 1 ? src.size() : cap - 1; memcpy(src_out, src.data(), n); src_out[n] = 0; }
   if (cubin_bytes) {
@@ -511,6 +526,16 @@ static void launch_prim(janc_ctx *c, const double *U, int reduce, int slot_base,
   k_prim<NS><<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, U, reduce, slot_base, dbgc);
 }
 static void do_prim(janc_ctx *c, const double *U, int reduce, int slot_base, double *dbgc, Prof *pf) {
+  if (c->jit_prim) {
+    const Params &P = c->P;
+    PrimArgs a{U, P.T, P.p, P.vel, dbgc, P.slots, P.level, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2],
+               P.st[0], P.st[1], P.st[2], P.pc, P.np, reduce, slot_base};
+    void *args[] = {&a};
+    cudaLaunchKernel((const void *)c->jit_prim, cell_grid(c, 256, c->np), dim3(256, 1, 1), args, 0, c->stream);
+    c->launches++;
+    prof_mark(c, pf, 0);
+    return;
+  }
   switch (c->ns) {
     case 1: launch_prim<1>(c, U, reduce, slot_base, dbgc); break;
     case 2: launch_prim<2>(c, U, reduce, slot_base, dbgc); break;

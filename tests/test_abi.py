@@ -77,4 +77,5 @@ def test_specialised_chemistry_source_compiles_for_sm100a(L, mech9):
         assert nbytes and nbytes > 1000
         # every reaction and every unknown appears as literals: no table lookups in the kernel
         assert f"// reaction {mech.nr - 1}" in src and f"A{mech.ns - 2}_{mech.ns - 2}" in src
-        assert "c_mech" not in src and "__shared__" not in src
+        assert "k_prim_jit" in src and "c_mech" not in src
+        assert "__shared__" not in src[src.index("k_chem_jit"):]
