@@ -27,12 +27,15 @@ METRIC = "fp64 cell-updates/sec (RK3 step incl. point-implicit chemistry)"
 UNIT = "cell-updates/s"
 
 # algorithmic work / traffic per cell-update, derived in DESIGN.md "Roofline arithmetic"
-WENO_OPS = 46            # DP instructions (FMA = 1, division = 1) of one WENO5-JS reconstruction
+WENO_OPS = 38            # DP instructions (FMA = 1) of one WENO5-JS reconstruction in difference form
+                         # (flux.cuh: differences 4 amortised, betas 9, squares 3, weights 6, candidates 4,
+                         #  numerator 3, denominator 2, reciprocal 5 + 1, final 1)
 
 
 def flux_ops_per_cell_stage(ndim, nvar):
-    # per component and direction: split (6) + 2 reconstructions + face sum/difference (4); RK update 3
-    return nvar * (ndim * (6 + 2 * WENO_OPS + 4) + 3)
+    # per component and direction: split flux 2f+- (3) + 2 reconstructions + face sum, difference, scale (3);
+    # RK update 3.  Pencil-end faces and ghost-row split fluxes (the kernel's redundancy) are NOT counted.
+    return nvar * (ndim * (3 + 2 * WENO_OPS + 3) + 3)
 
 
 def flux_bytes_per_cell_stage(ndim, nvar):
@@ -260,7 +263,7 @@ def main():
         fl_avg = fl_ms / max(fl_n, 1) * 1e-3
         ops = flux_ops_per_cell_stage(nd, nvar) * cells
         byt = flux_bytes_per_cell_stage(nd, nvar) * cells
-        roof = {"kernel": "k_flux_rk", "bound": "alu", "achieved": ops / fl_avg / 1e12, "peak": dfma / 1e12,
+        roof = {"kernel": "k_flux_rk2" if nd == 2 else "k_flux_rk", "bound": "alu", "achieved": ops / fl_avg / 1e12, "peak": dfma / 1e12,
                 "unit": "T fp64-instr/s (FMA=1)", "frac": ops / fl_avg / dfma, "traffic": None,
                 "peak_source": "measured: register-resident DFMA microbenchmark in this run",
                 "avg_launch_ms": fl_avg * 1e3, "launches_timed": fl_n,

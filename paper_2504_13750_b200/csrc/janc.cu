@@ -61,9 +61,11 @@ static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 __global__ void __launch_bounds__(256) k_pack(Params P, const double *__restrict__ src, double *__restrict__ dst,
                                               int nf, int unpack, double fill) {
   const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned nbx = (unsigned)((ncell + blockDim.x - 1) / blockDim.x);   // grid.x = nbx * np * nf (grid.y is limited to 65535)
+  const long long t = (long long)(blockIdx.x % nbx) * blockDim.x + threadIdx.x;
   if (t >= ncell) return;
-  const int f = blockIdx.y % nf, patch = blockIdx.y / nf;
+  const int fp = blockIdx.x / nbx;
+  const int f = fp % nf, patch = fp / nf;
   const int i = (int)(t % P.n[0]);
   const long long r = t / P.n[0];
   const int j = (int)(r % P.n[1]), k = (int)(r / P.n[1]);
@@ -101,6 +103,7 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
   c->device = device;
   c->stream = (cudaStream_t)cuda_stream;
   c->np = grid->n_patches > 0 ? grid->n_patches : 1;
+  if (c->np > 65535) { delete c; return JANC_EINVAL; }   // patches ride on gridDim.y
   if (grid->n_patches <= 0) { c->g.n_levels = 1; c->g.ratio = 2; }
   if (c->g.n_levels < 1 || c->g.n_levels > 2 || (c->g.n_levels == 2 && c->g.ratio != 2)) { delete c; return JANC_EINVAL; }
   Params &P = c->P;
@@ -448,6 +451,10 @@ static dim3 cell_grid(const janc_ctx *c, int threads, int ny) {
   return dim3((unsigned)((c->ncell + threads - 1) / threads), (unsigned)ny, 1);
 }
 
+static dim3 pack_grid(const janc_ctx *c, int nfields_total) {
+  return dim3((unsigned)((c->ncell + 255) / 256) * (unsigned)nfields_total, 1, 1);
+}
+
 extern "C" int janc_set_state(janc_ctx *c, const double *U, const double *Tg, int on_device) {
   if (!c || !U) return JANC_EINVAL;
   if (!c->have_ws) { c->err = "bind a workspace first"; return JANC_ESTATE; }
@@ -459,8 +466,8 @@ extern "C" int janc_set_state(janc_ctx *c, const double *U, const double *Tg, in
     dU = c->stageU;
     if (Tg) { CK(cudaMemcpyAsync(c->stageT, Tg, nT * 8, cudaMemcpyHostToDevice, c->stream)); dT = c->stageT; }
   }
-  k_pack<<<cell_grid(c, 256, c->np * c->nvar), 256, 0, c->stream>>>(c->P, dU, c->A, c->nvar, 0, 0.0);
-  k_pack<<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, dT, c->P.T, 1, 0, 1000.0);
+  k_pack<<<pack_grid(c, c->np * c->nvar), 256, 0, c->stream>>>(c->P, dU, c->A, c->nvar, 0, 0.0);
+  k_pack<<<pack_grid(c, c->np), 256, 0, c->stream>>>(c->P, dT, c->P.T, 1, 0, 1000.0);
   c->launches += 2;
   CK(cudaMemsetAsync(c->P.flag, 0, 4, c->stream));
   CK(cudaMemsetAsync(c->P.slots, 0, 36 * 8, c->stream));
@@ -493,13 +500,13 @@ extern "C" int janc_get_state(janc_ctx *c, double *U, double *T, int on_device) 
   const size_t nU = (size_t)c->np * c->nvar * c->ncell, nT = (size_t)c->np * c->ncell;
   if (U) {
     double *dst = on_device ? U : c->stageU;
-    k_pack<<<cell_grid(c, 256, c->np * c->nvar), 256, 0, c->stream>>>(c->P, c->A, dst, c->nvar, 1, 0.0);
+    k_pack<<<pack_grid(c, c->np * c->nvar), 256, 0, c->stream>>>(c->P, c->A, dst, c->nvar, 1, 0.0);
     c->launches++;
     if (!on_device) CK(cudaMemcpyAsync(U, c->stageU, nU * 8, cudaMemcpyDeviceToHost, c->stream));
   }
   if (T) {
     double *dst = on_device ? T : c->stageT;
-    k_pack<<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, c->P.T, dst, 1, 1, 0.0);
+    k_pack<<<pack_grid(c, c->np), 256, 0, c->stream>>>(c->P, c->P.T, dst, 1, 1, 0.0);
     c->launches++;
     if (!on_device) CK(cudaMemcpyAsync(T, c->stageT, nT * 8, cudaMemcpyDeviceToHost, c->stream));
   }
@@ -737,7 +744,7 @@ extern "C" int janc_debug_cons2prim(janc_ctx *c, double *T, double *p, double *c
   for (int q = 0; q < 3; q++) {
     if (!dsts[q]) continue;
     double *dst = on_device ? dsts[q] : c->stageT;
-    k_pack<<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, srcs[q], dst, 1, 1, 0.0);
+    k_pack<<<pack_grid(c, c->np), 256, 0, c->stream>>>(c->P, srcs[q], dst, 1, 1, 0.0);
     c->launches++;
     if (!on_device) {
       CK(cudaMemcpyAsync(dsts[q], c->stageT, nT * 8, cudaMemcpyDeviceToHost, c->stream));

@@ -231,6 +231,14 @@ def test_cfg2_full_size_one_step(B, ref):
     print("cfg2 full-size per-field rel err", e)
 
 
+def test_cfg3_full_size_one_step(B, ref):
+    """Config 3 at full size (8192 patches of 16 x 16, 2 levels): one synchronous step against the oracle."""
+    case = I.config3()
+    assert case.grid.n_patches == 8192
+    e = check(B, ref, case, 1, TOL1)
+    print("cfg3 full-size per-field rel err", e)
+
+
 # ------------------------------------------------------------------ chemistry kernel selection
 def test_specialised_chemistry_kernel_is_the_one_running(B, mech9, mech20):
     """janc_set_mechanism compiles the mechanism-specialised kernel (chemgen.h) for <= 12 unknowns;
