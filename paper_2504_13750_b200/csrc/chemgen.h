@@ -22,6 +22,7 @@
 
 #define JANC_JIT_MAX_N1 12
 #define JANC_JIT_NT 64
+#define JANC_JIT_NT_BIG 32
 
 namespace chemgen {
 
@@ -100,7 +101,57 @@ inline void emit_newton(Emitter &E, const MechC &M) {
   E.line("ok = ok && (T > 0.0) && isfinite(T);");
 }
 
-inline std::string generate(const MechC &M, int ndim) {
+// Shared-memory tail of the big-mechanism kernel: A = I - dt J in place (column Ns-1 becomes the
+// right-hand side), Gaussian elimination with partial pivoting, back substitution, store.
+inline void emit_big_solve(Emitter &E, const MechC &M, int ndim, const Acc &accW) {
+  const int ns = M.ns, n1 = ns - 1, NT = JANC_JIT_NT_BIG;
+  const std::string sNT = I(NT), sNS = I(ns), sN1 = I(n1);
+  std::string iw = "const double iW_[" + sN1 + "] = {";
+  for (int l = 0; l < n1; l++) iw += num(M.invW[l]) + (l + 1 < n1 ? ", " : "};");
+  E.line(iw);
+  E.line("#define EL(r, c) S[((r) * " + sNS + " + (c)) * " + sNT + "]");
+  for (int k = 0; k < n1; k++) {
+    const std::string sk = I(k);
+    E.line("{ const double dl = EL(" + sk + ", " + sN1 + ") * " + num(M.invW[n1]) + ", mw = -dt * " + num(M.W[k]) + ";");
+    E.line("  #pragma unroll 1");
+    E.line("  for (int l = 0; l < " + sN1 + "; l++) EL(" + sk + ", l) = fma(mw, fma(EL(" + sk + ", l), iW_[l], -dl), l == " + sk + " ? 1.0 : 0.0);");
+    E.line("  EL(" + sk + ", " + sN1 + ") = " + (accW.set[k] ? "-mw * w" + sk : std::string("0.0")) + "; }");
+  }
+  E.line("#pragma unroll 1");
+  E.line("for (int c = 0; c < " + sN1 + "; c++) {");
+  E.line("  int piv = c; double best = fabs(EL(c, c));");
+  E.line("  for (int r = c + 1; r < " + sN1 + "; r++) { const double v = fabs(EL(r, c)); if (v > best) { best = v; piv = r; } }");
+  E.line("  if (!(best > 0.0)) ok = false;");
+  E.line("  if (piv != c) for (int b = c; b <= " + sN1 + "; b++) { const double x_ = EL(c, b); EL(c, b) = EL(piv, b); EL(piv, b) = x_; }");
+  E.line("  const double ip = 1.0 / EL(c, c);");
+  E.line("  for (int r = c + 1; r < " + sN1 + "; r++) {");
+  E.line("    const double f = EL(r, c) * ip;");
+  E.line("    for (int b = c + 1; b <= " + sN1 + "; b++) EL(r, b) = fma(-f, EL(c, b), EL(r, b));");
+  E.line("  }");
+  E.line("  EL(c, c) = ip;");
+  E.line("}");
+  E.line("#pragma unroll 1");
+  E.line("for (int r = " + I(n1 - 1) + "; r >= 0; r--) {");
+  E.line("  double sum = EL(r, " + sN1 + ");");
+  E.line("  for (int b = r + 1; b < " + sN1 + "; b++) sum = fma(-EL(r, b), EL(b, " + sN1 + "), sum);");
+  E.line("  EL(r, " + sN1 + ") = sum * EL(r, r);");
+  E.line("}");
+  E.line("#pragma unroll 1");
+  E.line("for (int k = 0; k < " + sN1 + "; k++) {");
+  E.line("  const double d_ = EL(k, " + sN1 + ");");
+  E.line("  if (!isfinite(d_)) ok = false;");
+  E.line("  if (live) Up[(" + I(ndim + 2) + " + k) * a.pc] += d_;");
+  E.line("}");
+  E.line("if (!ok && live) *a.flag = 1;");
+  E.line("#undef EL");
+}
+
+// big == false: everything in registers (N1 <= JANC_JIT_MAX_N1).
+// big == true : the (Ns-1) x Ns derivative matrix / linear system lives in shared memory as [entry][lane]
+//               (32 threads per CTA, conflict-free); rates and the sparse Jacobian scatter are still
+//               specialised (literal addresses), the dense elimination is a loop over shared memory.
+inline std::string generate(const MechC &M, int ndim, bool big = false) {
+  const int NT = big ? JANC_JIT_NT_BIG : JANC_JIT_NT;
   const char *mb_ = getenv("JANC_JIT_MINB");            // experiment knob: min CTAs per SM
   const std::string MINB_STR = mb_ && mb_[0] ? std::string(", ") + mb_ : std::string("");
   const int ns = M.ns, nr = M.nr, n1 = ns - 1, nvar = ndim + 2 + n1;
@@ -109,9 +160,15 @@ inline std::string generate(const MechC &M, int ndim) {
   src += "// generated by chemgen.h for ns=" + I(ns) + " nr=" + I(nr) + " ndim=" + I(ndim) + "\n";
   src += "struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2;"
          " long long st0, st1, st2, pc; };\n";
-  src += "extern \"C\" __global__ void __launch_bounds__(" + I(JANC_JIT_NT) + MINB_STR + ") k_chem_jit(ChemArgs a) {\n";
+  src += "extern \"C\" __global__ void __launch_bounds__(" + I(NT) + MINB_STR + ") k_chem_jit(ChemArgs a) {\n";
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
-  E.line("long long t = (long long)blockIdx.x * " + I(JANC_JIT_NT) + " + threadIdx.x;");
+  if (big) {
+    E.line("extern __shared__ double sm_[];");
+    E.line("double *S = sm_ + threadIdx.x;          // entry i of this cell's matrix: S[i * " + I(NT) + "]");
+    E.line("#pragma unroll 1");
+    E.line("for (int i_ = 0; i_ < " + I(n1 * ns) + "; i_++) S[i_ * " + I(NT) + "] = 0.0;");
+  }
+  E.line("long long t = (long long)blockIdx.x * " + I(NT) + " + threadIdx.x;");
   E.line("const bool live = t < ncell;");
   E.line("if (!live) t = ncell - 1;   // idle lanes recompute the last cell and store nothing");
   E.line("const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;");
@@ -203,8 +260,20 @@ inline std::string generate(const MechC &M, int ndim) {
       if (dq.empty()) continue;
       const std::string dn = "dq" + si + "_" + I(j);
       E.line("const double " + dn + " = " + dq + ";");
-      for (int k = 0; k < n1; k++) accum(E, accD, k * ns + j, "D" + I(k) + "_" + I(j), dnu[k], dn);
+      for (int k = 0; k < n1; k++) {
+        if (!big) { accum(E, accD, k * ns + j, "D" + I(k) + "_" + I(j), dnu[k], dn); continue; }
+        if (dnu[k] == 0) continue;
+        const std::string el = "S[" + I((k * ns + j) * NT) + "]";
+        if (dnu[k] == 1) E.line(el + " += " + dn + ";");
+        else if (dnu[k] == -1) E.line(el + " -= " + dn + ";");
+        else E.line(el + " = fma(" + num((double)dnu[k]) + ", " + dn + ", " + el + ");");
+      }
     }
+  }
+  if (big) {
+    emit_big_solve(E, M, ndim, accW);
+    src += "}\n";
+    return src;
   }
   // ---- A = I - dt J,  J_kl = W_k (D_kl / W_l - D_kNs / W_Ns);  rhs = dt W_k wdot_k   (eq 4.12-4.13, A11)
   for (int k = 0; k < n1; k++) {
