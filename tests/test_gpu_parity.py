@@ -286,3 +286,28 @@ def test_chemistry_pivoting_path(B, ref, mech9):
     Ug, Tg, Ur, Tr = both(B, ref, case, 1, cfl=0.0, dt=2e-7)
     e = field_errors(case, Ug, Ur)
     assert e.max() <= 1e-8, e
+
+
+def test_gpu_detonation_speed_is_cj(B):
+    """Property check of the CUDA path on its own (no oracle): the same 1-D single-step detonation as
+    tests/test_oracle_cj.py reaches the closed-form Chapman-Jouguet speed."""
+    from tests.test_oracle_cj import d_cj, front_position
+    n, dx, ndrv = 1800, 1.0e-4, 10
+    mech = I.single_step_mechanism()
+    x = np.arange(n); drv = x < ndrv
+    p = np.where(drv, 4.0e6, 1.0e5); T = np.where(drv, 2500.0, 300.0)
+    Y = np.zeros((n, 2)); Y[:, 0] = 1.0
+    U = I.prim_to_cons(mech, 1, p, T, Y, [np.zeros(n)])
+    g = I.Grid(1, (n, 1, 1), (dx, 1.0, 1.0), (I.BC_REFLECT, 0, 0), (I.BC_OUTFLOW, 0, 0))
+    s = B.Solver(g, mech)
+    s.set_state(U.reshape(1, 4, 1, 1, n), T.reshape(1, 1, 1, n).astype(float))
+    t, marks = 0.0, []
+    for target in (4.0e-5, 8.0e-5):
+        while t < target:
+            t += s.step(50, cfl=0.4)
+        Uc, _ = s.get_state()
+        marks.append((t, front_position(Uc, dx)))
+    assert s.status == 0
+    s.close()
+    D = (marks[1][1] - marks[0][1]) / (marks[1][0] - marks[0][0])
+    assert abs(D - d_cj()) <= 0.004 * d_cj(), (D, d_cj())
