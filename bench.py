@@ -38,6 +38,11 @@ def flux_ops_per_cell_stage(ndim, nvar):
     return nvar * (ndim * (3 + 2 * WENO_OPS + 3) + 3)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
+# `ncu --set full` capture of this same command (profiles/r1d_summary.md); other workloads: not captured.
+NCU_TRAFFIC_BYTES = {"cfg2_2d_channel_4096x512": 6.32e8}
+
+
 def flux_bytes_per_cell_stage(ndim, nvar):
     # read U^(k) (nvar) + p + u_d (ndim) + U^n (nvar, stages 2,3 -> counted always), write U^(k+1) (nvar)
     return (3 * nvar + 1 + ndim) * 8
@@ -264,7 +269,8 @@ def main():
         ops = flux_ops_per_cell_stage(nd, nvar) * cells
         byt = flux_bytes_per_cell_stage(nd, nvar) * cells
         roof = {"kernel": "k_flux_rk2" if nd == 2 else "k_flux_rk", "bound": "alu", "achieved": ops / fl_avg / 1e12, "peak": dfma / 1e12,
-                "unit": "T fp64-instr/s (FMA=1)", "frac": ops / fl_avg / dfma, "traffic": None,
+                "unit": "T fp64-instr/s (FMA=1)", "frac": ops / fl_avg / dfma, "traffic": NCU_TRAFFIC_BYTES.get(case.name),
+                "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1d_summary.md)",
                 "peak_source": "measured: register-resident DFMA microbenchmark in this run",
                 "avg_launch_ms": fl_avg * 1e3, "launches_timed": fl_n,
                 "hbm": {"achieved": byt / fl_avg / 1e9, "peak": hbm_peak, "unit": "GB/s",
