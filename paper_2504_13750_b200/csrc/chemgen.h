@@ -126,6 +126,7 @@ inline void emit_big_solve(Emitter &E, const MechC &M, int ndim, const Acc &accW
   E.line("  const double ip = 1.0 / EL(c, c);");
   E.line("  for (int r = c + 1; r < " + sN1 + "; r++) {");
   E.line("    const double f = EL(r, c) * ip;");
+  E.line("    #pragma unroll 4");
   E.line("    for (int b = c + 1; b <= " + sN1 + "; b++) EL(r, b) = fma(-f, EL(c, b), EL(r, b));");
   E.line("  }");
   E.line("  EL(c, c) = ip;");

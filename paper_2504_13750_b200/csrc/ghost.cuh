@@ -5,6 +5,8 @@
 #pragma once
 #include "common.cuh"
 
+#define GHOST_FPT 4
+
 __device__ __forceinline__ int floordiv_i(int a, int b) {
   int q = a / b;
   if ((a % b != 0) && ((a < 0) != (b < 0))) q--;
@@ -17,11 +19,20 @@ __global__ void __launch_bounds__(256) k_ghost(Params P, double *__restrict__ U,
   const int patch = blockIdx.y;
   if (P.level[patch] != lev) return;
   const int nf = 2 * P.ndim;
-  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= (long long)nf * JANC_NG * amax) return;
-  const int t = (int)(idx % amax);
-  const int g = (int)((idx / amax) % JANC_NG) + 1;
-  const int f = (int)(idx / ((long long)amax * JANC_NG));
+  const int nfield = P.nvar + 2 + P.ndim;          // U components, T, p, u_d
+  const int ngrp = (nfield + GHOST_FPT - 1) / GHOST_FPT;   // a thread copies GHOST_FPT fields of one ghost cell
+  // 32-bit index arithmetic: one patch has far fewer than 2^31 (ghost cell, field group) items
+  unsigned idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned ncellf = (unsigned)(nf * JANC_NG * amax);
+  if (idx >= ncellf * (unsigned)ngrp) return;
+  const int grp = (int)(idx / ncellf);
+  idx -= (unsigned)grp * ncellf;
+  const int f = (int)(idx / (unsigned)(amax * JANC_NG));
+  const int r_ = (int)(idx - (unsigned)(f * amax * JANC_NG));
+  // x faces: the 3 layers are contiguous in memory, so the layer index runs fastest (one 32-byte
+  // sector per ghost row instead of three); y / z faces: x runs fastest
+  const int t = (f >> 1) == 0 ? r_ / JANC_NG : r_ % amax;
+  const int g = ((f >> 1) == 0 ? r_ % JANC_NG : r_ / amax) + 1;
   const int d = f >> 1, side = f & 1;
   const int e1 = d == 0 ? 1 : 0;            // fastest tangential dim
   const int e2 = d == 2 ? 1 : 2;            // slowest tangential dim
@@ -50,19 +61,23 @@ __global__ void __launch_bounds__(256) k_ghost(Params P, double *__restrict__ U,
   }
   const long long di = (long long)patch * P.pc + cell_index(P, dst[0], dst[1], dst[2]);
   const long long si = (long long)q * P.pc + cell_index(P, src[0], src[1], src[2]);
-  const long long dU = di + (long long)patch * (P.nvar - 1) * P.pc;   // = patch*nvar*pc + cell
-  const long long sU = si + (long long)q * (P.nvar - 1) * P.pc;
-  for (int v = 0; v < P.nvar; v++) {
-    double val = U[sU + (long long)v * P.pc];
-    if (flip && v == 1 + d) val = -val;
-    U[dU + (long long)v * P.pc] = val;
-  }
-  P.T[di] = P.T[si];
-  P.p[di] = P.p[si];
-  for (int e = 0; e < P.ndim; e++) {
-    double val = P.vel[(long long)e * P.np * P.pc + si];
-    if (flip && e == d) val = -val;
-    P.vel[(long long)e * P.np * P.pc + di] = val;
+  const long long cd = di - (long long)patch * P.pc, cs = si - (long long)q * P.pc;
+  const int f1 = min(nfield, (grp + 1) * GHOST_FPT);
+  for (int fld = grp * GHOST_FPT; fld < f1; fld++) {
+    if (fld < P.nvar) {
+      double val = U[((long long)q * P.nvar + fld) * P.pc + cs];
+      if (flip && fld == 1 + d) val = -val;
+      U[((long long)patch * P.nvar + fld) * P.pc + cd] = val;
+    } else if (fld == P.nvar) {
+      P.T[di] = P.T[si];
+    } else if (fld == P.nvar + 1) {
+      P.p[di] = P.p[si];
+    } else {
+      const int e = fld - P.nvar - 2;
+      double val = P.vel[(long long)e * P.np * P.pc + si];
+      if (flip && e == d) val = -val;
+      P.vel[(long long)e * P.np * P.pc + di] = val;
+    }
   }
 }
 

@@ -577,7 +577,7 @@ static void do_ghost(janc_ctx *c, double *U, Prof *pf) {
     for (int e = 0; e < nd; e++) if (e != d) a *= c->P.n[e];
     if (a > amax) amax = a;
   }
-  const long long total = (long long)2 * nd * JANC_NG * amax;
+  const long long total = (long long)2 * nd * JANC_NG * amax * ((c->nvar + 2 + nd + GHOST_FPT - 1) / GHOST_FPT);
   dim3 grid((unsigned)((total + 255) / 256), (unsigned)c->np, 1);
   for (int lev = 0; lev < c->g.n_levels; lev++) {
     k_ghost<<<grid, 256, 0, c->stream>>>(c->P, U, lev, amax);
