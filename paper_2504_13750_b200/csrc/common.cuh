@@ -76,3 +76,9 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, doub
 __device__ __forceinline__ double slot_value(const unsigned long long *addr) {
   return __longlong_as_double((long long)*addr);
 }
+
+__device__ __forceinline__ int floordiv_i(int a, int b) {
+  int q = a / b;
+  if ((a % b != 0) && ((a < 0) != (b < 0))) q--;
+  return q;
+}

@@ -218,25 +218,69 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-template <int TX, int TY, int SEG>
+// Where the value of cell (i, j) of `patch` (interior coordinates, ghosts at -3..-1 and n..n+2) comes from:
+// the rule of k_ghost (ghost.cuh) followed to an interior cell -- same-level neighbour, physical BC
+// (periodic / reflect / outflow), or piecewise-constant injection from the coarse parent, whose own ghost
+// is then resolved once more (reading A19).  flip bit d: the normal momentum / velocity of direction d
+// changes sign (slip wall, A15).  Corner ghosts are never read by the sweeps (A21).
+__device__ __forceinline__ void ghost_source2d(const Params &P, int patch, int i, int j, int &q, int &ci, int &cj, int &flip) {
+  q = patch; ci = i; cj = j; flip = 0;
+#pragma unroll 1
+  for (int pass = 0; pass < 2; pass++) {
+    const bool ox = ci < 0 || ci >= P.n[0], oy = cj < 0 || cj >= P.n[1];
+    if (!ox && !oy) return;
+    if (ox && oy) { ci = min(max(ci, 0), P.n[0] - 1); cj = min(max(cj, 0), P.n[1] - 1); return; }
+    const int d = ox ? 0 : 1;
+    const int cd = ox ? ci : cj;
+    const int side = cd < 0 ? 0 : 1;
+    const int g = side == 0 ? -cd : cd - P.n[d] + 1;
+    const int f = 2 * d + side;
+    const int kind = P.fkind[q * 4 + f];
+    const int bc = side == 0 ? P.bc_lo[d] : P.bc_hi[d];
+    int nd_ = cd;
+    bool done = true;
+    if (kind == FK_NEIGHBOUR || (kind == FK_PHYSICAL && bc == 0)) {
+      if (kind == FK_NEIGHBOUR) q = P.nbr[q * 4 + f];
+      nd_ = side == 0 ? P.n[d] - g : g - 1;
+    } else if (kind == FK_PHYSICAL && bc == 1) {
+      nd_ = side == 0 ? g - 1 : P.n[d] - g;
+      flip |= 1 << d;
+    } else if (kind == FK_PHYSICAL) {
+      nd_ = side == 0 ? 0 : P.n[d] - 1;
+    } else {
+      const int *par = P.parent + q * 3;
+      ci = floordiv_i(par[1] * P.n[0] + ci, P.ratio);
+      cj = floordiv_i(par[2] * P.n[1] + cj, P.ratio);
+      q = par[0];
+      done = false;
+    }
+    if (done) { if (ox) ci = nd_; else cj = nd_; return; }
+  }
+}
+
+// GATHER: the tile is a whole patch (n <= TX, TY) and the halo of the box is fetched straight from the cells
+// the ghost rule points at -- the ghost layers are never written to HBM and k_ghost is not launched.
+template <int TX, int TY, int SEG, bool GATHER = false>
 struct Flux2Cfg {
   static constexpr int NT = TX * TY / SEG;
   static constexpr int BX = TX + 6, BY = TY + 6;
   static constexpr int PIT = BX | 1;
   static constexpr int BOX = PIT * BY;
   static constexpr int LP = TX | 1;
-  static constexpr size_t SMEM = (size_t)(5 * BOX + TY * LP) * sizeof(double);
+  static constexpr size_t SMEM = (size_t)(5 * BOX + TY * LP) * sizeof(double) + (GATHER ? (size_t)BX * BY * 12 : 0);
   static constexpr int MINB = 512 / NT > 0 ? 512 / NT : 1;      // keeps the kernel at <= 128 registers
   static_assert(TX % SEG == 0 && TY % SEG == 0, "tile % SEG");
 };
 
-template <int TX, int TY, int SEG>
-__global__ void __launch_bounds__(Flux2Cfg<TX, TY, SEG>::NT, Flux2Cfg<TX, TY, SEG>::MINB)
+template <int TX, int TY, int SEG, bool GATHER>
+__global__ void __launch_bounds__(Flux2Cfg<TX, TY, SEG, GATHER>::NT, Flux2Cfg<TX, TY, SEG, GATHER>::MINB)
 k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uout, int slot_base, double coef) {
-  using C = Flux2Cfg<TX, TY, SEG>;
+  using C = Flux2Cfg<TX, TY, SEG, GATHER>;
   constexpr int NT = C::NT, PIT = C::PIT;
   extern __shared__ double flux_smem[];
   double *sp = flux_smem, *su = sp + C::BOX, *sv = su + C::BOX, *sU = sv + C::BOX, *sL = sU + 2 * C::BOX;
+  int *sq = (int *)(sL + TY * C::LP), *sc = sq + C::BX * C::BY;           // GATHER: source patch / cell
+  unsigned char *sfl = (unsigned char *)(sc + C::BX * C::BY);             //         flip bits
 
   const int tid = threadIdx.x;
   const int patch = blockIdx.y;
@@ -254,20 +298,40 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
   const int mxp = P.P[0] - 1, myp = P.P[1] - 1;     // last padded index (ragged tiles stay in the array)
   const bool same = Uk == U0;                        // stage 0: U^n is the stage state, already in smem
 
-  auto load_box = [&](double *dst, const double *src) {
+  if (GATHER) {
+    for (int it = tid; it < C::BX * C::BY; it += NT) {
+      int q, ci, cj, fl;
+      ghost_source2d(P, patch, it % C::BX - 3, it / C::BX - 3, q, ci, cj, fl);
+      sq[it] = q;
+      sc[it] = (int)cell_index(P, ci, cj, 0);
+      sfl[it] = (unsigned char)fl;
+    }
+    __syncthreads();
+  }
+  // copy field `fld` of an array with `fpp` fields per patch into a box
+  auto load_box = [&](double *dst, const double *base, int fpp, int fld) {
 #pragma unroll 4
     for (int it = tid; it < C::BX * C::BY; it += NT) {
       const int bx = it % C::BX, by = it / C::BX;
-      const int gx = min(o0 + bx, mxp), gy = min(o1 + by, myp);
-      cp_async8(dst + by * PIT + bx, src + (long long)gy * st1 + gx);
+      if (GATHER) {
+        cp_async8(dst + by * PIT + bx, base + ((long long)sq[it] * fpp + fld) * P.pc + sc[it]);
+      } else {
+        const int gx = min(o0 + bx, mxp), gy = min(o1 + by, myp);
+        cp_async8(dst + by * PIT + bx, base + ((long long)patch * fpp + fld) * P.pc + (long long)gy * st1 + gx);
+      }
     }
   };
-  load_box(sp, P.p + pbase);
-  load_box(su, P.vel + pbase);
-  load_box(sv, P.vel + (long long)P.np * P.pc + pbase);
-  load_box(sU, Ukp);
+  // slip walls: negate the mirrored normal momentum / velocity (bit = 1 << direction)
+  auto fix_flips = [&](double *box, int bit) {
+    for (int it = tid; it < C::BX * C::BY; it += NT)
+      if (sfl[it] & bit) { double *e = box + (it / C::BX) * PIT + it % C::BX; *e = -*e; }
+  };
+  load_box(sp, P.p, 1, 0);
+  load_box(su, P.vel, 1, 0);
+  load_box(sv, P.vel + (long long)P.np * P.pc, 1, 0);
+  load_box(sU, Uk, P.nvar, 0);
   cp_async_commit();
-  if (P.nvar > 1) load_box(sU + C::BOX, Ukp + P.pc);
+  if (P.nvar > 1) load_box(sU + C::BOX, Uk, P.nvar, 1);
   cp_async_commit();
 
 #pragma unroll 1
@@ -276,6 +340,11 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
     const double cEn = m == 3 ? 1.0 : 0.0;
     cp_async_wait<1>();
     __syncthreads();
+    if (GATHER && m <= 2) {
+      if (m == 0) { fix_flips(su, 1); fix_flips(sv, 2); }
+      else fix_flips(sU + (m & 1) * C::BOX, m);                 // m = 1: x momentum (bit 1), m = 2: y momentum (bit 2)
+      __syncthreads();
+    }
     {  // x pencils: lanes run over rows
       const double cM = m == 1 ? 1.0 : 0.0;
       const int r = tid % TY, xs = (tid / TY) * SEG;
@@ -320,7 +389,7 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
       }
     }
     __syncthreads();   // everyone is done with sU[m & 1] and sL
-    if (m + 2 < P.nvar) load_box(sU + (m & 1) * C::BOX, Ukp + (long long)(m + 2) * P.pc);
+    if (m + 2 < P.nvar) load_box(sU + (m & 1) * C::BOX, Uk, P.nvar, m + 2);
     cp_async_commit();
   }
 }

@@ -7,12 +7,6 @@
 
 #define GHOST_FPT 4
 
-__device__ __forceinline__ int floordiv_i(int a, int b) {
-  int q = a / b;
-  if ((a % b != 0) && ((a < 0) != (b < 0))) q--;
-  return q;
-}
-
 // grid: (ceil(nf*3*amax / 256), np); only patches with level == lev act (level 0 must be complete
 // before level 1 injects from its padded parent).
 __global__ void __launch_bounds__(256) k_ghost(Params P, double *__restrict__ U, int lev, int amax) {

@@ -569,7 +569,11 @@ static void do_prim(janc_ctx *c, const double *U, int reduce, int slot_base, dou
   prof_mark(c, pf, 0);
 }
 
+// 2-D patches of at most 16 x 16 cells: the flux kernel gathers its halo itself (flux.cuh, GATHER); no ghost fill
+static bool gather_mode(const janc_ctx *c) { return c->g.ndim == 2 && c->P.n[0] <= 16 && c->P.n[1] <= 16; }
+
 static void do_ghost(janc_ctx *c, double *U, Prof *pf) {
+  if (gather_mode(c)) return;
   const int nd = c->g.ndim;
   int amax = 1;
   for (int d = 0; d < nd; d++) {
@@ -599,24 +603,25 @@ static void launch_flux(janc_ctx *c, const double *Uk, const double *U0, double 
   k_flux_rk<NDIM, TX, TY, TZ, SEG><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
 }
 
-template <int TX, int TY, int SEG>
+template <int TX, int TY, int SEG, bool GATHER = false>
 static void launch_flux2(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef) {
-  using C = Flux2Cfg<TX, TY, SEG>;
+  using C = Flux2Cfg<TX, TY, SEG, GATHER>;
   const Params &P = c->P;
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(k_flux_rk2<TX, TY, SEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    cudaFuncSetAttribute(k_flux_rk2<TX, TY, SEG, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     attr_done = true;
   }
   const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY));
-  k_flux_rk2<TX, TY, SEG><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
+  k_flux_rk2<TX, TY, SEG, GATHER><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
 }
 
 static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef, Prof *pf) {
   const Params &P = c->P;
   if (c->g.ndim == 1) launch_flux<1, 128, 1, 1, 4>(c, Uk, U0, Uout, slot_base, coef);
   else if (c->g.ndim == 2) {
-    if (P.n[0] <= 16 && P.n[1] <= 16) launch_flux2<16, 16, 8>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches
+    if (gather_mode(c)) launch_flux2<16, 16, 8, true>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches: halo gathered in-kernel
+    else if ((long long)c->np * c->ncell < 600000) launch_flux2<32, 16, 4>(c, Uk, U0, Uout, slot_base, coef);   // small grids: 4x the CTAs
     else launch_flux2<64, 16, 8>(c, Uk, U0, Uout, slot_base, coef);
   } else launch_flux<3, 32, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);
   c->launches++;
