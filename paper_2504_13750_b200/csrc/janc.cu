@@ -14,6 +14,7 @@
 #include "../../include/janc.h"
 #include "chem.cuh"
 #include "chemgen.h"
+#include "chemgen_roles.h"
 #include "flux.cuh"
 #include "ghost.cuh"
 #include "prim.cuh"
@@ -35,7 +36,7 @@ struct janc_ctx {
   std::vector<int> level, nbr, parent, fkind;
   int parity;
   long long launches;
-  int jit_chem_nt;
+  int jit_chem_nt, jit_chem_cells, jit_chem_mode;   // threads per CTA, cells per CTA, see jit_chem_mode()
   size_t jit_chem_smem;
   cudaKernel_t jit_prim;     // mechanism-specialised cons->prim kernel, null if not in use
   cudaKernel_t jit_kernel;   // mechanism-specialised chemistry kernel (chemgen.h), null if not in use
@@ -271,12 +272,15 @@ struct PrimArgs { const double *U; double *T; double *p; double *vel; double *db
                   const int *level; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np, reduce, slot_base; };
 struct JitKernels { cudaKernel_t chem = nullptr, prim = nullptr; };
 
-// 0: table-driven kernel, 1: register-resident specialised kernel, 2: specialised kernel with the matrix in smem
+// 0: table-driven kernel, 1: register-resident specialised kernel (one thread per cell), 2: one thread per cell
+// with the matrix in smem, 3: 8 role-warps per 32 cells with the matrix columns in registers (chemgen_roles.h)
 static int jit_chem_mode(const MechC &M) {
   int max_n1 = JANC_JIT_MAX_N1;
-  if (const char *e = getenv("JANC_JIT_MAX_N1")) max_n1 = atoi(e);     // experiment knob
+  if (const char *e = getenv("JANC_JIT_MAX_N1")) max_n1 = atoi(e);     // test knob: push small mechanisms to the big path
   if (M.ns < 2 || M.nr < 1) return 0;
   if (M.ns - 1 <= max_n1) return 1;
+  const char *big = getenv("JANC_JIT_BIG");                            // test knob: "smem" selects mode 2
+  if (chemgen::roles_applicable(M) && !(big && strcmp(big, "smem") == 0)) return 3;
   const size_t smem = (size_t)(M.ns - 1) * M.ns * JANC_JIT_NT_BIG * sizeof(double);
   return smem <= 200 * 1024 ? 2 : 0;
 }
@@ -292,10 +296,13 @@ static void jit_setup(janc_ctx *c) {
   if (off && off[0] && off[0] != '0') { c->jit_log = "disabled by JANC_DISABLE_JIT"; return; }
   const int mode = jit_chem_mode(M);
   const bool chem = mode != 0;
-  c->jit_chem_nt = mode == 2 ? JANC_JIT_NT_BIG : JANC_JIT_NT;
-  c->jit_chem_smem = mode == 2 ? (size_t)(M.ns - 1) * M.ns * JANC_JIT_NT_BIG * sizeof(double) : 0;
+  c->jit_chem_mode = mode;
+  c->jit_chem_nt = mode == 3 ? JANC_ROLES * 32 : mode == 2 ? JANC_JIT_NT_BIG : JANC_JIT_NT;
+  c->jit_chem_cells = mode == 3 ? 32 : c->jit_chem_nt;
+  c->jit_chem_smem = mode == 3 ? chemgen::roles_layout(M).smem() : mode == 2 ? (size_t)(M.ns - 1) * M.ns * JANC_JIT_NT_BIG * sizeof(double) : 0;
   std::string src = chemgen::generate_prim(M, c->g.ndim);
-  if (chem) src += chemgen::generate(M, c->g.ndim, mode == 2);
+  if (mode == 3) src += chemgen::generate_roles(M, c->g.ndim);
+  else if (chem) src += chemgen::generate(M, c->g.ndim, mode == 2);
   else c->jit_log = "chemistry: mechanism outside the specialised range; ";
   static std::map<std::string, JitKernels> cache;          // per process; one device per process
   const std::string key = std::to_string(c->device) + "\n" + src;
@@ -320,7 +327,7 @@ static void jit_setup(janc_ctx *c) {
 
 extern "C" const char *janc_chem_kernel(const janc_ctx *c) {
   if (!c || !c->have_mech) return "none";
-  if (c->jit_kernel) return c->jit_chem_smem ? "jit-smem" : "jit";
+  if (c->jit_kernel) return c->jit_chem_mode == 3 ? "jit-roles" : c->jit_chem_mode == 2 ? "jit-smem" : "jit";
   return (c->ns == 2 || c->ns == 9) ? "reg" : "generic";
 }
 extern "C" const char *janc_jit_log(const janc_ctx *c) { return c ? c->jit_log.c_str() : ""; }
@@ -333,7 +340,8 @@ extern "C" int janc_jit_probe(const janc_mech *m, int ndim, char *src_out, size_
   int rc = fill_mech(m, M, err);
   if (rc) return rc;
   std::string src = chemgen::generate_prim(M, ndim);
-  if (jit_chem_mode(M)) src += chemgen::generate(M, ndim, jit_chem_mode(M) == 2);
+  if (jit_chem_mode(M) == 3) src += chemgen::generate_roles(M, ndim);
+  else if (jit_chem_mode(M)) src += chemgen::generate(M, ndim, jit_chem_mode(M) == 2);
   if (src_len) *src_len = src.size();
   if (src_out && cap > 0) { size_t n = src.size() < cap - 1 ? src.size() : cap - 1; memcpy(src_out, src.data(), n); src_out[n] = 0; }
   if (cubin_bytes) {
@@ -645,7 +653,7 @@ static void do_chem(janc_ctx *c, double *U, Prof *pf) {
     const Params &P = c->P;
     ChemArgs a{U, P.T, P.scal, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc};
     void *args[] = {&a};
-    cudaLaunchKernel((const void *)c->jit_kernel, cell_grid(c, c->jit_chem_nt, c->np), dim3(c->jit_chem_nt, 1, 1), args,
+    cudaLaunchKernel((const void *)c->jit_kernel, cell_grid(c, c->jit_chem_cells, c->np), dim3(c->jit_chem_nt, 1, 1), args,
                      c->jit_chem_smem, c->stream);
     c->launches++;
     prof_mark(c, pf, 3);

@@ -79,3 +79,14 @@ def test_specialised_chemistry_source_compiles_for_sm100a(L, mech9):
         assert f"// reaction {mech.nr - 1}" in src and f"A{mech.ns - 2}_{mech.ns - 2}" in src
         assert "k_prim_jit" in src and "c_mech" not in src
         assert "__shared__" not in src[src.index("k_chem_jit"):]
+
+
+def test_role_warp_chemistry_source_compiles_for_sm100a(L, mech20):
+    """csrc/chemgen_roles.h (mechanisms with 13..23 unknowns): 8 role-specific literal sections, the system
+    columns as named registers, reaction tables in __constant__ memory; compiles for sm_100a without a GPU."""
+    from paper_2504_13750_b200 import binding
+    src, nbytes = binding.jit_probe(mech20, 3)
+    k = src[src.index("k_chem_jit"):]
+    assert nbytes and nbytes > 1000
+    assert all(f"case {w}:" in k for w in range(8)) and "A2_18" in k and "BAR();" in k and "bar.sync" in src
+    assert "__constant__ double c_kb[" in src and "c_mech" not in src

@@ -242,7 +242,7 @@ def test_cfg3_full_size_one_step(B, ref):
 # ------------------------------------------------------------------ chemistry kernel selection
 def test_specialised_chemistry_kernel_is_the_one_running(B, mech9, mech20):
     """janc_set_mechanism compiles the mechanism-specialised kernel (chemgen.h) for <= 12 unknowns;
-    larger mechanisms get the same specialised rates / Jacobian scatter with the matrix in shared memory."""
+    larger mechanisms (up to 24 species) run the role-warp kernel of chemgen_roles.h."""
     c = I.config1(nx=32, ny=16)
     s = B.Solver(c.grid, mech9)
     assert s.chem_kernel() == "jit", s.jit_log()
@@ -253,8 +253,49 @@ def test_specialised_chemistry_kernel_is_the_one_running(B, mech9, mech20):
     s.close()
     c4 = I.config4(n=16, nspheres=2, radius=3)
     s = B.Solver(c4.grid, mech20)
+    assert s.chem_kernel() == "jit-roles", s.jit_log()
+    s.close()
+
+
+def big_dt_case(mech, nx, ny, seed):
+    """hot gas, random composition, one fixed-dt step of pure chemistry with a dt large enough for real row swaps"""
+    ns = mech.ns
+    rng = np.random.default_rng(seed)
+    z = np.zeros((ny, nx))
+    Y = np.broadcast_to(I.hot_Y(ns), (ny, nx, ns)).copy()
+    Y[..., :ns - 1] *= rng.uniform(0.2, 1.8, size=(ny, nx, ns - 1)); Y[..., ns - 1] = 1.0 - Y[..., :ns - 1].sum(-1)
+    T = 1500.0 + 1500.0 * rng.random((ny, nx))
+    U = I.prim_to_cons(mech, 2, z + 2.0e6, T, Y, [z, z])
+    g = I.Grid(2, (nx, ny, 1), (1e-3, 1e-3, 1), (0, 0, 0), (0, 0, 0))
+    return I.Case("chem_big_dt", g, mech, U.reshape(1, -1, 1, ny, nx), T.reshape(1, 1, ny, nx), 0.2, 1)
+
+
+def test_role_warp_chemistry_kernel(B, ref, mech9, mech20, monkeypatch):
+    """chemgen_roles.h: (a) the 20-species mechanism with a large dt (pivoting swaps rows across the roles'
+    register columns), ragged cell count; (b) the 9-species mechanism pushed through the same generator
+    (2 column slots, a role with no column in slot 1) on configs 1 and 3; (c) the one-thread-per-cell
+    shared-memory variant it replaces still agrees."""
+    case = big_dt_case(mech20, 37, 11, 11)
+    Ug, Tg, Ur, Tr = both(B, ref, case, 1, cfl=0.0, dt=1e-7)
+    assert field_errors(case, Ug, Ur).max() <= 1e-8
+    monkeypatch.setenv("JANC_JIT_MAX_N1", "4")
+    c1 = I.config1(nx=96, ny=40)
+    s = B.Solver(c1.grid, c1.mech)
+    assert s.chem_kernel() == "jit-roles", s.jit_log()
+    s.close()
+    check(B, ref, c1, 1, TOL1)
+    check(B, ref, c1, 20, TOL100)
+    check(B, ref, I.config3(pcols=8, prows=4, npc=16), 2, TOL1 * 10)
+    case9 = big_dt_case(mech9, 40, 24, 7)
+    Ug, Tg, Ur, Tr = both(B, ref, case9, 1, cfl=0.0, dt=2e-7)
+    assert field_errors(case9, Ug, Ur).max() <= 1e-8
+    monkeypatch.delenv("JANC_JIT_MAX_N1")
+    monkeypatch.setenv("JANC_JIT_BIG", "smem")
+    c4 = I.config4(n=16, nspheres=2, radius=3)
+    s = B.Solver(c4.grid, c4.mech)
     assert s.chem_kernel() == "jit-smem", s.jit_log()
     s.close()
+    check(B, ref, c4, 1, TOL1)
 
 
 def test_table_driven_chemistry_fallback_parity(B, ref, monkeypatch):
