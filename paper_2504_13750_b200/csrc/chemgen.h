@@ -160,7 +160,7 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
   std::string &src = E.s;
   src += "// generated by chemgen.h for ns=" + I(ns) + " nr=" + I(nr) + " ndim=" + I(ndim) + "\n";
   src += "struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2;"
-         " long long st0, st1, st2, pc; };\n";
+         " long long st0, st1, st2, pc; int np; };\n";
   src += "extern \"C\" __global__ void __launch_bounds__(" + I(NT) + MINB_STR + ") k_chem_jit(ChemArgs a) {\n";
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
   if (big) {

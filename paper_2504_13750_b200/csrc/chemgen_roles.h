@@ -3,19 +3,27 @@
 //
 // Why another kernel: with one thread per cell (chemgen.h) the (Ns-1) x Ns system of a 20-species mechanism
 // (3 KB per cell) has to live in shared memory, which leaves room for ~2 warps per SM and the kernel crawls
-// on latency.  Here a CTA of 8 warps advances 32 cells: lane = cell, warp = ROLE.  Role w owns
+// on latency.  Here a persistent CTA of 8 warps (one per SM) advances 32 cells per turn: lane = cell,
+// warp = ROLE.  Role w owns
 //   * species  k = w, w+8, w+16      (Newton partial sums for T, the final rho Y_k update),
-//   * reactions dealt round-robin    (Arrhenius / equilibrium exponentials, rates of progress; shared
-//                                     table-driven code, tables in __constant__ memory indexed by the
-//                                     warp-uniform role: no divergence, no per-lane table traffic),
+//   * reactions dealt round-robin    (Arrhenius / equilibrium exponentials, rates of progress: shared
+//                                     table-driven code; the tables are copied once per CTA into shared
+//                                     memory and read with warp-uniform indices: broadcast loads, no divergence;
+//                                     four reactions per trip through a branch-free body so their exp chains overlap),
 //   * columns  j = w, w+8, w+16 of the system [I - dt J | rhs], held in REGISTERS (57 doubles for Ns = 20).
 // The Jacobian columns are assembled by role-specific literal code (switch on the warp index: every
 // species / reaction index a literal, every update one register FMA, structural zeros never touched),
 // reading the 2 Nr rate coefficients the roles exchanged through shared memory ([row][cell], conflict-free).
-// Gaussian elimination with partial pivoting is column-distributed: the owner of column c finds the pivot
-// and publishes the multipliers (double-buffered: one CTA barrier per column), every role swaps / updates
-// its own columns in registers.  The upper triangle then goes to shared memory and the role holding the
-// right-hand side back-substitutes.  All 8 roles of a cell see bit-identical T (same sums, same order).
+// The elimination is column-distributed Gauss-Jordan written as a compact loop over columns (warm in the
+// instruction cache; a first, fully unrolled version was bound by instruction fetch): the update writes row
+// p + 1 into row p, so the pivot row is always physical row 0 and register names stay static.  One-column
+// look-ahead: the owner of column c + 1 updates that column first and publishes its multipliers; roles
+// synchronise per column with producer / consumer named barriers (barrier.arrive / barrier.sync, ids 1..15),
+// never with a CTA-wide barrier, and no multiplier row is reused within a turn, so roles may run columns apart.
+// The register path never swaps rows: the owner checks that the diagonal entry IS the partial-pivoting choice
+// (first row of maximal |a_rc|, r >= c); if any of the 32 cells needs a swap the CTA spills the system to
+// shared memory and finishes with a generic, loop-based pivoted elimination (same pivot rule as the oracle).
+// All 8 roles of a cell see bit-identical T (same sums, same order).
 #pragma once
 #include <algorithm>
 
@@ -27,9 +35,33 @@
 namespace chemgen {
 
 struct RolesLayout {
-  int oX, oP, oN, oRN, oDL, oRHS, oF, oPIV, oXS, oR, rows;   // offsets in rows of 32 doubles
-  size_t smem() const { return (size_t)rows * 32 * sizeof(double); }
+  int oX, oP, oN, oRN, oDL, oRHS, oF, oPIV, oIP, oXS, oR, rows;   // offsets in rows of 32 doubles
+  size_t ntd, nti;                                                 // table sizes (doubles, ints) behind the rows
+  size_t smem() const { return (size_t)rows * 32 * sizeof(double) + ntd * sizeof(double) + nti * sizeof(int); }
 };
+
+// sizes that depend on the mechanism only: polynomial degrees, reaction orders, table lengths
+struct RolesDims { int degh, degc, nkb, maxof, maxob, nslot; };
+inline RolesDims roles_dims(const MechC &M) {
+  RolesDims D{1, 0, 3, 1, 1, (M.nr + JANC_ROLES - 1) / JANC_ROLES};
+  for (int k = 0; k < M.ns; k++)
+    for (int q = 1; q <= 4; q++)
+      if (M.nasa[k][q] != 0.0) { D.degh = std::max(D.degh, q + 1); D.degc = std::max(D.degc, q); }
+  D.nkb = 3 + D.degc;
+  for (int i = 0; i < M.nr; i++) {
+    D.maxof = std::max(D.maxof, (int)M.nreac[i]);
+    if (M.rev[i]) D.maxob = std::max(D.maxob, (int)M.nprod[i]);
+  }
+  return D;
+}
+inline size_t roles_table_doubles(const MechC &M) {
+  const RolesDims D = roles_dims(M);
+  return (size_t)2 * M.ns + (size_t)M.ns * (D.degh + 1) + (size_t)M.ns * (D.degc + 1) + (size_t)M.nr * 3 + (size_t)M.nr * D.nkb + (size_t)M.ntb * M.ns;
+}
+inline size_t roles_table_ints(const MechC &M) {
+  const RolesDims D = roles_dims(M);
+  return (size_t)JANC_ROLES * D.nslot + M.nr + (size_t)M.nr * D.maxof + (size_t)M.nr * D.maxob;
+}
 
 inline bool roles_applicable(const MechC &M) {
   return M.ns >= 3 && M.ns <= JANC_ROLES * JANC_ROLES_MAXSLOT && M.nr >= 1;
@@ -45,11 +77,16 @@ inline RolesLayout roles_layout(const MechC &M) {
   L.oRN = o; o += M.ntb > 0 ? M.ntb : 1;     // net rate without the third-body factor (third-body reactions)
   L.oDL = o; o += n1;                        // D_kN / W_N
   L.oRHS = o; o += n1;                       // dt W_k wdot_k
-  L.oF = o; o += 2 * n1;                     // elimination multipliers, double-buffered
-  L.oPIV = o; o += 2;                        // pivot row (int), double-buffered
+  L.oPIV = o; o += n1;                       // "this cell needs a row swap" (int, first half of each row), per column
+  L.oIP = o; o += n1;                        // reciprocal pivots
   L.oXS = o; o += n1;                        // solution
-  L.oR = o; o += std::max(3 * nr, n1 * (n1 + 1) / 2);   // M k_f, M k_b, q per reaction; later the upper triangle
+  // one region, three lives: M k_f, M k_b, q per reaction (until the assembly barrier); the multipliers of every
+  // column (elimination: nothing is reused, so the roles may run several columns apart); the whole system (slow path)
+  L.oR = o; o += std::max(3 * nr, n1 * (n1 + 1));
+  L.oF = L.oR;
   L.rows = o;
+  L.ntd = roles_table_doubles(M);
+  L.nti = roles_table_ints(M);
   return L;
 }
 
@@ -65,23 +102,20 @@ inline std::string generate_roles(const MechC &M, int ndim) {
 
   // ---- per-reaction stoichiometry
   std::vector<std::vector<int>> cf(nr, std::vector<int>(ns, 0)), cb(nr, std::vector<int>(ns, 0)), dnu(nr, std::vector<int>(ns, 0));
-  int maxof = 1, maxob = 1;
+  const RolesDims DM = roles_dims(M);
+  const int maxof = DM.maxof, maxob = DM.maxob;
   bool any_rev = false;
   for (int i = 0; i < nr; i++) {
     for (int e = 0; e < M.nreac[i]; e++) cf[i][M.reac[i][e]]++;
     for (int e = 0; e < M.nprod[i]; e++) cb[i][M.prod[i][e]]++;
     for (int k = 0; k < ns; k++) dnu[i][k] = cb[i][k] - cf[i][k];
-    maxof = std::max(maxof, (int)M.nreac[i]);
-    if (M.rev[i]) { maxob = std::max(maxob, (int)M.nprod[i]); any_rev = true; }
+    if (M.rev[i]) any_rev = true;
   }
   // ---- Newton polynomials (h_k/R_k - T, c_p,k/R_k - 1) truncated at the highest degree any species uses
-  int degh = 1, degc = 0;
-  for (int k = 0; k < ns; k++)
-    for (int q = 1; q <= 4; q++)
-      if (M.nasa[k][q] != 0.0) { degh = std::max(degh, q + 1); degc = std::max(degc, q); }
+  const int degh = DM.degh, degc = DM.degc;
   // ---- reverse rate: ln k_b = ln k_f - dn ln(p_atm / (R_u T)) - sum_k dnu_k g_k(T) collected per reaction as
   //      d0 + d1 ln T + d2 / T + T (d3 + T (d4 + T (d5 + T d6)))   (eq 4.8-4.9; g_k = s_k/R - h_k/(R T))
-  const int NKB = 3 + degc;
+  const int NKB = DM.nkb;
   std::vector<double> kbc((size_t)nr * 7, 0.0);
   for (int i = 0; i < nr; i++) {
     double *d = &kbc[(size_t)i * 7];
@@ -105,71 +139,94 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   std::vector<int> order;
   for (int i = 0; i < nr; i++) if (M.tb[i]) order.push_back(i);
   for (int i = 0; i < nr; i++) if (!M.tb[i]) order.push_back(i);
-  const int NSLOT = (nr + NR - 1) / NR;
+  const int NSLOT = DM.nslot;
   std::vector<int> ri((size_t)NR * NSLOT, -1);
   for (int q = 0; q < nr; q++) ri[(size_t)(q % NR) * NSLOT + q / NR] = order[q];
 
   // =========================================================================== tables
   src += "// generated by chemgen_roles.h for ns=" + I(ns) + " nr=" + I(nr) + " ndim=" + I(ndim) + "\n";
   src += "struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2;"
-         " long long st0, st1, st2, pc; };\n";
-  auto table = [&](const std::string &decl, const std::vector<std::string> &v) {
-    src += "__constant__ " + decl + " = {";
-    for (size_t q = 0; q < v.size(); q++) src += (q ? ", " : "") + v[q];
-    src += "};\n";
-  };
-  std::vector<std::string> t;
-  t.clear(); for (int k = 0; k < ns; k++) t.push_back(num(M.invW[k]));
-  table("double c_iW[" + I(ns) + "]", t);
-  t.clear(); for (int k = 0; k < ns; k++) t.push_back(num(M.Rk[k]));
-  table("double c_Rk[" + I(ns) + "]", t);
-  t.clear();
+         " long long st0, st1, st2, pc; int np; };\n";
+  // Tables: emitted as two __constant__ arrays, copied once per (persistent) CTA into shared memory, where the
+  // warp-uniform, run-time indexed reads of the rate loop are plain broadcast loads.
+  std::vector<std::string> td, ti;
+  auto addd = [&](const std::string &name, int &off) { off = (int)td.size(); (void)name; };
+  int oiW, oRk, ohc, occ, okf, okb, oeff, ori, ofl, ore, opr;
+  addd("iW", oiW); for (int k = 0; k < ns; k++) td.push_back(num(M.invW[k]));
+  addd("Rk", oRk); for (int k = 0; k < ns; k++) td.push_back(num(M.Rk[k]));
+  addd("hc", ohc);
   for (int k = 0; k < ns; k++) {
     const double *c = M.nasa[k];
     const double hc[6] = {c[5], c[0] - 1.0, 0.5 * c[1], c[2] / 3.0, 0.25 * c[3], 0.2 * c[4]};
-    for (int q = 0; q <= degh; q++) t.push_back(num(hc[q]));
+    for (int q = 0; q <= degh; q++) td.push_back(num(hc[q]));
   }
-  table("double c_hc[" + I(ns * (degh + 1)) + "]", t);
-  t.clear();
+  addd("cc", occ);
   for (int k = 0; k < ns; k++) {
     const double *c = M.nasa[k];
     const double cc[5] = {c[0] - 1.0, c[1], c[2], c[3], c[4]};
-    for (int q = 0; q <= degc; q++) t.push_back(num(cc[q]));
+    for (int q = 0; q <= degc; q++) td.push_back(num(cc[q]));
   }
-  table("double c_cc[" + I(ns * (degc + 1)) + "]", t);
-  t.clear(); for (int i = 0; i < nr; i++) { t.push_back(num(M.lnA[i])); t.push_back(num(M.b[i])); t.push_back(num(-M.Ta[i])); }
-  table("double c_kf[" + I(nr * 3) + "]", t);
-  t.clear(); for (int i = 0; i < nr; i++) for (int q = 0; q < NKB; q++) t.push_back(num(kbc[(size_t)i * 7 + q]));
-  table("double c_kb[" + I(nr * NKB) + "]", t);
-  t.clear();
-  for (int q = 0; q < (M.ntb > 0 ? M.ntb : 1); q++) for (int k = 0; k < ns; k++) t.push_back(num(M.ntb > 0 ? M.eff[q][k] : 0.0));
-  table("double c_eff[" + I((M.ntb > 0 ? M.ntb : 1) * ns) + "]", t);
-  t.clear(); for (int v : ri) t.push_back(I(v));
-  table("int c_ri[" + I(NR * NSLOT) + "]", t);
-  t.clear(); for (int i = 0; i < nr; i++) t.push_back(I((M.rev[i] ? 1 : 0) | ((M.tb[i] ? M.tbi[i] + 1 : 0) << 1)));
-  table("int c_fl[" + I(nr) + "]", t);
-  t.clear(); for (int i = 0; i < nr; i++) for (int q = 0; q < maxof; q++) t.push_back(I(q < M.nreac[i] ? M.reac[i][q] : ns));
-  table("unsigned char c_re[" + I(nr * maxof) + "]", t);
-  t.clear(); for (int i = 0; i < nr; i++) for (int q = 0; q < maxob; q++) t.push_back(I(q < M.nprod[i] ? M.prod[i][q] : ns));
-  table("unsigned char c_pr[" + I(nr * maxob) + "]", t);
-
+  addd("kf", okf); for (int i = 0; i < nr; i++) { td.push_back(num(M.lnA[i])); td.push_back(num(M.b[i])); td.push_back(num(-M.Ta[i])); }
+  addd("kb", okb); for (int i = 0; i < nr; i++) for (int q = 0; q < NKB; q++) td.push_back(num(kbc[(size_t)i * 7 + q]));
+  addd("eff", oeff); for (int q = 0; q < M.ntb; q++) for (int k = 0; k < ns; k++) td.push_back(num(M.eff[q][k]));
+  ori = (int)ti.size(); for (int v : ri) ti.push_back(I(v));
+  ofl = (int)ti.size(); for (int i = 0; i < nr; i++) ti.push_back(I((M.rev[i] ? 1 : 0) | ((M.tb[i] ? M.tbi[i] + 1 : 0) << 1)));
+  ore = (int)ti.size(); for (int i = 0; i < nr; i++) for (int q = 0; q < maxof; q++) ti.push_back(I(q < M.nreac[i] ? M.reac[i][q] : ns));
+  opr = (int)ti.size(); for (int i = 0; i < nr; i++) for (int q = 0; q < maxob; q++) ti.push_back(I(q < M.nprod[i] ? M.prod[i][q] : ns));
+  const int NTD = (int)td.size(), NTI = (int)ti.size();
+  if ((size_t)NTD != roles_table_doubles(M) || (size_t)NTI != roles_table_ints(M)) return std::string("#error roles table size\n");
+  src += "__constant__ double g_td[" + I(NTD) + "] = {";
+  for (int q = 0; q < NTD; q++) src += (q ? ", " : "") + td[q];
+  src += "};\n__constant__ int g_ti[" + I(NTI) + "] = {";
+  for (int q = 0; q < NTI; q++) src += (q ? ", " : "") + ti[q];
+  src += "};\n";
+  // branch-free exp (Cody-Waite reduction, degree-13 Taylor polynomial on |r| <= ln2/2: < 2 ulp), argument clamped
+  // to the finite range; lets the scheduler interleave the exponentials of two reactions
+  src += "__device__ __forceinline__ double exp_nb(double x) {\n"
+         "  x = fmin(fmax(x, -708.0), 709.0);\n"
+         "  const double t = fma(x, 1.4426950408889634, 6755399441055744.0);\n"
+         "  const int n = __double2loint(t);\n"
+         "  const double nf = t - 6755399441055744.0;\n"
+         "  double r = fma(nf, -6.93147180369123816490e-01, x);\n"
+         "  r = fma(nf, -1.90821492927058770002e-10, r);\n"
+         "  double p = 1.6059043836821613e-10;\n"
+         "  p = fma(p, r, 2.08767569878681e-09); p = fma(p, r, 2.505210838544172e-08); p = fma(p, r, 2.755731922398589e-07);\n"
+         "  p = fma(p, r, 2.7557319223985893e-06); p = fma(p, r, 2.48015873015873e-05); p = fma(p, r, 1.984126984126984e-04);\n"
+         "  p = fma(p, r, 1.388888888888889e-03); p = fma(p, r, 8.333333333333333e-03); p = fma(p, r, 4.1666666666666664e-02);\n"
+         "  p = fma(p, r, 1.6666666666666666e-01); p = fma(p, r, 0.5); p = fma(p, r, 1.0); p = fma(p, r, 1.0);\n"
+         "  const int n1 = n >> 1, n2 = n - n1;\n"
+         "  return p * __hiloint2double((n1 + 1023) << 20, 0) * __hiloint2double((n2 + 1023) << 20, 0);\n"
+         "}\n";
   // =========================================================================== kernel
   src += "#define SM(r) sm_[(r) * 32 + lane]\n";
   src += "#define BAR() asm volatile(\"bar.sync 0;\" ::: \"memory\")\n";
+  src += "#define AWAIT(id) asm volatile(\"barrier.sync %0, " + I(NR * 32) + ";\" :: \"r\"(id) : \"memory\")\n";
+  src += "#define PUBLISH(id) do { asm volatile(\"barrier.arrive %0, " + I(NR * 32) + ";\" :: \"r\"(id) : \"memory\"); } while (0)\n";
   src += "extern \"C\" __global__ void __launch_bounds__(" + I(NR * 32) + ", 1) k_chem_jit(ChemArgs a) {\n";
   E.line("extern __shared__ double sm_[];");
   E.line("const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;");
-  E.line("int *s_piv = (int *)(sm_ + " + I(L.oPIV * 32) + ");");
-  E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
-  E.line("long long t = (long long)blockIdx.x * 32 + lane;");
+  E.line("double *s_td = sm_ + " + I(L.rows * 32) + ";");
+  E.line("int *s_ti = (int *)(s_td + " + I(NTD) + ");");
+  E.line("for (int q = threadIdx.x; q < " + I(NTD) + "; q += " + I(NR * 32) + ") s_td[q] = g_td[q];");
+  E.line("for (int q = threadIdx.x; q < " + I(NTI) + "; q += " + I(NR * 32) + ") s_ti[q] = g_ti[q];");
+  E.line("const double *c_iW = s_td + " + I(oiW) + ", *c_Rk = s_td + " + I(oRk) + ", *c_hc = s_td + " + I(ohc) + ", *c_cc = s_td + " + I(occ) +
+         ", *c_kf = s_td + " + I(okf) + ", *c_kb = s_td + " + I(okb) + ", *c_eff = s_td + " + I(oeff) + ";");
+  E.line("const int *c_ri = s_ti + " + I(ori) + ", *c_fl = s_ti + " + I(ofl) + ", *c_re = s_ti + " + I(ore) + ", *c_pr = s_ti + " + I(opr) + ";");
+  E.line("int *s_flag = (int *)(sm_ + " + I(L.oPIV * 32) + ");");
+  E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2, nbp = (ncell + 31) / 32, nbt = nbp * a.np;");
+  E.line("const double dt = a.scal[0];");
+  E.line("BAR();");
+  E.line("#pragma unroll 1");
+  E.line("for (long long bt = blockIdx.x; bt < nbt; bt += gridDim.x) {   // persistent CTA: 32 cells per turn");
+  E.line("const int patch = (int)(bt / nbp);");
+  E.line("long long t = (bt - (long long)patch * nbp) * 32 + lane;");
   E.line("const bool live = t < ncell;");
   E.line("if (!live) t = ncell - 1;   // idle lanes recompute the last cell and store nothing");
   E.line("const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;");
   E.line("const int cj = (int)(r_ % a.n1), ck = (int)(r_ / a.n1);");
   E.line("const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;");
-  E.line("double *Up = a.U + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
-  E.line("const long long pid = (long long)blockIdx.y * a.pc + id;");
-  E.line("const double dt = a.scal[0];");
+  E.line("double *Up = a.U + (long long)patch * " + I(nvar) + " * a.pc + id;");
+  E.line("const long long pid = (long long)patch * a.pc + id;");
   // ---- cons -> prim pieces (eq 4.2); species k = w + 8 s belong to this role
   E.line("const double rho = Up[0], irho = 1.0 / rho;");
   E.line("double ke = 0.0;");
@@ -219,41 +276,61 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("}");
   E.line("bool ok = conv && (T > 0.0) && isfinite(T);");
   E.line("if (live && w == 0) a.T[pid] = T;");
-  // ---- rates of progress (eq 4.7-4.9): shared code, tables indexed by the warp-uniform role
-  E.line("{ const double lnT = log(T), iT = 1.0 / T;");
-  E.line("  #pragma unroll 1");
-  E.line("  for (int r = 0; r < " + I(NSLOT) + "; r++) {");
-  E.line("    const int i = c_ri[w * " + I(NSLOT) + " + r];");
-  E.line("    if (i < 0) break;");
-  E.line("    const double *f_ = c_kf + 3 * i;");
-  E.line("    const double lkf = fma(f_[2], iT, fma(f_[1], lnT, f_[0]));");
-  E.line("    const double kf = exp(lkf);");
-  E.line("    const int fl = c_fl[i];");
-  E.line("    double kb = 0.0;");
-  if (any_rev) {
-    E.line("    if (fl & 1) { const double *d_ = c_kb + " + I(NKB) + " * i;");
-    std::string lk = "fma(d_[2], iT, fma(d_[1], lnT, d_[0]))";
-    if (degc > 0) {
-      std::string pol = "d_[" + I(NKB - 1) + "]";
-      for (int q = NKB - 2; q >= 3; q--) pol = "fma(T, " + pol + ", d_[" + I(q) + "])";
-      lk = "fma(T, " + pol + ", " + lk + ")";
+  // ---- rates of progress (eq 4.7-4.9): shared code, tables indexed by the warp-uniform role.  Third-body
+  //      reactions come first in every role's list; the others are taken two at a time (branch-free body,
+  //      so the two exponential chains interleave).
+  auto rate_body = [&](const std::string &S, const std::string &idx, bool tb) {
+    E.line("    const int i" + S + " = " + idx + ";");
+    E.line("    const double *f" + S + " = c_kf + 3 * i" + S + ";");
+    E.line("    const double kf" + S + " = exp_nb(fma(f" + S + "[2], iT, fma(f" + S + "[1], lnT, f" + S + "[0])));");
+    if (any_rev) {
+      E.line("    const double *d" + S + " = c_kb + " + I(NKB) + " * i" + S + ";");
+      std::string lk = "fma(d" + S + "[2], iT, fma(d" + S + "[1], lnT, d" + S + "[0]))";
+      if (degc > 0) {
+        std::string pol = "d" + S + "[" + I(NKB - 1) + "]";
+        for (int q = NKB - 2; q >= 3; q--) pol = "fma(T, " + pol + ", d" + S + "[" + I(q) + "])";
+        lk = "fma(T, " + pol + ", " + lk + ")";
+      }
+      E.line("    const double kb" + S + " = (c_fl[i" + S + "] & 1) ? exp_nb(" + lk + ") : 0.0;");
+    } else {
+      E.line("    const double kb" + S + " = 0.0;");
     }
-    E.line("      kb = exp(" + lk + "); }");
-  }
-  E.line("    double pf = kf, pb = kb;");
-  for (int q = 0; q < maxof; q++) E.line("    pf *= SM(" + I(L.oX) + " + c_re[i * " + I(maxof) + " + " + I(q) + "]);");
-  if (any_rev) for (int q = 0; q < maxob; q++) E.line("    pb *= SM(" + I(L.oX) + " + c_pr[i * " + I(maxob) + " + " + I(q) + "]);");
-  E.line("    const double rn = pf - pb;");
-  E.line("    double Mi = 1.0;");
+    E.line("    double pf" + S + " = kf" + S + ", pb" + S + " = kb" + S + ";");
+    for (int q = 0; q < maxof; q++) E.line("    pf" + S + " *= SM(" + I(L.oX) + " + c_re[i" + S + " * " + I(maxof) + " + " + I(q) + "]);");
+    if (any_rev) for (int q = 0; q < maxob; q++) E.line("    pb" + S + " *= SM(" + I(L.oX) + " + c_pr[i" + S + " * " + I(maxob) + " + " + I(q) + "]);");
+    E.line("    const double rn" + S + " = pf" + S + " - pb" + S + ";");
+    if (tb) {
+      E.line("    const int tb_ = (c_fl[i" + S + "] >> 1) - 1;");
+      E.line("    const double *ef = c_eff + tb_ * " + I(ns) + ";");
+      E.line("    double Mi = ef[0] * SM(" + I(L.oX) + ");");
+      E.line("    #pragma unroll");
+      E.line("    for (int j = 1; j < " + I(ns) + "; j++) Mi = fma(ef[j], SM(" + I(L.oX) + " + j), Mi);");
+      E.line("    SM(" + I(L.oRN) + " + tb_) = rn" + S + ";");
+      E.line("    SM(" + I(L.oR) + " + i" + S + ") = Mi * kf" + S + "; SM(" + I(L.oR + nr) + " + i" + S + ") = Mi * kb" + S + "; SM(" + I(L.oR + 2 * nr) + " + i" + S + ") = Mi * rn" + S + ";");
+    } else {
+      E.line("    SM(" + I(L.oR) + " + i" + S + ") = kf" + S + "; SM(" + I(L.oR + nr) + " + i" + S + ") = kb" + S + "; SM(" + I(L.oR + 2 * nr) + " + i" + S + ") = rn" + S + ";");
+    }
+  };
+  const std::string RI = "c_ri[w * " + I(NSLOT) + " + r]", RI1 = "c_ri[w * " + I(NSLOT) + " + r + 1]";
+  E.line("{ const double lnT = log(T), iT = 1.0 / T;");
+  E.line("  int r = 0;");
   if (M.ntb > 0) {
-    E.line("    const int tb_ = (fl >> 1) - 1;");
-    E.line("    if (tb_ >= 0) { const double *ef = c_eff + tb_ * " + I(ns) + ";");
-    E.line("      Mi = ef[0] * SM(" + I(L.oX) + ");");
-    E.line("      #pragma unroll");
-    E.line("      for (int j = 1; j < " + I(ns) + "; j++) Mi = fma(ef[j], SM(" + I(L.oX) + " + j), Mi);");
-    E.line("      SM(" + I(L.oRN) + " + tb_) = rn; }");
+    E.line("  #pragma unroll 1");
+    E.line("  for (; r < " + I(NSLOT) + "; r++) {");
+    E.line("    if (" + RI + " < 0 || (c_fl[" + RI + "] >> 1) == 0) break;");
+    rate_body("", RI, true);
+    E.line("  }");
   }
-  E.line("    SM(" + I(L.oR) + " + i) = Mi * kf; SM(" + I(L.oR + nr) + " + i) = Mi * kb; SM(" + I(L.oR + 2 * nr) + " + i) = Mi * rn;");
+  const std::string RIq[4] = {RI, RI1, "c_ri[w * " + I(NSLOT) + " + r + 2]", "c_ri[w * " + I(NSLOT) + " + r + 3]"};
+  E.line("  #pragma unroll 1");
+  E.line("  for (; r + 3 < " + I(NSLOT) + "; r += 4) {");
+  E.line("    if (" + RIq[3] + " < 0) break;");
+  for (int q = 0; q < 4; q++) rate_body(std::string(1, (char)('a' + q)), RIq[q], false);
+  E.line("  }");
+  E.line("  #pragma unroll 1");
+  E.line("  for (; r < " + I(NSLOT) + "; r++) {");
+  E.line("    if (" + RI + " < 0) break;");
+  rate_body("", RI, false);
   E.line("  }");
   E.line("}");
   E.line("BAR();");
@@ -347,81 +424,111 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     }
   }
   E.line("}");
-  // ---- Gaussian elimination with partial pivoting, column-distributed (the oracle's pivot choice: first row of
-  //      maximal |a_rc|); L is not kept: the right-hand side is a column of the system
-  auto swap_chain = [&](int s, int c, const std::string &ind) {
-    for (int r = c + 1; r < n1; r++)
-      E.line(ind + "{ const bool sw = piv == " + I(r) + "; const double x_ = " + A(s, c) + ", y_ = " + A(s, r) + "; " +
-             A(s, c) + " = sw ? y_ : x_; " + A(s, r) + " = sw ? x_ : y_; }");
+  // ---- Gauss-Jordan elimination, column-distributed, one-column look-ahead (see the header); L is not kept: the
+  //      right-hand side is column n1 of the system.  The column loop is a real loop (compact code, warm in the
+  //      instruction cache): the update writes row p + 1 into row p, so the pivot row is always physical row 0
+  //      (after n1 columns every surviving column is back in its original order) and only the slot is selected
+  //      at run time, by warp-uniform branches.
+  auto rot = [&](int s, const std::string &ind) {
+    std::string l = ind + "{ const double P_ = " + A(s, 0) + ";";
+    E.line(l);
+    for (int p = 0; p + 1 < n1; p++) E.line(ind + "  " + A(s, p) + " = fma(-f" + I(p + 1) + ", P_, " + A(s, p + 1) + ");");
+    E.line(ind + "  " + A(s, n1 - 1) + " = P_; }");
   };
-  for (int c = 0; c < n1; c++) {
-    const int oc = c % NR, sc = c / NR, pb = c & 1;
-    const bool last = c + 1 == n1;
-    E.line("{ // column " + I(c));
-    E.line("  if (w == " + I(oc) + ") {");
-    if (!last) {
-      E.line("    int piv = " + I(c) + "; double best = fabs(" + A(sc, c) + "), v;");
-      for (int r = c + 1; r < n1; r++)
-        E.line("    v = fabs(" + A(sc, r) + "); if (v > best) { best = v; piv = " + I(r) + "; }");
-      E.line("    if (!(best > 0.0)) ok = false;");
-      E.line("    if (__any_sync(0xffffffffu, piv != " + I(c) + ")) {");
-      swap_chain(sc, c, "      ");
-      E.line("    }");
-      E.line("    s_piv[" + I(pb * 32) + " + lane] = piv;");
-    } else {
-      E.line("    if (!(fabs(" + A(sc, c) + ") > 0.0)) ok = false;");
-    }
-    E.line("    const double ip = 1.0 / " + A(sc, c) + ";");
-    for (int r = c + 1; r < n1; r++) E.line("    " + row(L.oF + pb * n1 + r) + " = " + A(sc, r) + " * ip;");
-    E.line("    " + A(sc, c) + " = ip;");
-    E.line("  }");
-    if (!last) {
-      E.line("  BAR();");
-      E.line("  const int piv = s_piv[" + I(pb * 32) + " + lane];");
-      E.line("  if (__any_sync(0xffffffffu, piv != " + I(c) + ")) {");
-      E.line("    if (w != " + I(oc) + ") {");
-      swap_chain(sc, c, "      ");
-      E.line("    }");
-      for (int s = sc + 1; s < NSL; s++) swap_chain(s, c, "    ");
-      E.line("  }");
-      for (int r = c + 1; r < n1; r++) E.line("  const double f" + I(r) + " = " + row(L.oF + pb * n1 + r) + ";");
-      E.line("  if (w > " + I(oc) + ") {");
-      for (int r = c + 1; r < n1; r++) E.line("    " + A(sc, r) + " = fma(-f" + I(r) + ", " + A(sc, c) + ", " + A(sc, r) + ");");
-      E.line("  }");
-      for (int s = sc + 1; s < NSL; s++)
-        for (int r = c + 1; r < n1; r++) E.line("  " + A(s, r) + " = fma(-f" + I(r) + ", " + A(s, c) + ", " + A(s, r) + ");");
-    }
-    E.line("}");
-  }
-  // ---- upper triangle (reciprocal pivots on the diagonal) -> shared memory; the role holding the rhs solves
-  // (the rate arrays are dead since the barrier after the assembly: the triangle takes their place)
-  auto tri = [&](int k) { return L.oR + k * n1 - k * (k - 1) / 2 - k; };   // + j
+  // owner of column cn (variables cn, pbn in scope), already rotated into cn's frame: physical rows 1..n1-1-cn are the
+  // rows below the diagonal.  Publishes "needs a swap" and, if no cell does, the multipliers of all other rows.
+  auto owner = [&](int s, const std::string &ind) {
+    E.line(ind + "{ const double ac = fabs(" + A(s, 0) + "), ip = 1.0 / " + A(s, 0) + ";");
+    E.line(ind + "  const int nb_ = " + I(n1) + " - cn;");
+    E.line(ind + "  int bad = !(ac > 0.0);                       // branch-free: 18 independent compares");
+    for (int p = 1; p < n1; p++) E.line(ind + "  bad |= (int)(" + I(p) + " < nb_) & (int)(fabs(" + A(s, p) + ") > ac);");
+    E.line(ind + "  s_flag[cn * 64 + lane] = bad;");
+    E.line(ind + "  if (!__any_sync(0xffffffffu, bad != 0)) {");
+    for (int p = 1; p < n1; p++) E.line(ind + "    SM(" + I(L.oF) + " + cn * " + I(n1) + " + " + I(p) + ") = " + A(s, p) + " * ip;");
+    E.line(ind + "    SM(" + I(L.oIP) + " + cn) = ip;");
+    E.line(ind + "  }");
+    E.line(ind + "}");
+  };
+  E.line("int c0 = " + I(n1) + ";     // first column of the pivoted slow path (" + I(n1) + ": none)");
+  E.line("if (w == 0) { const int cn = 0;");
+  owner(0, "  ");
+  E.line("  PUBLISH(1);");
+  E.line("}");
+  E.line("#pragma unroll 1");
+  E.line("for (int c = 0; c < " + I(n1) + "; c++) {");
+  E.line("  const int sc = c >> 3, oc = c & 7;");
+  E.line("  if (w != oc) AWAIT(1 + c % 15);     // column c published by its owner (producer / consumer barrier)");
+  E.line("  const int fl_ = s_flag[c * 64 + lane];");
+  for (int p = 1; p < n1; p++) E.line("  const double f" + I(p) + " = SM(" + I(L.oF) + " + c * " + I(n1) + " + " + I(p) + ");");
+  E.line("  if (__any_sync(0xffffffffu, fl_ != 0)) { c0 = c; break; }");
+  E.line("  const int cn = c + 1, ocn = cn & 7, scn = cn >> 3;");
+  E.line("  const bool la = cn < " + I(n1) + " && w == ocn;     // this role owns the next column: update it first, publish");
+  E.line("  if (la) {");
   for (int s = 0; s < NSL; s++) {
-    const std::string js = "k" + I(s);
-    E.line("if (" + js + " < " + I(n1) + ") {");
-    for (int k = 0; k < n1; k++) {
-      if (k > NR * s + NR - 1) break;
-      E.line("  if (" + I(k) + " <= " + js + ") SM(" + I(tri(k)) + " + " + js + ") = " + A(s, k) + ";");
-    }
-    E.line("}");
+    if (NR * s >= n1) break;
+    E.line("    " + std::string(s ? "else " : "") + "if (scn == " + I(s) + ") {");
+    rot(s, "      ");
+    owner(s, "      ");
+    E.line("    }");
+    if (NR * (s + 1) >= n1 || s + 1 == NSL) E.line("    PUBLISH(1 + cn % 15);");
   }
+  E.line("  }");
+  for (int s = 0; s < NSL; s++) {
+    std::string cond = "(sc < " + I(s) + " || (sc == " + I(s) + " && w > oc)) && !(la && scn == " + I(s) + ")";
+    if (s == sN) cond += " && w <= " + I(wN);
+    E.line("  if (" + cond + ") {");
+    rot(s, "    ");
+    E.line("  }");
+  }
+  E.line("}");
+  // ---- fast path: the system is diagonal; the role holding the right-hand side scales it
   E.line("BAR();");
-  E.line("if (w == " + I(wN) + ") {");
-  for (int r = n1 - 1; r >= 0; r--) {
-    E.line("  " + A(sN, r) + " *= " + row(tri(r) + r) + ";");
-    for (int k = 0; k < r; k++) E.line("  " + A(sN, k) + " = fma(-" + row(tri(k) + r) + ", " + A(sN, r) + ", " + A(sN, k) + ");");
-  }
+  E.line("if (c0 == " + I(n1) + ") {");
+  E.line("  if (w == " + I(wN) + ") {");
   for (int k = 0; k < n1; k++) {
-    E.line("  if (!isfinite(" + A(sN, k) + ")) ok = false;");
-    E.line("  " + row(L.oXS + k) + " = " + A(sN, k) + ";");
+    E.line("    { const double x_ = " + A(sN, k) + " * " + row(L.oIP + k) + "; if (!isfinite(x_)) ok = false; " + row(L.oXS + k) + " = x_; }");
   }
+  E.line("  }");
+  E.line("} else {");
+  // ---- slow path: spill the system, finish columns c0.. with partial pivoting in shared memory (generic loops)
+  const int NC = n1 + 1;
+  E.line("  #define SMA(r, c) sm_[((" + I(L.oR) + ") + (r) * " + I(NC) + " + (c)) * 32 + lane]");
+  for (int s = 0; s < NSL; s++) {
+    E.line("  if (k" + I(s) + " >= c0 && k" + I(s) + " <= " + I(n1) + ") {   // registers are rotated by c0 rows");
+    for (int p = 0; p < n1; p++)
+      E.line("    { int lr = " + I(p) + " + c0; if (lr >= " + I(n1) + ") lr -= " + I(n1) + "; SMA(lr, k" + I(s) + ") = " + A(s, p) + "; }");
+    E.line("  }");
+  }
+  E.line("  BAR();");
+  E.line("  #pragma unroll 1");
+  E.line("  for (int c = c0; c < " + I(n1) + "; c++) {");
+  E.line("    int piv = c; double best = fabs(SMA(c, c));");
+  E.line("    for (int r = c + 1; r < " + I(n1) + "; r++) { const double v = fabs(SMA(r, c)); if (v > best) { best = v; piv = r; } }");
+  E.line("    if (!(best > 0.0)) ok = false;");
+  for (int s = 0; s < NSL; s++)
+    E.line("    if (k" + I(s) + " >= c && k" + I(s) + " <= " + I(n1) + " && piv != c) { const double x_ = SMA(c, k" + I(s) + "); SMA(c, k" + I(s) + ") = SMA(piv, k" + I(s) + "); SMA(piv, k" + I(s) + ") = x_; }");
+  E.line("    BAR();");
+  E.line("    const double ip = 1.0 / SMA(c, c);");
+  for (int s = 0; s < NSL; s++) {
+    E.line("    if (k" + I(s) + " > c && k" + I(s) + " <= " + I(n1) + ") { const double pj = SMA(c, k" + I(s) + ");");
+    E.line("      for (int r = 0; r < " + I(n1) + "; r++) if (r != c) SMA(r, k" + I(s) + ") = fma(-(SMA(r, c) * ip), pj, SMA(r, k" + I(s) + ")); }");
+  }
+  E.line("    if (w == 0) SM(" + I(L.oIP) + " + c) = ip;");
+  E.line("    BAR();");
+  E.line("  }");
+  E.line("  if (w == " + I(wN) + ") {");
+  E.line("    for (int k = 0; k < " + I(n1) + "; k++) { const double x_ = SMA(k, " + I(n1) + ") * SM(" + I(L.oIP) + " + k); if (!isfinite(x_)) ok = false; SM(" + I(L.oXS) + " + k) = x_; }");
+  E.line("  }");
+  E.line("  #undef SMA");
   E.line("}");
   E.line("BAR();");
   for (int s = 0; s < NSL; s++)
     E.line("if (live && k" + I(s) + " < " + I(n1) + ") Up[(long long)(" + I(ndim + 2) + " + k" + I(s) + ") * a.pc] = ry" + I(s) +
            " + SM(" + I(L.oXS) + " + k" + I(s) + ");");
   E.line("if (!ok && live) *a.flag = 1;");
-  src += "}\n#undef SM\n#undef BAR\n";
+  E.line("BAR();   // shared rows are reused by the next turn");
+  E.line("}");
+  src += "}\n#undef SM\n#undef BAR\n#undef AWAIT\n#undef PUBLISH\n";
   return src;
 }
 

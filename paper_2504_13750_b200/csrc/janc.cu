@@ -36,6 +36,7 @@ struct janc_ctx {
   std::vector<int> level, nbr, parent, fkind;
   int parity;
   long long launches;
+  int num_sms;
   int jit_chem_nt, jit_chem_cells, jit_chem_mode;   // threads per CTA, cells per CTA, see jit_chem_mode()
   size_t jit_chem_smem;
   cudaKernel_t jit_prim;     // mechanism-specialised cons->prim kernel, null if not in use
@@ -104,6 +105,8 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
   if (!c) return JANC_ENOMEM;
   c->g = *grid;
   c->device = device;
+  c->num_sms = 148;
+  cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
   c->stream = (cudaStream_t)cuda_stream;
   c->np = grid->n_patches > 0 ? grid->n_patches : 1;
   if (c->np > 65535) { delete c; return JANC_EINVAL; }   // patches ride on gridDim.y
@@ -214,7 +217,7 @@ static int fill_mech(const janc_mech *m, MechC &M, std::string &err) {
 // ------------------------------------------------------------------ run-time specialised chemistry
 // NVRTC is reached through dlopen so that libjanc.so loads (and the generic kernels run) where it is
 // absent; the cubin is loaded with the runtime's cudaLibrary API (no link against libcuda).
-struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; };
+struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np; };
 
 struct NvrtcApi {
   void *h = nullptr;
@@ -651,10 +654,14 @@ static void launch_chem_reg(janc_ctx *c, double *U) {
 static void do_chem(janc_ctx *c, double *U, Prof *pf) {
   if (c->jit_kernel) {
     const Params &P = c->P;
-    ChemArgs a{U, P.T, P.scal, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc};
+    ChemArgs a{U, P.T, P.scal, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc, c->np};
     void *args[] = {&a};
-    cudaLaunchKernel((const void *)c->jit_kernel, cell_grid(c, c->jit_chem_cells, c->np), dim3(c->jit_chem_nt, 1, 1), args,
-                     c->jit_chem_smem, c->stream);
+    dim3 grid = cell_grid(c, c->jit_chem_cells, c->np);
+    if (c->jit_chem_mode == 3) {      // persistent CTAs, one per SM, each takes 32-cell turns
+      const long long turns = (long long)grid.x * grid.y;
+      grid = dim3((unsigned)(turns < c->num_sms ? turns : c->num_sms), 1, 1);
+    }
+    cudaLaunchKernel((const void *)c->jit_kernel, grid, dim3(c->jit_chem_nt, 1, 1), args, c->jit_chem_smem, c->stream);
     c->launches++;
     prof_mark(c, pf, 3);
     return;
