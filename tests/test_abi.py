@@ -89,4 +89,4 @@ def test_role_warp_chemistry_source_compiles_for_sm100a(L, mech20):
     k = src[src.index("k_chem_jit"):]
     assert nbytes and nbytes > 1000
     assert all(f"case {w}:" in k for w in range(8)) and "A2_18" in k and "BAR();" in k and "bar.sync" in src
-    assert "__constant__ double c_kb[" in src and "c_mech" not in src
+    assert "__constant__ double g_td[" in src and "barrier.arrive" in src and "c_mech" not in src
