@@ -11,7 +11,8 @@
 // face costs ~2 x 38 fp64 instructions and each split flux is evaluated once per pencil.
 //   x: the tile rows (+3 ghosts each side) of 2f+- = F +- alpha U are staged once in shared memory
 //      with coalesced loads; pencils then read them row-wise (odd pitch, conflict-free).
-//   y, z: lanes run along x, so the strided pencil loads are already coalesced; no staging.
+//   y, z: the tile extended by 3 cells along the sweep direction is staged the same way ([z][y][x], odd x pitch);
+//      lanes run along x, so pencil reads are conflict-free.
 // Pencil results (-dF/dx_d) are summed per cell in shared memory; a coalesced pass applies the RK
 // stage.  No flux array ever goes to HBM: per stage the kernel reads U^(k) (+ U^n) and writes U^(k+1).
 //
@@ -96,9 +97,13 @@ struct FluxCfg {
   static constexpr int NT = TX * TY * TZ / SEG;          // threads per CTA = pencils per direction
   static constexpr int ROWS = TY * TZ;
   static constexpr int XP = ((TX + 6) | 1);              // odd pitch of the staged x rows
-  static constexpr int LP = TX | 1;                      // odd pitch of the per-cell accumulator
+  static constexpr int LP = TX | 1;                      // odd pitch of the per-cell accumulator and of the y / z stages
   static constexpr int NOUT = TX * TY * TZ;
-  static constexpr size_t SMEM = (size_t)(2 * ROWS * XP + ROWS * LP) * sizeof(double);
+  static constexpr int SX = ROWS * XP;                                    // staged cells, x sweep
+  static constexpr int SY = NDIM > 1 ? TZ * (TY + 6) * LP : 0;            //               y sweep: [TZ][TY+6][LP]
+  static constexpr int SZ = NDIM > 2 ? (TZ + 6) * TY * LP : 0;            //               z sweep: [TZ+6][TY][LP]
+  static constexpr int STAGE = SX > SY ? (SX > SZ ? SX : SZ) : (SY > SZ ? SY : SZ);
+  static constexpr size_t SMEM = (size_t)(2 * STAGE + ROWS * LP) * sizeof(double);
   static_assert(TX % SEG == 0 && (NDIM < 2 || TY % SEG == 0) && (NDIM < 3 || TZ % SEG == 0), "tile % SEG");
   static_assert(NT >= 32 && NT <= 1024, "threads");
 };
@@ -110,7 +115,7 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
   using C = FluxCfg<NDIM, TX, TY, TZ, SEG>;
   constexpr int NT = C::NT;
   extern __shared__ double flux_smem[];
-  double *sFp = flux_smem, *sFm = sFp + C::ROWS * C::XP, *sL = sFm + C::ROWS * C::XP;
+  double *sFp = flux_smem, *sFm = sFp + C::STAGE, *sL = sFm + C::STAGE;
 
   const int tid = threadIdx.x;
   const int patch = blockIdx.y;
@@ -123,7 +128,6 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
   const double *U0p = U0 + pbase * P.nvar;
   double *Uop = Uout + pbase * P.nvar;
   const double *pp = P.p + pbase;
-  const long long st1 = P.st[1], st2 = P.st[2];
   double alpha[3], hidx[3];
 #pragma unroll
   for (int d = 0; d < NDIM; d++) {
@@ -142,7 +146,7 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
     {
       const double cM = m == 1 ? 1.0 : 0.0;
       const double *ux = P.vel + pbase;
-#pragma unroll 1
+#pragma unroll 4
       for (int it = tid; it < C::ROWS * (TX + 6); it += NT) {
         const int xi = it % (TX + 6), r = it / (TX + 6);
         const int gx = min(o0 + xi - 3, mx0), gy = min(o1 + r % TY, in1), gz = min(o2 + r / TY, in2);
@@ -161,28 +165,36 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
       for (int i = 0; i < SEG; i++) sL[r * C::LP + xs + i] = (Fh[i] - Fh[i + 1]) * hidx[0];
       __syncthreads();
     }
-    // ---------------- y and z: strided pencils straight from global memory
+    // ---------------- y and z: the tile extended by 3 cells along d is staged as 2f+- (coalesced along x, all
+    //                  loads of a thread independent), pencils then read shared memory (lanes along x: conflict-free)
 #pragma unroll
     for (int d = 1; d < NDIM; d++) {
       const double cM = m == 1 + d ? 1.0 : 0.0;
       const double *ud = P.vel + (long long)d * P.np * P.pc + pbase;
+      const double al = alpha[d];
+      const int EY = d == 1 ? TY + 6 : TY, EZ = d == 2 ? TZ + 6 : TZ;     // staged extent
+#pragma unroll 4
+      for (int it = tid; it < TX * EY * EZ; it += NT) {
+        const int x = it % TX, yy = (it / TX) % EY, zz = it / (TX * EY);
+        const int gx = min(o0 + x, P.n[0] - 1);
+        const int gy = d == 1 ? min(o1 + yy - 3, mx1) : min(o1 + yy, in1);
+        const int gz = d == 2 ? min(o2 + zz - 3, mx2) : min(o2 + zz, in2);
+        const long long id = cell_index(P, gx, gy, gz);
+        double a, b;
+        split2(Um[id], ud[id], pp[id], cEn, cM, al, a, b);
+        sFp[(zz * EY + yy) * C::LP + x] = a;
+        sFm[(zz * EY + yy) * C::LP + x] = b;
+      }
+      __syncthreads();
       const int x = tid % TX, rest = tid / TX;
       // d == 1: pencils along y, the other index is z;  d == 2: pencils along z, the other index is y
       const int other = d == 1 ? rest % TZ : rest % TY;
       const int seg = (d == 1 ? rest / TZ : rest / TY) * SEG;
       const int ly = d == 1 ? seg : other, lz = d == 1 ? other : seg;
-      const int gx = min(o0 + x, P.n[0] - 1);
-      const int gy = d == 1 ? o1 + ly : min(o1 + ly, in1);
-      const int gz = d == 2 ? o2 + lz : min(o2 + lz, in2);
-      const long long sd = d == 1 ? st1 : st2;
-      const int gd = d == 1 ? gy : gz, mxd = d == 1 ? mx1 : mx2;
-      const long long id0 = cell_index(P, gx, gy, gz);
+      const int base = (lz * EY + ly) * C::LP + x;
+      const int sk = d == 1 ? C::LP : EY * C::LP;                          // stride of one pencil step in the stage
       double Fh[SEG + 1];
-      const double al = alpha[d];
-      weno_faces<SEG>([&](int k, double &a, double &b) {
-        const long long id = id0 + (long long)(min(gd + k - 3, mxd) - gd) * sd;
-        split2(Um[id], ud[id], pp[id], cEn, cM, al, a, b);
-      }, Fh);
+      weno_faces<SEG>([&](int k, double &a, double &b) { a = sFp[base + k * sk]; b = sFm[base + k * sk]; }, Fh);
       double *acc = sL + (lz * TY + ly) * C::LP + x;
       const int sa = d == 1 ? C::LP : TY * C::LP;
 #pragma unroll
