@@ -79,6 +79,37 @@ inline std::string xprod(const std::string &pre, const int *cnt, int ns, int ski
   return s;
 }
 
+// Device helpers shared by the generated kernels.
+//   exp_nb: branch-free exp (Cody-Waite reduction, degree-13 Taylor polynomial on |r| <= ln2/2: < 2 ulp), argument
+//           clamped to the finite range; half the instructions of the library exp and no slow-path branch, so the
+//           exponentials of neighbouring reactions interleave.
+//   rcp_nb: 1/x from the MUFU seed + 2 Newton steps (full fp64 precision for normal x of either sign; a zero or
+//           denormal pivot gives inf / nan, which the callers' isfinite checks flag).
+inline void emit_math(std::string &src) {
+  src += "__device__ __forceinline__ double exp_nb(double x) {\n"
+         "  x = fmin(fmax(x, -708.0), 709.0);\n"
+         "  const double t = fma(x, 1.4426950408889634, 6755399441055744.0);\n"
+         "  const int n = __double2loint(t);\n"
+         "  const double nf = t - 6755399441055744.0;\n"
+         "  double r = fma(nf, -6.93147180369123816490e-01, x);\n"
+         "  r = fma(nf, -1.90821492927058770002e-10, r);\n"
+         "  double p = 1.6059043836821613e-10;\n"
+         "  p = fma(p, r, 2.08767569878681e-09); p = fma(p, r, 2.505210838544172e-08); p = fma(p, r, 2.755731922398589e-07);\n"
+         "  p = fma(p, r, 2.7557319223985893e-06); p = fma(p, r, 2.48015873015873e-05); p = fma(p, r, 1.984126984126984e-04);\n"
+         "  p = fma(p, r, 1.388888888888889e-03); p = fma(p, r, 8.333333333333333e-03); p = fma(p, r, 4.1666666666666664e-02);\n"
+         "  p = fma(p, r, 1.6666666666666666e-01); p = fma(p, r, 0.5); p = fma(p, r, 1.0); p = fma(p, r, 1.0);\n"
+         "  const int n1 = n >> 1, n2 = n - n1;\n"
+         "  return p * __hiloint2double((n1 + 1023) << 20, 0) * __hiloint2double((n2 + 1023) << 20, 0);\n"
+         "}\n"
+         "__device__ __forceinline__ double rcp_nb(double x) {\n"
+         "  double r;\n"
+         "  asm(\"rcp.approx.ftz.f64 %0, %1;\" : \"=d\"(r) : \"d\"(x));\n"
+         "  r = fma(fma(-x, r, 1.0), r, r);\n"
+         "  r = fma(fma(-x, r, 1.0), r, r);\n"
+         "  return r;\n"
+         "}\n";
+}
+
 // Newton on e(T) = sum_k Y_k R_k (h_k/R_k - T) (eq 4.3-4.4; reading A6): expects yr<k>, e, T; sets ok
 inline void emit_newton(Emitter &E, const MechC &M) {
   const int ns = M.ns;
@@ -161,6 +192,7 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
   src += "// generated by chemgen.h for ns=" + I(ns) + " nr=" + I(nr) + " ndim=" + I(ndim) + "\n";
   src += "struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2;"
          " long long st0, st1, st2, pc; int np; };\n";
+  emit_math(src);
   src += "extern \"C\" __global__ void __launch_bounds__(" + I(NT) + MINB_STR + ") k_chem_jit(ChemArgs a) {\n";
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
   if (big) {
@@ -225,7 +257,7 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
     if (M.b[i] != 0.0) lnk = "fma(" + num(M.b[i]) + ", lnT, " + lnk + ")";
     if (M.Ta[i] != 0.0) lnk = "fma(" + num(-M.Ta[i]) + ", iT, " + lnk + ")";
     E.line("const double lk" + si + " = " + lnk + ";");
-    E.line("const double kf" + si + " = exp(lk" + si + ");");
+    E.line("const double kf" + si + " = exp_nb(lk" + si + ");");
     const bool rev = M.rev[i] != 0, tb = M.tb[i] != 0;
     if (rev) {
       std::string dg = M.dn[i] != 0 ? num((double)M.dn[i]) + " * lnC0" : std::string("0.0");
@@ -233,7 +265,7 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
         if (dnu[k] == 0) continue;
         dg = "fma(" + num((double)dnu[k]) + ", g" + I(k) + ", " + dg + ")";
       }
-      E.line("const double kb" + si + " = exp(lk" + si + " - " + dg + ");");
+      E.line("const double kb" + si + " = exp_nb(lk" + si + " - " + dg + ");");
     }
     std::string rn = xprod("kf" + si, cf, ns, -1);
     if (rev) rn += " - " + xprod("kb" + si, cb, ns, -1);
@@ -317,7 +349,7 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
     } else {
       E.line("  if (!(fabs(" + A(c, c) + ") > 0.0)) ok = false;");
     }
-    E.line("  const double ip = 1.0 / " + A(c, c) + ";");
+    E.line("  const double ip = rcp_nb(" + A(c, c) + ");");
     for (int r = c + 1; r < n1; r++) {
       E.line("  { const double f = " + A(r, c) + " * ip;");
       for (int b = c + 1; b < n1; b++) E.line("    " + A(r, b) + " = fma(-f, " + A(c, b) + ", " + A(r, b) + ");");

@@ -180,23 +180,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   src += "};\n__constant__ int g_ti[" + I(NTI) + "] = {";
   for (int q = 0; q < NTI; q++) src += (q ? ", " : "") + ti[q];
   src += "};\n";
-  // branch-free exp (Cody-Waite reduction, degree-13 Taylor polynomial on |r| <= ln2/2: < 2 ulp), argument clamped
-  // to the finite range; lets the scheduler interleave the exponentials of two reactions
-  src += "__device__ __forceinline__ double exp_nb(double x) {\n"
-         "  x = fmin(fmax(x, -708.0), 709.0);\n"
-         "  const double t = fma(x, 1.4426950408889634, 6755399441055744.0);\n"
-         "  const int n = __double2loint(t);\n"
-         "  const double nf = t - 6755399441055744.0;\n"
-         "  double r = fma(nf, -6.93147180369123816490e-01, x);\n"
-         "  r = fma(nf, -1.90821492927058770002e-10, r);\n"
-         "  double p = 1.6059043836821613e-10;\n"
-         "  p = fma(p, r, 2.08767569878681e-09); p = fma(p, r, 2.505210838544172e-08); p = fma(p, r, 2.755731922398589e-07);\n"
-         "  p = fma(p, r, 2.7557319223985893e-06); p = fma(p, r, 2.48015873015873e-05); p = fma(p, r, 1.984126984126984e-04);\n"
-         "  p = fma(p, r, 1.388888888888889e-03); p = fma(p, r, 8.333333333333333e-03); p = fma(p, r, 4.1666666666666664e-02);\n"
-         "  p = fma(p, r, 1.6666666666666666e-01); p = fma(p, r, 0.5); p = fma(p, r, 1.0); p = fma(p, r, 1.0);\n"
-         "  const int n1 = n >> 1, n2 = n - n1;\n"
-         "  return p * __hiloint2double((n1 + 1023) << 20, 0) * __hiloint2double((n2 + 1023) << 20, 0);\n"
-         "}\n";
+  emit_math(src);
   // =========================================================================== kernel
   src += "#define SM(r) sm_[(r) * 32 + lane]\n";
   src += "#define BAR() asm volatile(\"bar.sync 0;\" ::: \"memory\")\n";
@@ -438,15 +422,15 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   // owner of column cn (variables cn, pbn in scope), already rotated into cn's frame: physical rows 1..n1-1-cn are the
   // rows below the diagonal.  Publishes "needs a swap" and, if no cell does, the multipliers of all other rows.
   auto owner = [&](int s, const std::string &ind) {
-    E.line(ind + "{ const double ac = fabs(" + A(s, 0) + "), ip = 1.0 / " + A(s, 0) + ";");
+    E.line(ind + "{ const double ac = fabs(" + A(s, 0) + "), ip = rcp_nb(" + A(s, 0) + ");");
     E.line(ind + "  const int nb_ = " + I(n1) + " - cn;");
     E.line(ind + "  int bad = !(ac > 0.0);                       // branch-free: 18 independent compares");
     for (int p = 1; p < n1; p++) E.line(ind + "  bad |= (int)(" + I(p) + " < nb_) & (int)(fabs(" + A(s, p) + ") > ac);");
+    // multipliers are published unconditionally (garbage if a swap is needed: every role then leaves the loop
+    // before using them), so nothing on the owner's critical path waits for a vote
+    for (int p = 1; p < n1; p++) E.line(ind + "  SM(" + I(L.oF) + " + cn * " + I(n1) + " + " + I(p) + ") = " + A(s, p) + " * ip;");
+    E.line(ind + "  SM(" + I(L.oIP) + " + cn) = ip;");
     E.line(ind + "  s_flag[cn * 64 + lane] = bad;");
-    E.line(ind + "  if (!__any_sync(0xffffffffu, bad != 0)) {");
-    for (int p = 1; p < n1; p++) E.line(ind + "    SM(" + I(L.oF) + " + cn * " + I(n1) + " + " + I(p) + ") = " + A(s, p) + " * ip;");
-    E.line(ind + "    SM(" + I(L.oIP) + " + cn) = ip;");
-    E.line(ind + "  }");
     E.line(ind + "}");
   };
   E.line("int c0 = " + I(n1) + ";     // first column of the pivoted slow path (" + I(n1) + ": none)");
