@@ -38,8 +38,31 @@ def flux_ops_per_cell_stage(ndim, nvar):
     return nvar * (ndim * (3 + 2 * WENO_OPS + 3) + 3)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
-# `ncu --set full` capture of this same command (profiles/r1d_summary.md); other workloads: not captured.
+def chem_ops_per_cell(mech):
+    """Algorithmic DP instructions (FMA = 1) of the point-implicit update of one cell, counted from the mechanism
+    (DESIGN.md section 6): 3 Newton iterations on e(T); per reaction 2 exponentials (25 each) + Arrhenius arguments,
+    concentration products and the net rate (12); one multiply per non-zero dq_i/dX_j and one add per non-zero
+    contribution to D_kj (third-body reactions touch every column); I - dt J (2 per entry); elimination n^3/3 and
+    the two triangular solves n^2."""
+    import numpy as np
+    ns, nr, n1 = mech.ns, mech.nr, mech.ns - 1
+    nu_f, nu_b = np.asarray(mech.nu_f), np.asarray(mech.nu_b)
+    tb = np.asarray(mech.third_body).astype(bool) if mech.third_body is not None else np.zeros(nr, bool)
+    deg = max([q for q in range(5) if np.any(np.asarray(mech.nasa)[:, q] != 0.0)] + [0])
+    newton = 3 * ns * (2 * deg + 3)
+    rates = nr * (2 * 25 + 12)
+    entries = updates = 0
+    for i in range(nr):
+        rows = int(np.count_nonzero((nu_b[i] - nu_f[i])[:n1]))
+        cols = ns if tb[i] else int(np.count_nonzero(nu_f[i] + nu_b[i]))
+        entries += cols
+        updates += rows * cols
+    return newton + rates + entries + updates + 2 * n1 * n1 + n1 ** 3 // 3 + n1 * n1
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel (stages 2 and 3; the first
+# stage reads U^n only once: 4.21e8), from the committed `ncu --set full` capture of this same command
+# (profiles/r1e_summary.md); other workloads: not captured.
 NCU_TRAFFIC_BYTES = {"cfg2_2d_channel_4096x512": 6.32e8}
 
 
@@ -201,6 +224,7 @@ def main():
     cells = case.cells
     K, W = args.steps, max(args.warmup, 3)
     s = binding.Solver(case.grid, case.mech, case.blocks, device=local)
+    chem_kernel = s.chem_kernel()
     dev = f"cuda:{local}"
     Ud = torch.from_numpy(case.U).to(dev); Td = torch.from_numpy(case.T).to(dev)
     s.set_state(Ud, Td)
@@ -277,11 +301,18 @@ def main():
         byt = flux_bytes_per_cell_stage(nd, nvar) * cells
         roof = {"kernel": "k_flux_rk2" if nd == 2 else "k_flux_rk", "bound": "alu", "achieved": ops / fl_avg / 1e12, "peak": dfma / 1e12,
                 "unit": "T fp64-instr/s (FMA=1)", "frac": ops / fl_avg / dfma, "traffic": NCU_TRAFFIC_BYTES.get(case.name),
-                "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1d_summary.md)",
+                "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1e_summary.md)",
                 "peak_source": "measured: register-resident DFMA microbenchmark in this run",
                 "avg_launch_ms": fl_avg * 1e3, "launches_timed": fl_n,
                 "hbm": {"achieved": byt / fl_avg / 1e9, "peak": hbm_peak, "unit": "GB/s",
                         "frac": byt / fl_avg / 1e9 / hbm_peak, "peak_source": hbm_src}}
+        ch_ms, ch_n = phases["chem"]
+        if ch_n > 0:      # the chemistry kernel's achieved FP64 fraction (north_star asks for it)
+            ch_ops = chem_ops_per_cell(case.mech)
+            ch_avg = ch_ms / ch_n * 1e-3
+            roof["chem"] = {"kernel": "k_chem_jit (%s)" % chem_kernel, "bound": "alu", "ops_per_cell": ch_ops,
+                            "achieved": ch_ops * cells / ch_avg / 1e12, "peak": dfma / 1e12, "unit": "T fp64-instr/s (FMA=1)",
+                            "frac": ch_ops * cells / ch_avg / dfma, "avg_launch_ms": ch_avg * 1e3}
         line = {"metric": METRIC, "value": cells * world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
                 "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",

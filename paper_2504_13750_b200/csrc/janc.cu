@@ -37,6 +37,12 @@ struct janc_ctx {
   int parity;
   long long launches;
   int num_sms;
+  // One step = 11..12 small launches; a step of each slot parity is captured once into a CUDA graph and replayed
+  // (launch-bound grids: cfg 0 / cfg 1).  Captured on an internal stream (the caller's may be the legacy default
+  // stream, which cannot be captured), launched on the caller's.
+  struct StepGraph { cudaGraphExec_t exec = nullptr; double cfl = 0.0, dt = 0.0; int flags = 0; long long launches = 0; } graph[2];
+  cudaStream_t cap_stream = nullptr;
+  bool use_graph = true, warmed = false;
   int jit_chem_nt, jit_chem_cells, jit_chem_mode;   // threads per CTA, cells per CTA, see jit_chem_mode()
   size_t jit_chem_smem;
   cudaKernel_t jit_prim;     // mechanism-specialised cons->prim kernel, null if not in use
@@ -106,6 +112,7 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
   c->g = *grid;
   c->device = device;
   c->num_sms = 148;
+  { const char *ng = getenv("JANC_NO_GRAPH"); c->use_graph = !(ng && ng[0] && ng[0] != '0'); }
   cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
   c->stream = (cudaStream_t)cuda_stream;
   c->np = grid->n_patches > 0 ? grid->n_patches : 1;
@@ -146,9 +153,13 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
   return JANC_OK;
 }
 
+static void invalidate_graphs(janc_ctx *c);
+
 extern "C" void janc_destroy(janc_ctx *c) {
   if (!c) return;
   if (g_mech_owner == c->id) g_mech_owner = 0;
+  invalidate_graphs(c);
+  if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
   delete c;
 }
 
@@ -361,6 +372,7 @@ extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
   if (!c || !m) return JANC_EINVAL;
   int rc = fill_mech(m, c->mech, c->err);
   if (rc) return rc;
+  invalidate_graphs(c);
   jit_setup(c);
   c->ns = m->ns; c->nr = m->nr;
   c->nvar = c->g.ndim + 2 + m->ns - 1;
@@ -421,6 +433,7 @@ extern "C" int janc_bind_workspace(janc_ctx *c, void *dev_ptr, size_t bytes) {
   size_t need = janc_workspace_bytes(c);
   if (bytes < need || ((uintptr_t)dev_ptr & 255)) { c->err = "workspace too small or misaligned"; return JANC_EINVAL; }
   CK(cudaSetDevice(c->device));
+  invalidate_graphs(c);
   carve(c, (char *)dev_ptr, nullptr);
   c->ws_bytes = need;
   CK(cudaMemsetAsync(dev_ptr, 0, need, c->stream));
@@ -431,6 +444,7 @@ extern "C" int janc_bind_workspace(janc_ctx *c, void *dev_ptr, size_t bytes) {
 // ------------------------------------------------------------------ block lists
 extern "C" int janc_set_blocks(janc_ctx *c, const int32_t *level, const int32_t *nbr, const int32_t *parent) {
   if (!c || c->g.n_patches <= 0 || !level || !nbr) return JANC_EINVAL;
+  invalidate_graphs(c);
   const int nd = c->g.ndim, nf = 2 * nd, np = c->np;
   for (int p = 0; p < np; p++) {
     if (level[p] < 0 || level[p] >= c->g.n_levels) { c->err = "level out of range"; return JANC_EINVAL; }
@@ -631,7 +645,7 @@ static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uou
   const Params &P = c->P;
   if (c->g.ndim == 1) launch_flux<1, 128, 1, 1, 4>(c, Uk, U0, Uout, slot_base, coef);
   else if (c->g.ndim == 2) {
-    if (gather_mode(c)) launch_flux2<16, 16, 8, true>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches: halo gathered in-kernel
+    if (gather_mode(c)) launch_flux2<16, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches: halo gathered in-kernel; 2 warps per patch
     else if ((long long)c->np * c->ncell < 600000) launch_flux2<32, 16, 4>(c, Uk, U0, Uout, slot_base, coef);   // small grids: 4x the CTAs
     else launch_flux2<64, 16, 8>(c, Uk, U0, Uout, slot_base, coef);
   } else launch_flux<3, 32, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);
@@ -711,6 +725,50 @@ static void step_once(janc_ctx *c, double cfl, double dt_fixed, int flags, Prof 
   c->parity = 1 - par;
 }
 
+static void invalidate_graphs(janc_ctx *c) {
+  for (auto &G : c->graph) { if (G.exec) cudaGraphExecDestroy(G.exec); G.exec = nullptr; }
+  c->warmed = false;
+}
+
+// One step through the cached graph of the current parity; the first step after any (re)configuration runs eagerly
+// (it also sets the kernels' shared-memory attributes), and any capture problem switches the context to eager launches.
+static void run_step(janc_ctx *c, double cfl, double dt_fixed, int flags) {
+  if (!c->use_graph || !c->warmed) { step_once(c, cfl, dt_fixed, flags, nullptr); c->warmed = true; return; }
+  const int par = c->parity;
+  janc_ctx::StepGraph &G = c->graph[par];
+  if (!G.exec || G.cfl != cfl || G.dt != dt_fixed || G.flags != flags) {
+    if (G.exec) { cudaGraphExecDestroy(G.exec); G.exec = nullptr; }
+    if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) c->cap_stream = nullptr;
+    bool ok = c->cap_stream != nullptr;
+    const cudaStream_t user = c->stream;
+    const long long l0 = c->launches;
+    cudaGraph_t g = nullptr;
+    if (ok) ok = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed) == cudaSuccess;
+    if (ok) {
+      c->stream = c->cap_stream;
+      step_once(c, cfl, dt_fixed, flags, nullptr);
+      c->stream = user;
+      ok = cudaStreamEndCapture(c->cap_stream, &g) == cudaSuccess && g != nullptr;
+      G.launches = c->launches - l0;
+      c->launches = l0;
+      c->parity = par;
+    }
+    if (ok) ok = cudaGraphInstantiate(&G.exec, g, 0) == cudaSuccess;
+    if (g) cudaGraphDestroy(g);
+    if (!ok) {
+      cudaGetLastError();
+      G.exec = nullptr;
+      c->use_graph = false;
+      step_once(c, cfl, dt_fixed, flags, nullptr);
+      return;
+    }
+    G.cfl = cfl; G.dt = dt_fixed; G.flags = flags;
+  }
+  if (cudaGraphLaunch(G.exec, c->stream) != cudaSuccess) { cudaGetLastError(); c->use_graph = false; step_once(c, cfl, dt_fixed, flags, nullptr); return; }
+  c->launches += G.launches;
+  c->parity = 1 - par;
+}
+
 static int check_ready(janc_ctx *c) {
   if (!c) return JANC_EINVAL;
   if (!c->have_state) { c->err = "no state"; return JANC_ESTATE; }
@@ -730,7 +788,7 @@ extern "C" int janc_step(janc_ctx *c, int nsteps, double cfl, double dt_fixed, i
     CK(cudaMemcpyAsync(&t0, c->P.scal + 1, 8, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
   }
-  for (int s = 0; s < nsteps; s++) step_once(c, cfl, dt_fixed, flags, nullptr);
+  for (int s = 0; s < nsteps; s++) run_step(c, cfl, dt_fixed, flags);
   CK(cudaGetLastError());
   if (t_advanced) {
     double t1 = 0.0;

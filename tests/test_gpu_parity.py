@@ -352,3 +352,24 @@ def test_gpu_detonation_speed_is_cj(B):
     s.close()
     D = (marks[1][1] - marks[0][1]) / (marks[1][0] - marks[0][0])
     assert abs(D - d_cj()) <= 0.004 * d_cj(), (D, d_cj())
+
+
+def test_graph_replay_is_bitwise_the_eager_path(B, monkeypatch):
+    """janc_step replays a captured CUDA graph per slot parity (first step eager).  Same kernels, same order:
+    the state must be bit-identical to eager launches, across several calls, a cfl change (re-capture) and the
+    explicit variant (other flags), in uniform and block-list mode; the launch counter counts graph nodes too."""
+    for case in (I.config1(nx=96, ny=40), I.config3(pcols=8, prows=4, npc=16), I.config0(n=130)):
+        out = []
+        for no_graph in ("0", "1"):
+            monkeypatch.setenv("JANC_NO_GRAPH", no_graph)
+            s = B.Solver(case.grid, case.mech, case.blocks)
+            s.set_state(case.U, case.T)
+            t = s.step(3, cfl=case.cfl) + s.step(1, cfl=case.cfl) + s.step(4, cfl=0.5 * case.cfl)
+            t += s.step(2, cfl=case.cfl, chem=False) + s.step(3, cfl=case.cfl)
+            U, T = s.get_state()
+            assert s.status == 0
+            out.append((t, U, T, s.launch_count()))
+            s.close()
+        assert out[0][0] == out[1][0]
+        assert np.array_equal(out[0][1], out[1][1]) and np.array_equal(out[0][2], out[1][2])
+        assert out[0][3] == out[1][3] > 0
