@@ -35,7 +35,7 @@
 namespace chemgen {
 
 struct RolesLayout {
-  int oX, oP, oN, oRN, oDL, oRHS, oF, oPIV, oIP, oXS, oR, rows;   // offsets in rows of 32 doubles
+  int oX, oP, oN, oRN, oDL, oRHS, oF, oPIV, oIP, oXS, oNX, oR, rows;   // offsets in rows of 32 doubles
   size_t ntd, nti;                                                 // table sizes (doubles, ints) behind the rows
   size_t smem() const { return (size_t)rows * 32 * sizeof(double) + ntd * sizeof(double) + nti * sizeof(int); }
 };
@@ -67,7 +67,7 @@ inline bool roles_applicable(const MechC &M) {
   return M.ns >= 3 && M.ns <= JANC_ROLES * JANC_ROLES_MAXSLOT && M.nr >= 1;
 }
 
-inline RolesLayout roles_layout(const MechC &M) {
+inline RolesLayout roles_layout(const MechC &M, int ndim) {
   const int ns = M.ns, n1 = ns - 1, nr = M.nr;
   RolesLayout L;
   int o = 0;
@@ -80,6 +80,7 @@ inline RolesLayout roles_layout(const MechC &M) {
   L.oPIV = o; o += n1;                       // "this cell needs a row swap" (int, first half of each row), per column
   L.oIP = o; o += n1;                        // reciprocal pivots
   L.oXS = o; o += n1;                        // solution
+  L.oNX = o; o += ndim + 2 + n1 + 1;         // U (nvar rows) and T of the NEXT turn's cells, prefetched with cp.async
   // one region, three lives: M k_f, M k_b, q per reaction (until the assembly barrier); the multipliers of every
   // column (elimination: nothing is reused, so the roles may run several columns apart); the whole system (slow path)
   L.oR = o; o += std::max(3 * nr, n1 * (n1 + 1));
@@ -94,7 +95,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   const int ns = M.ns, nr = M.nr, n1 = ns - 1, nvar = ndim + 2 + n1, NR = JANC_ROLES;
   const int NSL = (ns + NR - 1) / NR;                  // column slots per role (columns 0..n1)
   const int wN = n1 % NR, sN = n1 / NR;                // role / slot of column N (later the right-hand side)
-  const RolesLayout L = roles_layout(M);
+  const RolesLayout L = roles_layout(M, ndim);
   Emitter E;
   std::string &src = E.s;
   auto row = [](int r) { return "SM(" + I(r) + ")"; };
@@ -186,6 +187,22 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   src += "#define BAR() asm volatile(\"bar.sync 0;\" ::: \"memory\")\n";
   src += "#define AWAIT(id) asm volatile(\"barrier.sync %0, " + I(NR * 32) + ";\" :: \"r\"(id) : \"memory\")\n";
   src += "#define PUBLISH(id) do { asm volatile(\"barrier.arrive %0, " + I(NR * 32) + ";\" :: \"r\"(id) : \"memory\"); } while (0)\n";
+  // the next turn's inputs: (nvar + 1) x 32 doubles, one 8-byte cp.async each, spread over the CTA
+  src += "__device__ __forceinline__ void prefetch_turn(const ChemArgs &a, double *sm_, long long bt, long long nbp, long long ncell) {\n"
+         "  for (int q = threadIdx.x; q < " + I((nvar + 1) * 32) + "; q += " + I(NR * 32) + ") {\n"
+         "    const int v = q >> 5, l = q & 31;\n"
+         "    const int patch = (int)(bt / nbp);\n"
+         "    long long t = (bt - (long long)patch * nbp) * 32 + l;\n"
+         "    if (t >= ncell) t = ncell - 1;\n"
+         "    const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;\n"
+         "    const int cj = (int)(r_ % a.n1), ck = (int)(r_ / a.n1);\n"
+         "    const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;\n"
+         "    const double *src = v < " + I(nvar) + " ? a.U + ((long long)patch * " + I(nvar) + " + v) * a.pc + id : a.T + (long long)patch * a.pc + id;\n"
+         "    const unsigned dst = (unsigned)__cvta_generic_to_shared(sm_ + (" + I(L.oNX) + " + v) * 32 + l);\n"
+         "    asm volatile(\"cp.async.ca.shared.global [%0], [%1], 8;\" :: \"r\"(dst), \"l\"(src) : \"memory\");\n"
+         "  }\n"
+         "  asm volatile(\"cp.async.commit_group;\" ::: \"memory\");\n"
+         "}\n";
   src += "extern \"C\" __global__ void __launch_bounds__(" + I(NR * 32) + ", 1) k_chem_jit(ChemArgs a) {\n";
   E.line("extern __shared__ double sm_[];");
   E.line("const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;");
@@ -199,6 +216,8 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("int *s_flag = (int *)(sm_ + " + I(L.oPIV * 32) + ");");
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2, nbp = (ncell + 31) / 32, nbt = nbp * a.np;");
   E.line("const double dt = a.scal[0];");
+  E.line("if ((long long)blockIdx.x < nbt) prefetch_turn(a, sm_, blockIdx.x, nbp, ncell);");
+  E.line("asm volatile(\"cp.async.wait_all;\" ::: \"memory\");");
   E.line("BAR();");
   E.line("#pragma unroll 1");
   E.line("for (long long bt = blockIdx.x; bt < nbt; bt += gridDim.x) {   // persistent CTA: 32 cells per turn");
@@ -212,16 +231,17 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("double *Up = a.U + (long long)patch * " + I(nvar) + " * a.pc + id;");
   E.line("const long long pid = (long long)patch * a.pc + id;");
   // ---- cons -> prim pieces (eq 4.2); species k = w + 8 s belong to this role
-  E.line("const double rho = Up[0], irho = 1.0 / rho;");
+  E.line("const double rho = SM(" + I(L.oNX) + "), irho = 1.0 / rho;");
   E.line("double ke = 0.0;");
   for (int d = 0; d < ndim; d++)
-    E.line("{ const double ud = Up[" + I(1 + d) + " * a.pc] * irho; ke = fma(0.5 * ud, ud, ke); }");
-  E.line("const double e = Up[" + I(ndim + 1) + " * a.pc] * irho - ke;");
+    E.line("{ const double ud = SM(" + I(L.oNX + 1 + d) + ") * irho; ke = fma(0.5 * ud, ud, ke); }");
+  E.line("const double e = SM(" + I(L.oNX + ndim + 1) + ") * irho - ke;");
+  E.line("double T = SM(" + I(L.oNX + nvar) + ");");
   E.line("double pr_ = 0.0, py_ = 0.0;");
   for (int s = 0; s < NSL; s++) {
     const std::string ss = I(s);
     E.line("const int k" + ss + " = w + " + I(NR * s) + ";");
-    E.line("double ry" + ss + " = k" + ss + " < " + I(n1) + " ? Up[(long long)(" + I(ndim + 2) + " + k" + ss + ") * a.pc] : 0.0;");
+    E.line("double ry" + ss + " = k" + ss + " < " + I(n1) + " ? SM(" + I(L.oNX + ndim + 2) + " + k" + ss + ") : 0.0;");
     E.line("double Y" + ss + " = ry" + ss + " * irho;");
     E.line("pr_ += ry" + ss + "; py_ += Y" + ss + ";");
     E.line("if (k" + ss + " < " + I(n1) + ") SM(" + I(L.oX) + " + k" + ss + ") = ry" + ss + " * c_iW[k" + ss + "];");
@@ -229,6 +249,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("SM(" + I(L.oP) + " + w) = pr_; SM(" + I(L.oP + 8) + " + w) = py_;");
   E.line("if (w == 0) SM(" + I(L.oX + ns) + ") = 1.0;");
   E.line("BAR();");
+  E.line("if (bt + gridDim.x < nbt) prefetch_turn(a, sm_, bt + gridDim.x, nbp, ncell);   // lands during this turn");
   E.line("{ double rsum = 0.0, ysum = 0.0;");
   E.line("  #pragma unroll");
   E.line("  for (int q = 0; q < 8; q++) { rsum += SM(" + I(L.oP) + " + q); ysum += SM(" + I(L.oP + 8) + " + q); }");
@@ -236,7 +257,6 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   for (int s = 0; s < NSL; s++)
     E.line("const double yr" + I(s) + " = k" + I(s) + " < " + I(ns) + " ? Y" + I(s) + " * c_Rk[k" + I(s) + " < " + I(ns) + " ? k" + I(s) + " : 0] : 0.0;");
   // ---- Newton on e(T) (eq 4.3-4.4, reading A6): partial sums per role, summed in the same order by everyone
-  E.line("double T = a.T[pid];");
   E.line("bool conv = false;");
   E.line("#pragma unroll 1");
   E.line("for (int it = 0; it < 50; it++) {");
@@ -510,7 +530,8 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     E.line("if (live && k" + I(s) + " < " + I(n1) + ") Up[(long long)(" + I(ndim + 2) + " + k" + I(s) + ") * a.pc] = ry" + I(s) +
            " + SM(" + I(L.oXS) + " + k" + I(s) + ");");
   E.line("if (!ok && live) *a.flag = 1;");
-  E.line("BAR();   // shared rows are reused by the next turn");
+  E.line("asm volatile(\"cp.async.wait_all;\" ::: \"memory\");");
+  E.line("BAR();   // shared rows are reused by the next turn; the prefetched inputs are visible to every role");
   E.line("}");
   src += "}\n#undef SM\n#undef BAR\n#undef AWAIT\n#undef PUBLISH\n";
   return src;
