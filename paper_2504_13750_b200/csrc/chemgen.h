@@ -80,24 +80,38 @@ inline std::string xprod(const std::string &pre, const int *cnt, int ns, int ski
 }
 
 // Device helpers shared by the generated kernels.
-//   exp_nb: branch-free exp (Cody-Waite reduction, degree-13 Taylor polynomial on |r| <= ln2/2: < 2 ulp), argument
+//   exp_nb: branch-free exp (Cody-Waite reduction, degree-13 Taylor polynomial on |r| <= ln2/2 in Estrin form: < 2 ulp), argument
 //           clamped to the finite range; half the instructions of the library exp and no slow-path branch, so the
 //           exponentials of neighbouring reactions interleave.
 //   rcp_nb: 1/x from the MUFU seed + 2 Newton steps (full fp64 precision for normal x of either sign; a zero or
 //           denormal pivot gives inf / nan, which the callers' isfinite checks flag).
-inline void emit_math(std::string &src) {
+inline void emit_math(std::string &src, bool estrin = false) {
   src += "__device__ __forceinline__ double exp_nb(double x) {\n"
          "  x = fmin(fmax(x, -708.0), 709.0);\n"
          "  const double t = fma(x, 1.4426950408889634, 6755399441055744.0);\n"
          "  const int n = __double2loint(t);\n"
          "  const double nf = t - 6755399441055744.0;\n"
          "  double r = fma(nf, -6.93147180369123816490e-01, x);\n"
-         "  r = fma(nf, -1.90821492927058770002e-10, r);\n"
+         "  r = fma(nf, -1.90821492927058770002e-10, r);\n";
+  // Horner (13 FMAs) where many threads hide the chain (one thread per cell); Estrin (16 operations, depth 5) in the
+  // role-warp kernel, which runs 2 warps per scheduler
+  if (estrin)
+    src +=
+         "  const double r2 = r * r, r4 = r2 * r2, r8 = r4 * r4;            // Estrin: dependency depth 5 instead of 13\n"
+         "  const double q0 = r + 1.0, q1 = fma(1.6666666666666666e-01, r, 0.5), q2 = fma(8.333333333333333e-03, r, 4.1666666666666664e-02);\n"
+         "  const double q3 = fma(1.984126984126984e-04, r, 1.388888888888889e-03), q4 = fma(2.7557319223985893e-06, r, 2.48015873015873e-05);\n"
+         "  const double q5 = fma(2.505210838544172e-08, r, 2.755731922398589e-07), q6 = fma(1.6059043836821613e-10, r, 2.08767569878681e-09);\n"
+         "  const double s0 = fma(q1, r2, q0), s1 = fma(q3, r2, q2), s2 = fma(q5, r2, q4);\n"
+         "  const double t0 = fma(s1, r4, s0), t1 = fma(q6, r4, s2);\n"
+         "  const double p = fma(t1, r8, t0);\n";
+  else
+    src +=
          "  double p = 1.6059043836821613e-10;\n"
          "  p = fma(p, r, 2.08767569878681e-09); p = fma(p, r, 2.505210838544172e-08); p = fma(p, r, 2.755731922398589e-07);\n"
          "  p = fma(p, r, 2.7557319223985893e-06); p = fma(p, r, 2.48015873015873e-05); p = fma(p, r, 1.984126984126984e-04);\n"
          "  p = fma(p, r, 1.388888888888889e-03); p = fma(p, r, 8.333333333333333e-03); p = fma(p, r, 4.1666666666666664e-02);\n"
-         "  p = fma(p, r, 1.6666666666666666e-01); p = fma(p, r, 0.5); p = fma(p, r, 1.0); p = fma(p, r, 1.0);\n"
+         "  p = fma(p, r, 1.6666666666666666e-01); p = fma(p, r, 0.5); p = fma(p, r, 1.0); p = fma(p, r, 1.0);\n";
+  src +=
          "  const int n1 = n >> 1, n2 = n - n1;\n"
          "  return p * __hiloint2double((n1 + 1023) << 20, 0) * __hiloint2double((n2 + 1023) << 20, 0);\n"
          "}\n"
