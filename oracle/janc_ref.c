@@ -15,6 +15,9 @@
  *   TVD-RK3
  *   rates, K_eq                PAPER.md:260-277 (eq 4.6-4.9)
  *   point-implicit             PAPER.md:297-304 (eq 4.12-4.13), :333, :340
+ *   explicit source variant    PAPER.md:322 (source_terms advanced with the convection terms by the TVD RK3),
+ *                              :338 (rhs = flux gradient + source_terms), :351-357 (advance_one_step without
+ *                              advance_source_term); the source is the mechanism's own W_k omega_k of eq 4.6
  *   average-down
  * No blocking, fusion or reordering beyond that.  OpenMP only splits independent cells/lines;
  * reductions are exact max, so results do not depend on the thread count.
@@ -66,6 +69,7 @@ typedef struct {
 } mech_t;
 
 typedef struct jref_ctx {
+  int explicit_src;            /* 1: chemical source added to the rhs of every RK stage */
   jref_grid g;
   int np, nvar, have_mech, have_state;
   int P[3], G[3];
@@ -554,11 +558,14 @@ static void flux_divergence(jref_ctx *c, const double *U, double alpha[2][3], do
 }
 
 /* rhs of PAPER.md:338: ghost fill -> update_aux -> flux gradient */
+static void source_terms(jref_ctx *c, const double *U, double *L);
+
 static void rhs(jref_ctx *c, double *U, double *L) {
   double s[2][3];
   ghost_fill(c, U);
   prim_all(c, U, 1, s);
   flux_divergence(c, U, s, L);
+  if (c->explicit_src) source_terms(c, U, L);
 }
 
 static void chemistry(jref_ctx *c, double dt) {
@@ -615,9 +622,37 @@ static void average_down(jref_ctx *c) {
   }
 }
 
+/* aux_func.source_terms of the explicit variant: S_k = W_k omega_k(T, X) of eq 4.6-4.9 on the
+ * species rows, evaluated on the stage state with the temperature update_aux has just recovered; added to L. */
+static void source_terms(jref_ctx *c, const double *U, double *L) {
+  const int *n = c->g.n; int nd = c->g.ndim, nv = c->nvar, ns = c->m.ns, n1 = ns - 1, nr = c->m.nr;
+  if (n1 < 1 || nr < 1) return;
+  for (int p = 0; p < c->np; p++) {
+    const double *Up = U + (long)p * nv * c->pc;
+#pragma omp parallel
+    {
+      double *work = malloc(sizeof(double) * (size_t)(ns + nr + nr * ns));
+      double *ry = malloc(sizeof(double) * ns), *om = malloc(sizeof(double) * ns), *J = malloc(sizeof(double) * (size_t)n1 * n1);
+#pragma omp for collapse(2) schedule(static)
+      for (int k = 0; k < n[2]; k++)
+        for (int j = 0; j < n[1]; j++)
+          for (int i = 0; i < n[0]; i++) {
+            long id = cidx(c, i, j, k);
+            for (int q = 0; q < n1; q++) ry[q] = Up[(long)(nd + 2 + q) * c->pc + id];
+            omega_jac(&c->m, c->T[(long)p * c->pc + id], Up[id], ry, om, J, work);
+            for (int q = 0; q < n1; q++) L[((long)p * nv + nd + 2 + q) * c->pc + id] += om[q];
+          }
+      free(work); free(ry); free(om); free(J);
+    }
+  }
+}
+
 /* advance_one_step: CFL -> advance_flux (RK3) -> advance_source_term */
+/* do_chem: 0 no chemistry, 1 point-implicit after the RK3, 2 explicit: source inside every RK stage
+ * and no advance_source_term */
 int jref_step(jref_ctx *c, int nsteps, double cfl, double dt_fixed, int do_chem, double *t_adv) {
   if (!c || !c->have_state) return JREF_ESTATE;
+  c->explicit_src = do_chem == 2;
   size_t N = (size_t)c->np * c->nvar * c->pc;
   double t = 0.0, s[2][3];
   for (int it = 0; it < nsteps; it++) {
@@ -643,7 +678,7 @@ int jref_step(jref_ctx *c, int nsteps, double cfl, double dt_fixed, int do_chem,
     for (size_t i = 0; i < N; i++) c->U[i] = c->U0[i] + (2.0 / 3.0) * ((c->U[i] - c->U0[i]) + dt * c->L[i]);
     /* advance_source_term: update_aux -> solve_implicit_rate -> U + dU */
     prim_all(c, c->U, 0, s);
-    if (do_chem) chemistry(c, dt);
+    if (do_chem == 1) chemistry(c, dt);
     average_down(c);
     t += dt;
   }

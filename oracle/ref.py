@@ -113,8 +113,10 @@ class RefSolver:
             raise RuntimeError(f"jref_set_state failed: {rc}")
 
     def step(self, nsteps, cfl=0.0, dt=0.0, chem=True):
+        """chem: True point-implicit, False none, "explicit" source inside the RK stages (:351-357)."""
         t = C.c_double(0.0)
-        rc = lib().jref_step(self._h, int(nsteps), C.c_double(cfl), C.c_double(dt), int(bool(chem)), C.byref(t))
+        mode = 2 if chem == "explicit" else int(bool(chem))
+        rc = lib().jref_step(self._h, int(nsteps), C.c_double(cfl), C.c_double(dt), mode, C.byref(t))
         self.status = rc
         return t.value
 

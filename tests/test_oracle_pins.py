@@ -461,6 +461,76 @@ def test_zero_d_vs_rk4_reference(ref, mech9):
     assert np.abs(U[0, 3:, 0, 0, 0] - ry).max() <= 2e-3 * np.abs(ry).max()
 
 
+# ----------------------------------------------------------------------------- explicit source variant
+def _zero_d_explicit(ref, mech, T0, p0, dt, nsteps, Y=None):
+    Y = I.hot_Y(mech.ns) if Y is None else Y
+    U = I.prim_to_cons(mech, 1, np.array([p0]), np.array([T0]), Y[None], [np.zeros(1)])
+    g = I.Grid(1, (1, 1, 1), (1e-3, 1, 1), (I.BC_OUTFLOW, 0, 0), (I.BC_OUTFLOW, 0, 0))
+    c = I.Case("0d", g, mech, U.reshape(1, -1, 1, 1, 1), np.array(T0).reshape(1, 1, 1, 1), 0.0, nsteps)
+    return run(ref, c, nsteps=nsteps, cfl=0.0, dt=dt, chem="explicit"), U
+
+
+def test_explicit_source_linear_decay_is_the_rk3_polynomial(ref):
+    """the source is advanced WITH the convection terms by the TVD RK3.  For a first
+    order reaction R -> P at constant k (b = 0, Ta = 0, no heat release, uniform gas at rest) the stage recursion
+    of SSP-RK3 on y' = -k y gives y (1 - z + z^2/2 - z^3/6), z = k dt, exactly; rho, momentum, E, T stay put."""
+    W = np.array([0.029, 0.029]); nasa = np.zeros((2, 7)); nasa[:, 0] = 3.5
+    k = 4.0e6
+    m = I.Mechanism(2, 1, W, nasa, np.array([[1, 0]], dtype=np.int32), np.array([[0, 1]], dtype=np.int32),
+                    np.array([k]), np.array([0.0]), np.array([0.0]), np.array([0], dtype=np.int32),
+                    np.array([0], dtype=np.int32), np.ones((1, 2)))
+    dt, nsteps = 1.0e-7, 3
+    (U, T, t, st), U0 = _zero_d_explicit(ref, m, 900.0, 2.0e5, dt, nsteps, Y=np.array([0.7, 0.3]))
+    assert st == 0 and abs(t - nsteps * dt) <= 1e-20
+    z = k * dt
+    amp = (1.0 - z + z * z / 2.0 - z ** 3 / 6.0) ** nsteps
+    assert abs(U[0, 3, 0, 0, 0] - U0[3, 0] * amp) <= 2e-15 * U0[3, 0]
+    assert np.array_equal(U[0, :3, 0, 0, 0], U0[:3, 0])
+    assert abs(T[0, 0, 0, 0] - 900.0) <= 1e-9
+
+
+def test_explicit_source_third_order_and_agrees_with_rk4(ref, mech9):
+    """0-D reactor with the 9-species mechanism: the explicit variant converges with order 3 in dt (T is refreshed
+    by update_aux in every stage) to the same answer as an independent classical RK4 on the oracle's omega."""
+    T0, p0, tend = 2000.0, 2.0e6, 4.0e-8
+    Y = I.hot_Y(9)
+    U0 = I.prim_to_cons(mech9, 1, np.array([p0]), np.array([T0]), Y[None], [np.zeros(1)])[:, 0]
+    rho = U0[0]
+
+    def f(ry):
+        Uc = np.concatenate([U0[:3], ry])
+        Tc = ref.cons2prim(mech9, 1, Uc, T0)[1][0]
+        return ref.omega_jac(mech9, Tc, rho, ry)[0]
+
+    ry = U0[3:].copy(); n = 2000; h = tend / n
+    for _ in range(n):
+        k1 = f(ry); k2 = f(ry + h / 2 * k1); k3 = f(ry + h / 2 * k2); k4 = f(ry + h * k3)
+        ry = ry + h / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+    errs = []
+    for ns_ in (8, 16, 32):
+        (U, T, _, st), _ = _zero_d_explicit(ref, mech9, T0, p0, tend / ns_, ns_)
+        assert st == 0
+        errs.append(np.abs(U[0, 3:, 0, 0, 0] - ry).max())
+    assert errs[2] <= 1e-6 * np.abs(ry).max()
+    assert errs[0] / errs[1] > 5.0 and errs[1] / errs[2] > 5.0, errs      # ~ 8 for third order
+
+
+def test_explicit_source_conserves_mass_elements_energy(ref, mech9):
+    """Periodic 2-D flow with the source inside the stages: total mass, momentum, energy and every element stay to
+    round-off (sum_k W_k omega_k = 0 and element balance hold stage by stage)."""
+    case = _random_smooth_2d(mech9, 24, 20, 5, I.BC_PERIODIC)
+    U, T, _, st = run(ref, case, nsteps=4, cfl=0.3, chem="explicit")
+    assert st == 0
+    for v in (0, 1, 2, 3):
+        assert abs(U[0, v].sum() - case.U[0, v].sum()) <= 1e-12 * max(np.abs(case.U[0, v]).sum(), 1.0)
+    el = np.asarray(mech9.elements, dtype=float)                     # [ns][n_elements]
+    def moles(Us):
+        ry = np.concatenate([Us[0, 4:], (Us[0, 0] - Us[0, 4:].sum(0))[None]])
+        return (ry.reshape(9, -1).sum(1) / mech9.W) @ el
+    assert np.abs(moles(U) - moles(case.U)).max() <= 1e-12 * np.abs(moles(case.U)).max()
+    assert np.abs(U - case.U).max() > 0
+
+
 # ----------------------------------------------------------------------------- block mode
 def test_tiled_block_list_equals_uniform_grid(ref, mech9):
     for bc in (I.BC_REFLECT, I.BC_PERIODIC):
