@@ -93,7 +93,10 @@ int janc_set_state(janc_ctx *, const double *U, const double *T_guess, int on_de
  * rhs: ghost fill, update_aux, LF-split WENO5 fluxes, divergence) -> advance_source_term
  * (point-implicit chemistry, eq 4.12-4.13) [-> average-down in 2-level block mode, PAPER.md:188].
  * cfl > 0: dt = cfl * min_d dx_d(finest) / max(|u_d| + c) each step (reading A16);
- * cfl <= 0: dt = dt_fixed.  flags: bit 0 set => skip chemistry (explicit variant).
+ * cfl <= 0: dt = dt_fixed.  flags: bit 0 set => no chemistry at all (explicit variant of PAPER.md:351-357 with a zero
+ * source_terms); bit 1 set => explicit variant with the mechanism's own source: S_k = W_k omega_k(T, X) (eq 4.6) is added to
+ * the right-hand side of every RK stage and advance_source_term is not executed; returns JANC_ESTATE if
+ * the run-time specialised source kernel is not available (no NVRTC).
  * t_advanced (host, nullable): receives the sum of dt; forces a stream synchronise. */
 int janc_step(janc_ctx *, int nsteps, double cfl, double dt_fixed, int flags, double *t_advanced);
 

@@ -386,6 +386,87 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
   return src;
 }
 
+// Explicit source variant: S_k = W_k omega_k(T, X) of the stage state is part of the
+// right-hand side of every RK stage.  The flux kernel has already written Uout = U0 + coef ((Uk - U0) + dt L(Uk)); this
+// kernel adds coef dt S(Uk) on the species rows, with the temperature cons->prim recovered for Uk.  One thread per cell,
+// rates fully specialised (literal indices, immediate coefficients); emits helpers only if `with_math`.
+inline std::string generate_source(const MechC &M, int ndim, bool with_math) {
+  const int ns = M.ns, nr = M.nr, n1 = ns - 1, nvar = ndim + 2 + n1;
+  Emitter E;
+  std::string &src = E.s;
+  src += "struct SrcArgs { const double *Uk; double *Uout; const double *T; const double *scal; int n0, n1, n2, G0, G1, G2;"
+         " long long st0, st1, st2, pc; double coef; };\n";
+  if (with_math) emit_math(src);
+  src += "extern \"C\" __global__ void __launch_bounds__(128) k_src_jit(SrcArgs a) {\n";
+  E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
+  E.line("const long long t = (long long)blockIdx.x * 128 + threadIdx.x;");
+  E.line("if (t >= ncell) return;");
+  E.line("const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;");
+  E.line("const int cj = (int)(r_ % a.n1), ck = (int)(r_ / a.n1);");
+  E.line("const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;");
+  E.line("const double *Up = a.Uk + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
+  E.line("double *Uo = a.Uout + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
+  E.line("const double T = a.T[(long long)blockIdx.y * a.pc + id];");
+  E.line("const double rho = Up[0];");
+  E.line("double rsum = 0.0;");
+  for (int k = 0; k < n1; k++) {
+    E.line("const double ry" + I(k) + " = Up[" + I(ndim + 2 + k) + " * a.pc], X" + I(k) + " = ry" + I(k) + " * " + num(M.invW[k]) + ";");
+    E.line("rsum += ry" + I(k) + ";");
+  }
+  E.line("const double X" + I(n1) + " = (rho - rsum) * " + num(M.invW[n1]) + ";");
+  std::vector<char> need_g(ns, 0);
+  bool any_rev = false;
+  for (int i = 0; i < nr; i++)
+    if (M.rev[i]) {
+      any_rev = true;
+      for (int k = 0; k < ns; k++) if (M.dnu[i][k] != 0.0) need_g[k] = 1;
+    }
+  E.line("const double lnT = log(T), iT = 1.0 / T;");
+  for (int k = 0; k < ns; k++) {
+    if (!need_g[k]) continue;
+    const double *c = M.nasa[k];
+    double sc[5] = {c[6], c[1], 0.5 * c[2], c[3] / 3.0, 0.25 * c[4]};
+    double hc[6] = {c[5], c[0], 0.5 * c[1], c[2] / 3.0, 0.25 * c[3], 0.2 * c[4]};
+    E.line("const double g" + I(k) + " = fma(" + num(c[0]) + ", lnT, " + horner(sc, 5) + ") - (" + horner(hc, 6) + ") * iT;");
+  }
+  if (any_rev) E.line("const double lnC0 = log(" + num(JANC_PATM / JANC_RU) + " * iT);");
+  Acc accW(ns);
+  for (int i = 0; i < nr; i++) {
+    const std::string si = I(i);
+    int cf[JANC_MAX_NS] = {0}, cb[JANC_MAX_NS] = {0}, dnu[JANC_MAX_NS];
+    for (int e = 0; e < M.nreac[i]; e++) cf[M.reac[i][e]]++;
+    for (int e = 0; e < M.nprod[i]; e++) cb[M.prod[i][e]]++;
+    for (int k = 0; k < ns; k++) dnu[k] = cb[k] - cf[k];
+    std::string lnk = num(M.lnA[i]);
+    if (M.b[i] != 0.0) lnk = "fma(" + num(M.b[i]) + ", lnT, " + lnk + ")";
+    if (M.Ta[i] != 0.0) lnk = "fma(" + num(-M.Ta[i]) + ", iT, " + lnk + ")";
+    E.line("const double lk" + si + " = " + lnk + ";");
+    std::string rn = xprod("exp_nb(lk" + si + ")", cf, ns, -1);
+    if (M.rev[i]) {
+      std::string dg = M.dn[i] != 0 ? num((double)M.dn[i]) + " * lnC0" : std::string("0.0");
+      for (int k = 0; k < ns; k++) {
+        if (dnu[k] == 0) continue;
+        dg = "fma(" + num((double)dnu[k]) + ", g" + I(k) + ", " + dg + ")";
+      }
+      rn += " - " + xprod("exp_nb(lk" + si + " - " + dg + ")", cb, ns, -1);
+    }
+    std::string q = "(" + rn + ")";
+    if (M.tb[i]) {
+      const double *ef = M.eff[M.tbi[i]];
+      std::string m = num(ef[0]) + " * X0";
+      for (int k = 1; k < ns; k++) m = "fma(" + num(ef[k]) + ", X" + I(k) + ", " + m + ")";
+      q = "(" + m + ") * " + q;
+    }
+    E.line("const double q" + si + " = " + q + ";");
+    for (int k = 0; k < n1; k++) accum(E, accW, k, "w" + I(k), dnu[k], "q" + si);
+  }
+  E.line("const double cdt = a.coef * a.scal[0];");
+  for (int k = 0; k < n1; k++)
+    if (accW.set[k]) E.line("Uo[" + I(ndim + 2 + k) + " * a.pc] = fma(cdt * " + num(M.W[k]) + ", w" + I(k) + ", Uo[" + I(ndim + 2 + k) + " * a.pc]);");
+  src += "}\n";
+  return src;
+}
+
 // Specialised fused cons->prim + thermo kernel with the alpha / CFL max-reduction (same contract as
 // k_prim of prim.cuh).  256 threads per CTA.
 inline std::string generate_prim(const MechC &M, int ndim) {

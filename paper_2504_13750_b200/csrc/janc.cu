@@ -46,6 +46,7 @@ struct janc_ctx {
   int jit_chem_nt, jit_chem_cells, jit_chem_mode;   // threads per CTA, cells per CTA, see jit_chem_mode()
   size_t jit_chem_smem;
   cudaKernel_t jit_prim;     // mechanism-specialised cons->prim kernel, null if not in use
+  cudaKernel_t jit_src = nullptr;   // explicit-variant source kernel (chemgen::generate_source), null without NVRTC
   cudaKernel_t jit_kernel;   // mechanism-specialised chemistry kernel (chemgen.h), null if not in use
   std::string jit_log;
   unsigned long long id;
@@ -284,7 +285,8 @@ static bool jit_compile(const std::string &src, std::vector<char> &cubin, std::s
 
 struct PrimArgs { const double *U; double *T; double *p; double *vel; double *dbgc; unsigned long long *slots;
                   const int *level; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np, reduce, slot_base; };
-struct JitKernels { cudaKernel_t chem = nullptr, prim = nullptr; };
+struct SrcArgs { const double *Uk; double *Uout; const double *T; const double *scal; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; double coef; };
+struct JitKernels { cudaKernel_t chem = nullptr, prim = nullptr, src = nullptr; };
 
 // 0: table-driven kernel, 1: register-resident specialised kernel (one thread per cell), 2: one thread per cell
 // with the matrix in smem, 3: 8 role-warps per 32 cells with the matrix columns in registers (chemgen_roles.h)
@@ -304,6 +306,7 @@ static int jit_chem_mode(const MechC &M) {
 static void jit_setup(janc_ctx *c) {
   c->jit_kernel = nullptr;
   c->jit_prim = nullptr;
+  c->jit_src = nullptr;
   c->jit_log.clear();
   const MechC &M = c->mech;
   const char *off = getenv("JANC_DISABLE_JIT");
@@ -317,11 +320,13 @@ static void jit_setup(janc_ctx *c) {
   std::string src = chemgen::generate_prim(M, c->g.ndim);
   if (mode == 3) src += chemgen::generate_roles(M, c->g.ndim);
   else if (chem) src += chemgen::generate(M, c->g.ndim, mode == 2);
+  const bool have_src = M.ns >= 2 && M.nr >= 1;
+  if (have_src) src += chemgen::generate_source(M, c->g.ndim, !chem);
   else c->jit_log = "chemistry: mechanism outside the specialised range; ";
   static std::map<std::string, JitKernels> cache;          // per process; one device per process
   const std::string key = std::to_string(c->device) + "\n" + src;
   auto it = cache.find(key);
-  if (it != cache.end()) { c->jit_kernel = it->second.chem; c->jit_prim = it->second.prim; return; }
+  if (it != cache.end()) { c->jit_kernel = it->second.chem; c->jit_prim = it->second.prim; c->jit_src = it->second.src; return; }
   std::vector<char> cubin;
   std::string log;
   if (!jit_compile(src, cubin, log)) { c->jit_log += log; return; }
@@ -331,12 +336,14 @@ static void jit_setup(janc_ctx *c) {
   JitKernels k;
   e = cudaLibraryGetKernel(&k.prim, lib, "k_prim_jit");
   if (e == cudaSuccess && chem) e = cudaLibraryGetKernel(&k.chem, lib, "k_chem_jit");
+  if (e == cudaSuccess && have_src) e = cudaLibraryGetKernel(&k.src, lib, "k_src_jit");
   if (e == cudaSuccess && c->jit_chem_smem > 48 * 1024)
     e = cudaKernelSetAttributeForDevice(k.chem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->jit_chem_smem, c->device);
   if (e != cudaSuccess) { c->jit_log += std::string("cudaLibraryGetKernel: ") + cudaGetErrorString(e); cudaGetLastError(); return; }
   cache[key] = k;
   c->jit_kernel = k.chem;
   c->jit_prim = k.prim;
+  c->jit_src = k.src;
 }
 
 extern "C" const char *janc_chem_kernel(const janc_ctx *c) {
@@ -356,6 +363,7 @@ extern "C" int janc_jit_probe(const janc_mech *m, int ndim, char *src_out, size_
   std::string src = chemgen::generate_prim(M, ndim);
   if (jit_chem_mode(M) == 3) src += chemgen::generate_roles(M, ndim);
   else if (jit_chem_mode(M)) src += chemgen::generate(M, ndim, jit_chem_mode(M) == 2);
+  if (M.ns >= 2 && M.nr >= 1) src += chemgen::generate_source(M, ndim, jit_chem_mode(M) == 0);
   if (src_len) *src_len = src.size();
   if (src_out && cap > 0) { size_t n = src.size() < cap - 1 ? src.size() : cap - 1; memcpy(src_out, src.data(), n); src_out[n] = 0; }
   if (cubin_bytes) {
@@ -690,6 +698,16 @@ static void do_chem(janc_ctx *c, double *U, Prof *pf) {
   prof_mark(c, pf, 3);
 }
 
+// explicit variant: add coef dt S(Uk) to the stage result on the species rows
+static void do_src(janc_ctx *c, const double *Uk, double *Uout, double coef, Prof *pf) {
+  const Params &P = c->P;
+  SrcArgs a{Uk, Uout, P.T, P.scal, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc, coef};
+  void *args[] = {&a};
+  cudaLaunchKernel((const void *)c->jit_src, cell_grid(c, 128, c->np), dim3(128, 1, 1), args, 0, c->stream);
+  c->launches++;
+  prof_mark(c, pf, 3);
+}
+
 // advance_one_step: cfl -> advance_flux (RK3 over rhs) -> advance_source_term
 static void step_once(janc_ctx *c, double cfl, double dt_fixed, int flags, Prof *pf) {
   const int par = c->parity;
@@ -700,17 +718,21 @@ static void step_once(janc_ctx *c, double cfl, double dt_fixed, int flags, Prof 
   c->launches++;
   prof_mark(c, pf, 0);
   do_ghost(c, c->A, pf);
+  const bool esrc = (flags & 2) && c->jit_src && c->ns > 1 && c->nr > 0;   // source inside every stage
   do_flux(c, c->A, c->A, c->B, SLOT(par, 0, 0, 0), 1.0, pf);
+  if (esrc) do_src(c, c->A, c->B, 1.0, pf);
   // stage 1
   do_prim(c, c->B, 1, SLOT(par, 1, 0, 0), nullptr, pf);
   do_ghost(c, c->B, pf);
   do_flux(c, c->B, c->A, c->C, SLOT(par, 1, 0, 0), 0.25, pf);
+  if (esrc) do_src(c, c->B, c->C, 0.25, pf);
   // stage 2 (writes U* over U^n in place: each cell reads its own U^n before writing)
   do_prim(c, c->C, 1, SLOT(par, 2, 0, 0), nullptr, pf);
   do_ghost(c, c->C, pf);
   do_flux(c, c->C, c->A, c->A, SLOT(par, 2, 0, 0), 2.0 / 3.0, pf);
+  if (esrc) do_src(c, c->C, c->A, 2.0 / 3.0, pf);
   // advance_source_term: T* inside the chemistry kernel; explicit variant: only refresh aux
-  const bool chem = !(flags & 1) && c->ns > 1 && c->nr > 0;
+  const bool chem = !(flags & 3) && c->ns > 1 && c->nr > 0;
   if (chem) do_chem(c, c->A, pf);
   else do_prim(c, c->A, 0, 0, nullptr, pf);
   if (c->g.n_levels > 1) {
@@ -780,6 +802,10 @@ extern "C" int janc_step(janc_ctx *c, int nsteps, double cfl, double dt_fixed, i
   int rc = check_ready(c);
   if (rc) return rc;
   if (nsteps < 0 || (!(cfl > 0.0) && !(dt_fixed > 0.0))) { c->err = "need cfl > 0 or dt_fixed > 0"; return JANC_EINVAL; }
+  if ((flags & 2) && c->ns > 1 && c->nr > 0 && !c->jit_src) {
+    c->err = "explicit source variant needs the run-time specialised kernel (NVRTC): " + c->jit_log;
+    return JANC_ESTATE;
+  }
   CK(cudaSetDevice(c->device));
   rc = upload_mech(c);
   if (rc) return rc;

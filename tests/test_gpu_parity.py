@@ -365,7 +365,7 @@ def test_graph_replay_is_bitwise_the_eager_path(B, monkeypatch):
             s = B.Solver(case.grid, case.mech, case.blocks)
             s.set_state(case.U, case.T)
             t = s.step(3, cfl=case.cfl) + s.step(1, cfl=case.cfl) + s.step(4, cfl=0.5 * case.cfl)
-            t += s.step(2, cfl=case.cfl, chem=False) + s.step(3, cfl=case.cfl)
+            t += s.step(2, cfl=case.cfl, chem=False) + s.step(3, cfl=case.cfl) + s.step(2, cfl=case.cfl, chem="explicit")
             U, T = s.get_state()
             assert s.status == 0
             out.append((t, U, T, s.launch_count()))
@@ -373,3 +373,39 @@ def test_graph_replay_is_bitwise_the_eager_path(B, monkeypatch):
         assert out[0][0] == out[1][0]
         assert np.array_equal(out[0][1], out[1][1]) and np.array_equal(out[0][2], out[1][2])
         assert out[0][3] == out[1][3] > 0
+
+
+# ------------------------------------------------------------------ explicit source variant
+def test_explicit_source_variant_parity(B, ref):
+    """the mechanism's source W_k omega_k inside every RK stage, no point-implicit
+    step.  Same parity bar against the oracle's explicit variant in 1-D, 2-D, block-list and 3-D / 20-species form."""
+    check(B, ref, I.config0(n=130), 5, TOL100, chem="explicit")
+    c1 = I.config1(nx=96, ny=40)
+    check(B, ref, c1, 1, TOL1, chem="explicit")
+    check(B, ref, c1, 20, TOL100, chem="explicit")
+    check(B, ref, I.config3(pcols=8, prows=4, npc=16), 2, TOL1 * 10, chem="explicit")
+    check(B, ref, I.config4(n=16, nspheres=2, radius=3), 1, TOL1, chem="explicit")
+
+
+def test_explicit_source_is_the_rk3_polynomial_on_gpu(B):
+    """Property of the CUDA path on its own: first-order reaction at constant k in a uniform gas at rest ->
+    y (1 - z + z^2/2 - z^3/6)^n, z = k dt (the SSP-RK3 stage recursion on y' = -k y)."""
+    W = np.array([0.029, 0.029]); nasa = np.zeros((2, 7)); nasa[:, 0] = 3.5
+    k = 4.0e6
+    m = I.Mechanism(2, 1, W, nasa, np.array([[1, 0]], dtype=np.int32), np.array([[0, 1]], dtype=np.int32),
+                    np.array([k]), np.array([0.0]), np.array([0.0]), np.array([0], dtype=np.int32),
+                    np.array([0], dtype=np.int32), np.ones((1, 2)))
+    n, dt, nsteps = 37, 1.0e-7, 3
+    z = np.zeros(n)
+    U = I.prim_to_cons(m, 1, z + 2.0e5, z + 900.0, np.tile([0.7, 0.3], (n, 1)), [z])
+    g = I.Grid(1, (n, 1, 1), (1e-3, 1, 1), (I.BC_PERIODIC, 0, 0), (I.BC_PERIODIC, 0, 0))
+    s = B.Solver(g, m)
+    s.set_state(U.reshape(1, -1, 1, 1, n), (z + 900.0).reshape(1, 1, 1, n))
+    s.step(nsteps, dt=dt, chem="explicit")
+    Ug, Tg = s.get_state()
+    assert s.status == 0
+    s.close()
+    zz = k * dt
+    amp = (1.0 - zz + zz * zz / 2.0 - zz ** 3 / 6.0) ** nsteps
+    assert np.abs(Ug[0, 3, 0, 0] - U[3] * amp).max() <= 4e-15 * U[3].max()
+    assert np.array_equal(Ug[0, 0, 0, 0], U[0]) and np.abs(Tg - 900.0).max() <= 1e-9
