@@ -46,7 +46,8 @@ struct janc_ctx {
   int jit_chem_nt, jit_chem_cells, jit_chem_mode;   // threads per CTA, cells per CTA, see jit_chem_mode()
   size_t jit_chem_smem;
   cudaKernel_t jit_prim;     // mechanism-specialised cons->prim kernel, null if not in use
-  cudaKernel_t jit_src = nullptr;   // explicit-variant source kernel (chemgen::generate_source), null without NVRTC
+  cudaKernel_t jit_src = nullptr;   // explicit-variant source kernel (chemgen::generate_source), compiled on first use
+  bool jit_src_tried = false;
   cudaKernel_t jit_kernel;   // mechanism-specialised chemistry kernel (chemgen.h), null if not in use
   std::string jit_log;
   unsigned long long id;
@@ -307,6 +308,7 @@ static void jit_setup(janc_ctx *c) {
   c->jit_kernel = nullptr;
   c->jit_prim = nullptr;
   c->jit_src = nullptr;
+  c->jit_src_tried = false;
   c->jit_log.clear();
   const MechC &M = c->mech;
   const char *off = getenv("JANC_DISABLE_JIT");
@@ -320,13 +322,11 @@ static void jit_setup(janc_ctx *c) {
   std::string src = chemgen::generate_prim(M, c->g.ndim);
   if (mode == 3) src += chemgen::generate_roles(M, c->g.ndim);
   else if (chem) src += chemgen::generate(M, c->g.ndim, mode == 2);
-  const bool have_src = M.ns >= 2 && M.nr >= 1;
-  if (have_src) src += chemgen::generate_source(M, c->g.ndim, !chem);
   else c->jit_log = "chemistry: mechanism outside the specialised range; ";
   static std::map<std::string, JitKernels> cache;          // per process; one device per process
   const std::string key = std::to_string(c->device) + "\n" + src;
   auto it = cache.find(key);
-  if (it != cache.end()) { c->jit_kernel = it->second.chem; c->jit_prim = it->second.prim; c->jit_src = it->second.src; return; }
+  if (it != cache.end()) { c->jit_kernel = it->second.chem; c->jit_prim = it->second.prim; return; }
   std::vector<char> cubin;
   std::string log;
   if (!jit_compile(src, cubin, log)) { c->jit_log += log; return; }
@@ -336,14 +336,38 @@ static void jit_setup(janc_ctx *c) {
   JitKernels k;
   e = cudaLibraryGetKernel(&k.prim, lib, "k_prim_jit");
   if (e == cudaSuccess && chem) e = cudaLibraryGetKernel(&k.chem, lib, "k_chem_jit");
-  if (e == cudaSuccess && have_src) e = cudaLibraryGetKernel(&k.src, lib, "k_src_jit");
   if (e == cudaSuccess && c->jit_chem_smem > 48 * 1024)
     e = cudaKernelSetAttributeForDevice(k.chem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->jit_chem_smem, c->device);
   if (e != cudaSuccess) { c->jit_log += std::string("cudaLibraryGetKernel: ") + cudaGetErrorString(e); cudaGetLastError(); return; }
   cache[key] = k;
   c->jit_kernel = k.chem;
   c->jit_prim = k.prim;
-  c->jit_src = k.src;
+}
+
+// The explicit-variant source kernel is compiled on first use (janc_step with flags bit 1): a 100-reaction mechanism
+// costs ~5 s of NVRTC time that the default path should not pay.
+static void jit_setup_source(janc_ctx *c) {
+  if (c->jit_src || c->jit_src_tried) return;
+  c->jit_src_tried = true;
+  const MechC &M = c->mech;
+  const char *off = getenv("JANC_DISABLE_JIT");
+  if (off && off[0] && off[0] != '0') { c->jit_log += " source kernel: disabled by JANC_DISABLE_JIT"; return; }
+  if (M.ns < 2 || M.nr < 1) return;
+  const std::string src = chemgen::generate_source(M, c->g.ndim, true);
+  static std::map<std::string, cudaKernel_t> cache;
+  const std::string key = std::to_string(c->device) + "\n" + src;
+  auto it = cache.find(key);
+  if (it != cache.end()) { c->jit_src = it->second; return; }
+  std::vector<char> cubin;
+  std::string log;
+  if (!jit_compile(src, cubin, log)) { c->jit_log += log; return; }
+  cudaLibrary_t lib;
+  cudaKernel_t k = nullptr;
+  cudaError_t e = cudaLibraryLoadData(&lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+  if (e == cudaSuccess) e = cudaLibraryGetKernel(&k, lib, "k_src_jit");
+  if (e != cudaSuccess) { c->jit_log += std::string("source kernel: ") + cudaGetErrorString(e); cudaGetLastError(); return; }
+  cache[key] = k;
+  c->jit_src = k;
 }
 
 extern "C" const char *janc_chem_kernel(const janc_ctx *c) {
@@ -363,7 +387,7 @@ extern "C" int janc_jit_probe(const janc_mech *m, int ndim, char *src_out, size_
   std::string src = chemgen::generate_prim(M, ndim);
   if (jit_chem_mode(M) == 3) src += chemgen::generate_roles(M, ndim);
   else if (jit_chem_mode(M)) src += chemgen::generate(M, ndim, jit_chem_mode(M) == 2);
-  if (M.ns >= 2 && M.nr >= 1) src += chemgen::generate_source(M, ndim, jit_chem_mode(M) == 0);
+  if (M.ns >= 2 && M.nr >= 1) src += chemgen::generate_source(M, ndim, jit_chem_mode(M) == 0);   // same translation unit here: helpers once
   if (src_len) *src_len = src.size();
   if (src_out && cap > 0) { size_t n = src.size() < cap - 1 ? src.size() : cap - 1; memcpy(src_out, src.data(), n); src_out[n] = 0; }
   if (cubin_bytes) {
@@ -802,6 +826,7 @@ extern "C" int janc_step(janc_ctx *c, int nsteps, double cfl, double dt_fixed, i
   int rc = check_ready(c);
   if (rc) return rc;
   if (nsteps < 0 || (!(cfl > 0.0) && !(dt_fixed > 0.0))) { c->err = "need cfl > 0 or dt_fixed > 0"; return JANC_EINVAL; }
+  if ((flags & 2) && c->ns > 1 && c->nr > 0) jit_setup_source(c);
   if ((flags & 2) && c->ns > 1 && c->nr > 0 && !c->jit_src) {
     c->err = "explicit source variant needs the run-time specialised kernel (NVRTC): " + c->jit_log;
     return JANC_ESTATE;
