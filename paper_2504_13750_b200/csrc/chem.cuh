@@ -180,7 +180,7 @@ template <int NS, int NT>
 __global__ void __launch_bounds__(NT) k_chem_reg(Params P, double *__restrict__ U) {
   constexpr int N1 = NS - 1;
   extern __shared__ double sm[];
-  const int nr = c_mech.nr, ntb = c_mech.ntb;
+  const int nr = c_mech.nr;
   double *sX = sm + threadIdx.x;                  // [NS]
   double *scf = sX + NS * NT;                     // [nr]  M k_f
   double *scb = scf + nr * NT;                    // [nr]  -M k_b

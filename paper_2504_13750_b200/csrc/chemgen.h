@@ -198,8 +198,6 @@ inline void emit_big_solve(Emitter &E, const MechC &M, int ndim, const Acc &accW
 //               specialised (literal addresses), the dense elimination is a loop over shared memory.
 inline std::string generate(const MechC &M, int ndim, bool big = false) {
   const int NT = big ? JANC_JIT_NT_BIG : JANC_JIT_NT;
-  const char *mb_ = getenv("JANC_JIT_MINB");            // experiment knob: min CTAs per SM
-  const std::string MINB_STR = mb_ && mb_[0] ? std::string(", ") + mb_ : std::string("");
   const int ns = M.ns, nr = M.nr, n1 = ns - 1, nvar = ndim + 2 + n1;
   Emitter E;
   std::string &src = E.s;
@@ -207,7 +205,7 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
   src += "struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2;"
          " long long st0, st1, st2, pc; int np; };\n";
   emit_math(src);
-  src += "extern \"C\" __global__ void __launch_bounds__(" + I(NT) + MINB_STR + ") k_chem_jit(ChemArgs a) {\n";
+  src += "extern \"C\" __global__ void __launch_bounds__(" + I(NT) + ") k_chem_jit(ChemArgs a) {\n";
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
   if (big) {
     E.line("extern __shared__ double sm_[];");

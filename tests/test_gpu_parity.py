@@ -239,6 +239,75 @@ def test_cfg3_full_size_one_step(B, ref):
     print("cfg3 full-size per-field rel err", e)
 
 
+def test_cfg1_full_size_100_steps(B, ref):
+    """BASELINE config[1] exactly: 1024 x 128, 9 species / 21 reactions, 100 steps, <= 1e-6 per field."""
+    case = I.config1()
+    assert case.grid.n[0] == 1024 and case.grid.n[1] == 128
+    e = check(B, ref, case, 100, TOL100)
+    print("cfg1 full-size 100-step per-field rel err", e)
+
+
+def test_cfg4_full_size_conservation_and_sampled_chemistry(B, ref, mech20):
+    """Config 4 at full size (256^3, 20 species / 100 reactions, periodic) in the launch configuration bench.py
+    times.  The oracle cannot finish 16.7 M cells in seconds, so:
+    (a) properties that hold at any size: total mass, momentum, energy and every element are conserved to round-off
+        on the periodic box, and no error flag is raised;
+    (b) sampled outputs the oracle can compute one by one: the step is run twice from the same state, once without
+        the chemistry (U*) and once with it; the flow part is the same kernels on the same inputs, so the difference
+        is the role-warp kernel's increment, which is recomputed for 64 sampled cells (48 inside the hot spheres)
+        from U* with the oracle's cons2prim + chem_cell."""
+    case = I.config4()
+    assert case.cells == 256 ** 3
+    s = B.Solver(case.grid, case.mech, case.blocks)
+    assert s.chem_kernel() == "jit-roles"
+    s.set_state(case.U, case.T)
+    s.step(1, cfl=case.cfl, chem=False)                       # RK3 only: U*
+    Ustar, Tstar = s.get_state()
+    assert s.status == 0
+    s.set_state(case.U, case.T)
+    dt = s.step(1, cfl=case.cfl)                              # RK3 + point-implicit
+    U1, T1 = s.get_state()
+    assert s.status == 0
+    s.close()
+    # (a) conservation on the periodic box
+    for v in range(5):
+        a, b = case.U[0, v].sum(dtype=np.float64), U1[0, v].sum(dtype=np.float64)
+        scale = np.abs(case.U[0, v]).sum(dtype=np.float64) if v not in (1, 2, 3) else case.U[0, 0].sum() * 300.0
+        assert abs(a - b) <= 1e-11 * scale, (v, a, b)
+    el = np.asarray(mech20.elements, dtype=float)
+    def moles(Us):
+        ry = [Us[0, 5 + k].sum(dtype=np.float64) for k in range(19)]
+        ry.append(Us[0, 0].sum(dtype=np.float64) - sum(ry))
+        return (np.array(ry) / mech20.W) @ el
+    m0, m1 = moles(case.U), moles(U1)
+    assert np.abs(m1 - m0).max() <= 1e-11 * np.abs(m0).max()
+    # (b) sampled cells: hot-sphere cells (chemistry active) and ambient ones; the flow part is identical in both
+    # runs (same kernels, same inputs), so U1 - U* is the chemistry increment of the role-warp kernel
+    assert np.array_equal(U1[0, :5], Ustar[0, :5])
+    hot = np.argwhere(case.T[0] > 2000.0)
+    rng = np.random.default_rng(4)
+    pick = [tuple(hot[i]) for i in rng.choice(len(hot), 48, replace=False)] + [tuple(rng.integers(0, 256, 3)) for _ in range(16)]
+    worst = worst_d = 0.0
+    active = 0
+    for (k, j, i) in pick:
+        rho = Ustar[0, 0, k, j, i]
+        ry = Ustar[0, 5:, k, j, i].copy()
+        Uc = Ustar[0, :, k, j, i].copy()
+        rc, out = ref.cons2prim(mech20, 3, Uc, case.T[0, k, j, i])
+        assert rc == 0
+        rc, d = ref.chem_cell(mech20, out[0], rho, ry, dt)
+        assert rc == 0
+        got = U1[0, 5:, k, j, i] - ry
+        worst = max(worst, np.abs(got - d).max() / max(np.abs(ry).max(), 1e-6 * rho))
+        if np.abs(d).max() > 1e-9 * np.abs(ry).max():          # chemistry is doing something here: compare the increment itself
+            active += 1
+            worst_d = max(worst_d, np.abs(got - d).max() / np.abs(d).max())
+        assert abs(T1[0, k, j, i] - out[0]) <= 1e-10 * out[0]
+    assert worst <= 1e-10, worst
+    assert active >= 40 and worst_d <= 1e-6, (active, worst_d)
+    print("cfg4 full-size sampled chemistry: state rel err", worst, "increment rel err", worst_d, "active cells", active)
+
+
 # ------------------------------------------------------------------ chemistry kernel selection
 def test_specialised_chemistry_kernel_is_the_one_running(B, mech9, mech20):
     """janc_set_mechanism compiles the mechanism-specialised kernel (chemgen.h) for <= 12 unknowns;
