@@ -29,10 +29,17 @@
 
 #include "chemgen.h"
 
-#define JANC_ROLES 8
-#define JANC_ROLES_MAXSLOT 3      // columns per role held in registers => Ns <= 24
+#define JANC_ROLES_MAXCOLS 24      // columns of [I - dt J | rhs] incl. the temporary N column => Ns <= 24
 
 namespace chemgen {
+
+// roles (warps) per CTA: 8 roles x 3 column slots (255 registers; the default) or 16 roles x 2 slots (128 registers).
+// Measured on cfg 4: 59 ms with 8 roles, 81 ms with 16 -- the per-column publish -> consume chain, not the number of
+// resident warps, bounds the elimination, and it is longer with 16 participants.
+inline int roles_nr() {
+  const char *e = getenv("JANC_ROLES_N");              // test knob
+  return e && atoi(e) == 16 ? 16 : 8;
+}
 
 struct RolesLayout {
   int oX, oP, oN, oRN, oDL, oRHS, oF, oPIV, oIP, oXS, oNX, oR, rows;   // offsets in rows of 32 doubles
@@ -43,7 +50,7 @@ struct RolesLayout {
 // sizes that depend on the mechanism only: polynomial degrees, reaction orders, table lengths
 struct RolesDims { int degh, degc, nkb, maxof, maxob, nslot; };
 inline RolesDims roles_dims(const MechC &M) {
-  RolesDims D{1, 0, 3, 1, 1, (M.nr + JANC_ROLES - 1) / JANC_ROLES};
+  RolesDims D{1, 0, 3, 1, 1, (M.nr + roles_nr() - 1) / roles_nr()};
   for (int k = 0; k < M.ns; k++)
     for (int q = 1; q <= 4; q++)
       if (M.nasa[k][q] != 0.0) { D.degh = std::max(D.degh, q + 1); D.degc = std::max(D.degc, q); }
@@ -60,11 +67,11 @@ inline size_t roles_table_doubles(const MechC &M) {
 }
 inline size_t roles_table_ints(const MechC &M) {
   const RolesDims D = roles_dims(M);
-  return (size_t)JANC_ROLES * D.nslot + M.nr + (size_t)M.nr * D.maxof + (size_t)M.nr * D.maxob;
+  return (size_t)roles_nr() * D.nslot + M.nr + (size_t)M.nr * D.maxof + (size_t)M.nr * D.maxob;
 }
 
 inline bool roles_applicable(const MechC &M) {
-  return M.ns >= 3 && M.ns <= JANC_ROLES * JANC_ROLES_MAXSLOT && M.nr >= 1;
+  return M.ns >= 3 && M.ns <= JANC_ROLES_MAXCOLS && M.nr >= 1;
 }
 
 inline RolesLayout roles_layout(const MechC &M, int ndim) {
@@ -72,8 +79,8 @@ inline RolesLayout roles_layout(const MechC &M, int ndim) {
   RolesLayout L;
   int o = 0;
   L.oX = o; o += ns + 1;                     // X_k, plus a dummy species with X = 1
-  L.oP = o; o += 16;                         // partial sums of rho Y_k and Y_k per role
-  L.oN = o; o += 16;                         // Newton partial sums per role
+  L.oP = o; o += 2 * roles_nr();             // partial sums of rho Y_k and Y_k per role
+  L.oN = o; o += 2 * roles_nr();             // Newton partial sums per role
   L.oRN = o; o += M.ntb > 0 ? M.ntb : 1;     // net rate without the third-body factor (third-body reactions)
   L.oDL = o; o += n1;                        // D_kN / W_N
   L.oRHS = o; o += n1;                       // dt W_k wdot_k
@@ -92,7 +99,7 @@ inline RolesLayout roles_layout(const MechC &M, int ndim) {
 }
 
 inline std::string generate_roles(const MechC &M, int ndim) {
-  const int ns = M.ns, nr = M.nr, n1 = ns - 1, nvar = ndim + 2 + n1, NR = JANC_ROLES;
+  const int ns = M.ns, nr = M.nr, n1 = ns - 1, nvar = ndim + 2 + n1, NR = roles_nr();
   const int NSL = (ns + NR - 1) / NR;                  // column slots per role (columns 0..n1)
   const int wN = n1 % NR, sN = n1 / NR;                // role / slot of column N (later the right-hand side)
   const RolesLayout L = roles_layout(M, ndim);
@@ -246,13 +253,13 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     E.line("pr_ += ry" + ss + "; py_ += Y" + ss + ";");
     E.line("if (k" + ss + " < " + I(n1) + ") SM(" + I(L.oX) + " + k" + ss + ") = ry" + ss + " * c_iW[k" + ss + "];");
   }
-  E.line("SM(" + I(L.oP) + " + w) = pr_; SM(" + I(L.oP + 8) + " + w) = py_;");
+  E.line("SM(" + I(L.oP) + " + w) = pr_; SM(" + I(L.oP + NR) + " + w) = py_;");
   E.line("if (w == 0) SM(" + I(L.oX + ns) + ") = 1.0;");
   E.line("BAR();");
   E.line("if (bt + gridDim.x < nbt) prefetch_turn(a, sm_, bt + gridDim.x, nbp, ncell);   // lands during this turn");
   E.line("{ double rsum = 0.0, ysum = 0.0;");
   E.line("  #pragma unroll");
-  E.line("  for (int q = 0; q < 8; q++) { rsum += SM(" + I(L.oP) + " + q); ysum += SM(" + I(L.oP + 8) + " + q); }");
+  E.line("  for (int q = 0; q < " + I(NR) + "; q++) { rsum += SM(" + I(L.oP) + " + q); ysum += SM(" + I(L.oP + NR) + " + q); }");
   E.line("  if (w == " + I(wN) + ") { ry" + I(sN) + " = rho - rsum; Y" + I(sN) + " = 1.0 - ysum; SM(" + I(L.oX + n1) + ") = ry" + I(sN) + " * " + num(M.invW[n1]) + "; } }");
   for (int s = 0; s < NSL; s++)
     E.line("const double yr" + I(s) + " = k" + I(s) + " < " + I(ns) + " ? Y" + I(s) + " * c_Rk[k" + I(s) + " < " + I(ns) + " ? k" + I(s) + " : 0] : 0.0;");
@@ -269,11 +276,11 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     E.line("  if (" + ks + " < " + I(ns) + ") { const double *h_ = c_hc + " + ks + " * " + I(degh + 1) + ", *c_ = c_cc + " + ks + " * " + I(degc + 1) + ";");
     E.line("    f = fma(yr" + I(s) + ", " + h + ", f); cv = fma(yr" + I(s) + ", " + c + ", cv); }");
   }
-  E.line("  SM(" + I(L.oN) + " + w) = f; SM(" + I(L.oN + 8) + " + w) = cv;");
+  E.line("  SM(" + I(L.oN) + " + w) = f; SM(" + I(L.oN + NR) + " + w) = cv;");
   E.line("  BAR();");
   E.line("  f = -e; cv = 0.0;");
   E.line("  #pragma unroll");
-  E.line("  for (int q = 0; q < 8; q++) { f += SM(" + I(L.oN) + " + q); cv += SM(" + I(L.oN + 8) + " + q); }");
+  E.line("  for (int q = 0; q < " + I(NR) + "; q++) { f += SM(" + I(L.oN) + " + q); cv += SM(" + I(L.oN + NR) + " + q); }");
   E.line("  const double dT = -f / cv;");
   E.line("  if (!conv) { T += dT; if (fabs(dT) <= 1e-11 * fabs(T)) conv = true; }");
   E.line("  if (__syncthreads_and(conv)) break;");
@@ -460,12 +467,12 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("}");
   E.line("#pragma unroll 1");
   E.line("for (int c = 0; c < " + I(n1) + "; c++) {");
-  E.line("  const int sc = c >> 3, oc = c & 7;");
+  E.line("  const int sc = c / " + I(NR) + ", oc = c % " + I(NR) + ";");
   E.line("  if (w != oc) AWAIT(1 + c % 15);     // column c published by its owner (producer / consumer barrier)");
   E.line("  const int fl_ = s_flag[c * 64 + lane];");
   for (int p = 1; p < n1; p++) E.line("  const double f" + I(p) + " = SM(" + I(L.oF) + " + c * " + I(n1) + " + " + I(p) + ");");
   E.line("  if (__any_sync(0xffffffffu, fl_ != 0)) { c0 = c; break; }");
-  E.line("  const int cn = c + 1, ocn = cn & 7, scn = cn >> 3;");
+  E.line("  const int cn = c + 1, ocn = cn % " + I(NR) + ", scn = cn / " + I(NR) + ";");
   E.line("  const bool la = cn < " + I(n1) + " && w == ocn;     // this role owns the next column: update it first, publish");
   E.line("  if (la) {");
   for (int s = 0; s < NSL; s++) {

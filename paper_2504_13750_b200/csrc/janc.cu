@@ -316,7 +316,7 @@ static void jit_setup(janc_ctx *c) {
   const int mode = jit_chem_mode(M);
   const bool chem = mode != 0;
   c->jit_chem_mode = mode;
-  c->jit_chem_nt = mode == 3 ? JANC_ROLES * 32 : mode == 2 ? JANC_JIT_NT_BIG : JANC_JIT_NT;
+  c->jit_chem_nt = mode == 3 ? chemgen::roles_nr() * 32 : mode == 2 ? JANC_JIT_NT_BIG : JANC_JIT_NT;
   c->jit_chem_cells = mode == 3 ? 32 : c->jit_chem_nt;
   c->jit_chem_smem = mode == 3 ? chemgen::roles_layout(M, c->g.ndim).smem() : mode == 2 ? (size_t)(M.ns - 1) * M.ns * JANC_JIT_NT_BIG * sizeof(double) : 0;
   std::string src = chemgen::generate_prim(M, c->g.ndim);

@@ -359,6 +359,11 @@ def test_role_warp_chemistry_kernel(B, ref, mech9, mech20, monkeypatch):
     Ug, Tg, Ur, Tr = both(B, ref, case9, 1, cfl=0.0, dt=2e-7)
     assert field_errors(case9, Ug, Ur).max() <= 1e-8
     monkeypatch.delenv("JANC_JIT_MAX_N1")
+    monkeypatch.setenv("JANC_ROLES_N", "16")                  # 16 roles x 2 column slots: same generator, other split
+    Ug, Tg, Ur, Tr = both(B, ref, case, 1, cfl=0.0, dt=1e-7)
+    assert field_errors(case, Ug, Ur).max() <= 1e-8
+    check(B, ref, I.config4(n=16, nspheres=2, radius=3), 1, TOL1)
+    monkeypatch.delenv("JANC_ROLES_N")
     monkeypatch.setenv("JANC_JIT_BIG", "smem")
     c4 = I.config4(n=16, nspheres=2, radius=3)
     s = B.Solver(c4.grid, c4.mech)
