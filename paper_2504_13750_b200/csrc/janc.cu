@@ -680,7 +680,7 @@ static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uou
     if (gather_mode(c)) launch_flux2<16, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches: halo gathered in-kernel; 2 warps per patch
     else if ((long long)c->np * c->ncell < 600000) launch_flux2<32, 16, 4>(c, Uk, U0, Uout, slot_base, coef);   // small grids: 4x the CTAs
     else launch_flux2<64, 16, 8>(c, Uk, U0, Uout, slot_base, coef);
-  } else launch_flux<3, 32, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);
+  } else launch_flux<3, 16, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);   // 128 threads, 39 KB: 4 independent CTAs per SM overlap stage / walk
   c->launches++;
   prof_mark(c, pf, 2);
 }
