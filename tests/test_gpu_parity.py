@@ -483,3 +483,19 @@ def test_explicit_source_is_the_rk3_polynomial_on_gpu(B):
     amp = (1.0 - zz + zz * zz / 2.0 - zz ** 3 / 6.0) ** nsteps
     assert np.abs(Ug[0, 3, 0, 0] - U[3] * amp).max() <= 4e-15 * U[3].max()
     assert np.array_equal(Ug[0, 0, 0, 0], U[0]) and np.abs(Tg - 900.0).max() <= 1e-9
+
+
+def test_explicit_source_without_nvrtc_fails_loudly(B, monkeypatch):
+    """No silent fallback: with the run-time specialised kernels switched off the explicit-source variant is
+    refused (JANC_ESTATE with a message), while the point-implicit and no-chemistry variants still run."""
+    monkeypatch.setenv("JANC_DISABLE_JIT", "1")
+    case = I.config1(nx=32, ny=16)
+    s = B.Solver(case.grid, case.mech)
+    s.set_state(case.U, case.T)
+    with pytest.raises(B.JancError) as e:
+        s.step(1, cfl=case.cfl, chem="explicit")
+    assert "explicit source variant" in str(e.value)
+    s.step(1, cfl=case.cfl)
+    s.step(1, cfl=case.cfl, chem=False)
+    assert s.status == 0
+    s.close()
