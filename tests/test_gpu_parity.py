@@ -499,3 +499,18 @@ def test_explicit_source_without_nvrtc_fails_loudly(B, monkeypatch):
     s.step(1, cfl=case.cfl, chem=False)
     assert s.status == 0
     s.close()
+
+
+def test_degenerate_mechanisms(B, ref, mech9):
+    """Degenerate cases of the method: a mixture with NO reactions (nr = 0: the chemistry step is the identity, the
+    specialised cons->prim kernel still runs), explicit-source mode on it (nothing to add), and the thinnest grid the 3-layer mirror admits (3 rows)."""
+    m0 = I.Mechanism(9, 0, mech9.W, mech9.nasa, np.zeros((0, 9), dtype=np.int32), np.zeros((0, 9), dtype=np.int32),
+                     np.zeros(0), np.zeros(0), np.zeros(0), np.zeros(0, dtype=np.int32), np.zeros(0, dtype=np.int32),
+                     np.zeros((0, 9)))
+    base = I.config1(nx=48, ny=24)
+    case = I.Case("inert9", base.grid, m0, base.U, base.T, base.cfl, 2)
+    check(B, ref, case, 2, TOL1 * 10)
+    check(B, ref, case, 2, TOL1 * 10, chem="explicit")
+    g3 = I.Grid(2, (40, 3, 1), base.grid.dx, base.grid.bc_lo, base.grid.bc_hi)     # three rows of cells in y
+    thin = I.Case("three_rows", g3, mech9, base.U[:, :, :, :3, :40].copy(), base.T[:, :, :3, :40].copy(), base.cfl, 2)
+    check(B, ref, thin, 2, TOL1 * 10)
