@@ -137,6 +137,10 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
       if (dxf < dxmin) dxmin = dxf;
       P.bc_lo[d] = grid->bc_lo[d]; P.bc_hi[d] = grid->bc_hi[d];
       if (P.bc_lo[d] < 0 || P.bc_lo[d] > 2 || P.bc_hi[d] < 0 || P.bc_hi[d] > 2) { delete c; return JANC_EINVAL; }
+      // 3 ghost layers are copied from 3 distinct interior cells by the periodic / mirror / neighbour rules;
+      // only zero-gradient sides work on thinner grids (e.g. the one-cell 0-D reactor)
+      const bool thin_ok = grid->n_patches <= 0 && P.bc_lo[d] == 2 && P.bc_hi[d] == 2;
+      if (grid->n[d] < JANC_NG && !thin_ok) { delete c; return JANC_EINVAL; }
     } else {
       c->g.n[d] = 1; P.n[d] = 1; P.G[d] = 0; P.P[d] = 1; P.invdx[0][d] = P.invdx[1][d] = 0.0;
     }

@@ -221,6 +221,12 @@ def test_error_flag_and_arguments(B):
     s.step(1, cfl=0.4)
     assert s.status == 0
     s.close()
+    # fewer cells than ghost layers along a mirrored / periodic direction: refused at creation (janc.h)
+    m = I.config1(nx=32, ny=16).mech
+    for bc in (I.BC_REFLECT, I.BC_PERIODIC):
+        with pytest.raises(B.JancError):
+            B.Solver(I.Grid(2, (40, 2, 1), (1e-4, 1e-4, 1), (I.BC_OUTFLOW, bc, 0), (I.BC_OUTFLOW, bc, 0)), m)
+    B.Solver(I.Grid(2, (40, 2, 1), (1e-4, 1e-4, 1), (I.BC_OUTFLOW, I.BC_OUTFLOW, 0), (I.BC_OUTFLOW, I.BC_OUTFLOW, 0)), m).close()
 
 
 # ------------------------------------------------------------------ full-size bench workload (config 2)
