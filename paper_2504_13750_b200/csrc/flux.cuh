@@ -270,8 +270,9 @@ __device__ __forceinline__ void ghost_source2d(const Params &P, int patch, int i
   }
 }
 
-// GATHER: the tile is a whole patch (n <= TX, TY) and the halo of the box is fetched straight from the cells
-// the ghost rule points at -- the ghost layers are never written to HBM and k_ghost is not launched.
+// GATHER: the halo of the box is fetched straight from the cells the ghost rule points at -- the ghost layers are
+// never written to HBM and k_ghost is not launched (AMR patches of <= 16 x 16, one tile per patch; small uniform
+// grids, where three extra launches per step are a tenth of the step).
 template <int TX, int TY, int SEG, bool GATHER = false>
 struct Flux2Cfg {
   static constexpr int NT = TX * TY / SEG;
@@ -313,7 +314,8 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
   if (GATHER) {
     for (int it = tid; it < C::BX * C::BY; it += NT) {
       int q, ci, cj, fl;
-      ghost_source2d(P, patch, it % C::BX - 3, it / C::BX - 3, q, ci, cj, fl);
+      // patch coordinates of this box cell (ragged tiles stay within the 3 ghost layers)
+      ghost_source2d(P, patch, min(o0 + it % C::BX - 3, P.n[0] + 2), min(o1 + it / C::BX - 3, P.n[1] + 2), q, ci, cj, fl);
       sq[it] = q;
       sc[it] = (int)cell_index(P, ci, cj, 0);
       sfl[it] = (unsigned char)fl;

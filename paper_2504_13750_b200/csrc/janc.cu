@@ -630,8 +630,12 @@ static void do_prim(janc_ctx *c, const double *U, int reduce, int slot_base, dou
   prof_mark(c, pf, 0);
 }
 
-// 2-D patches of at most 16 x 16 cells: the flux kernel gathers its halo itself (flux.cuh, GATHER); no ghost fill
-static bool gather_mode(const janc_ctx *c) { return c->g.ndim == 2 && c->P.n[0] <= 16 && c->P.n[1] <= 16; }
+// 2-D patches of at most 16 x 16 cells, and small 2-D grids (launch-bound): the flux kernel gathers its halo itself
+// (flux.cuh, GATHER); no ghost fill
+static bool small_grid(const janc_ctx *c) { return (long long)c->np * c->ncell < 600000; }
+static bool gather_mode(const janc_ctx *c) {
+  return c->g.ndim == 2 && ((c->P.n[0] <= 16 && c->P.n[1] <= 16) || small_grid(c));
+}
 
 static void do_ghost(janc_ctx *c, double *U, Prof *pf) {
   if (gather_mode(c)) return;
@@ -681,8 +685,8 @@ static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uou
   const Params &P = c->P;
   if (c->g.ndim == 1) launch_flux<1, 128, 1, 1, 4>(c, Uk, U0, Uout, slot_base, coef);
   else if (c->g.ndim == 2) {
-    if (gather_mode(c)) launch_flux2<16, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches: halo gathered in-kernel; 2 warps per patch
-    else if ((long long)c->np * c->ncell < 600000) launch_flux2<32, 16, 4>(c, Uk, U0, Uout, slot_base, coef);   // small grids: 4x the CTAs
+    if (c->P.n[0] <= 16 && c->P.n[1] <= 16) launch_flux2<16, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches: halo gathered in-kernel; 2 warps per patch
+    else if (small_grid(c)) launch_flux2<32, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // small grids: 4x the CTAs, no ghost launches
     else launch_flux2<64, 16, 8>(c, Uk, U0, Uout, slot_base, coef);
   } else launch_flux<3, 16, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);   // 128 threads, 39 KB: 4 independent CTAs per SM overlap stage / walk
   c->launches++;

@@ -204,7 +204,7 @@ def test_device_resident_state_and_async(B, ref):
     U1, T1 = s.get_state(device=True)
     s2 = B.Solver(case.grid, case.mech); s2.set_state(case.U, case.T); s2.step(2, cfl=case.cfl); U2, _ = s2.get_state()
     assert np.array_equal(U1.cpu().numpy(), U2)
-    assert s.launch_count() > 20
+    assert s.launch_count() >= 16            # 2 steps x (3 prim + dt + 3 flux + chem); small 2-D grids gather their halo in the flux kernel
     s.close(); s2.close()
 
 
