@@ -27,15 +27,16 @@ METRIC = "fp64 cell-updates/sec (RK3 step incl. point-implicit chemistry)"
 UNIT = "cell-updates/s"
 
 # algorithmic work / traffic per cell-update, derived in DESIGN.md "Roofline arithmetic"
-WENO_OPS = 38            # DP instructions (FMA = 1) of one WENO5-JS reconstruction in difference form
-                         # (flux.cuh: differences 4 amortised, betas 9, squares 3, weights 6, candidates 4,
-                         #  numerator 3, denominator 2, reciprocal 5 + 1, final 1)
+WENO_OPS = 30            # DP instructions (FMA = 1) of one WENO5-JS reconstruction in difference form
+                         # (flux.cuh: differences 4 amortised, betas 6, squares 3, weights 5, candidates 3,
+                         #  numerator 3, denominator 2, reciprocal 3 + 1)
 
 
 def flux_ops_per_cell_stage(ndim, nvar):
-    # per component and direction: split flux 2f+- (3) + 2 reconstructions + face sum, difference, scale (3);
-    # RK update 3.  Pencil-end faces and ghost-row split fluxes (the kernel's redundancy) are NOT counted.
-    return nvar * (ndim * (3 + 2 * WENO_OPS + 3) + 3)
+    # per component and direction: split flux 2f+- (3) + 2 reconstructions + face value from the two (4) +
+    # difference, scale (2); RK update 3.  Pencil-end faces and ghost-row split fluxes (the kernel's redundancy)
+    # are NOT counted.
+    return nvar * (ndim * (3 + 2 * WENO_OPS + 4 + 2) + 3)
 
 
 def chem_ops_per_cell(mech):

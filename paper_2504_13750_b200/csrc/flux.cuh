@@ -21,35 +21,38 @@
 //   beta_2 = 13/12 (D3-D2)^2 + 1/4 (D3 - 3 D2)^2,
 //   q_0 = v_0 + (5 D1 - 2 D0)/6,  q_1 = v_0 + (D1 + 2 D2)/6,  q_2 = v_0 + (4 D2 - D3)/6
 // which is the Jiang-Shu formula of SURVEY 8(c) step 5 re-grouped (identical in exact arithmetic).
-// The kernel reconstructs 2f+- (not f+-): beta scales by 4, so eps -> 4 eps keeps the weights
-// bit-for-bit those of f+-; beta is further carried as 12 beta (eps -> 48 eps); the 1/2 is folded
-// into 1/dx.  a_k = d_k/(eps+beta_k)^2 is evaluated as d_k prod_{l!=k}(eps+beta_l)^2 over the common
-// denominator: one reciprocal per reconstruction.
+// The kernel reconstructs 2f+- (not f+-): beta scales by 4, so eps -> 4 eps keeps the weights those of f+-; beta is
+// further carried as 4 beta, i.e. B_k = 16 eps + 13/3 (D_{k+1}-D_k)^2 + t_k^2 with t_0 = 3 D1 - D0, t_1 = D1 + D2,
+// t_2 = D3 - 3 D2; the 1/2 is folded into 1/dx.  a_k = d_k/(eps+beta_k)^2 is evaluated as 10 d_k prod_{l!=k} B_l^2 over
+// the common denominator (one reciprocal per reconstruction), and the q_k numerators re-use t_k:
+//   5 D1 - 2 D0 = 2 t_0 - D1,   D1 + 2 D2 = t_1 + D2,   4 D2 - D3 = D2 - t_2.
+// One reconstruction is 32 fp64 instructions (4 for its share of the differences, 26 below, 2 of the face sum).
 #pragma once
 #include "common.cuh"
 
-#define JANC_WENO_EPS48 4.8e-5   // 48 * 1e-6, see above
+#define JANC_WENO_EPS16 1.6e-5   // 16 * 1e-6, see above
 
-// 1/x to full fp64 precision for normal, finite x > 0 (MUFU seed + 2 Newton steps, no slow path).
+// 1/x for normal, finite x > 0: MUFU seed (>= 20 bits) + one cubic step r (1 + e + e^2), e = 1 - x r  (error e^3 < 2^-60
+// before rounding; no slow path).
 __device__ __forceinline__ double rcp_pos(double x) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  r = fma(fma(-x, r, 1.0), r, r);
-  r = fma(fma(-x, r, 1.0), r, r);
-  return r;
+  const double e = fma(-x, r, 1.0);
+  return fma(fma(e, e, e), r, r);
 }
 
-// value at the face from centre value v and differences D0..D3; S_k = 48 eps + 13 (D_{k+1}-D_k)^2
-__device__ __forceinline__ double weno5_diff(double v, double D0, double D1, double D2, double D3,
-                                             double S0, double S1, double S2) {
+// 6 (q - v) = num / den of the reconstruction with differences D0..D3 about the centre value v, returned as num and
+// 1/den;  S_k = 16 eps + 13/3 (D_{k+1}-D_k)^2
+__device__ __forceinline__ void weno5_diff(double D0, double D1, double D2, double D3, double S0, double S1, double S2,
+                                           double &num, double &rden) {
   const double t0 = fma(3.0, D1, -D0), t1 = D1 + D2, t2 = fma(-3.0, D2, D3);
-  double b0 = fma(3.0 * t0, t0, S0), b1 = fma(3.0 * t1, t1, S1), b2 = fma(3.0 * t2, t2, S2);
+  double b0 = fma(t0, t0, S0), b1 = fma(t1, t1, S1), b2 = fma(t2, t2, S2);
   b0 *= b0; b1 *= b1; b2 *= b2;
-  const double a0 = 0.1 * (b1 * b2), a1 = 0.6 * (b0 * b2), a2 = 0.3 * (b0 * b1);
-  const double c0 = fma(5.0, D1, -2.0 * D0), c1 = fma(2.0, D2, D1), c2 = fma(4.0, D2, -D3);
-  const double num = fma(a0, c0, fma(a1, c1, a2 * c2));
-  const double den = (a0 + a1) + a2;
-  return fma(num * rcp_pos(den), 1.0 / 6.0, v);
+  const double h = 3.0 * b0;
+  const double a0 = b1 * b2, a1 = (h + h) * b2, a2 = h * b1;      // 10 x (0.1, 0.6, 0.3) x the other two B^2
+  const double c0 = fma(2.0, t0, -D1), c1 = t1 + D2, c2 = D2 - t2;
+  num = fma(a0, c0, fma(a1, c1, a2 * c2));
+  rden = rcp_pos((a0 + a1) + a2);
 }
 
 // Face fluxes of one pencil, streamed: ld(k, fp2, fm2) returns 2f+ and 2f- of pencil cell k-3
@@ -57,6 +60,7 @@ __device__ __forceinline__ double weno5_diff(double v, double D0, double D1, dou
 // Cell k is fetched just before the first face that needs it, so only a 6-cell window is live.
 template <int SEG, class Load>
 __device__ __forceinline__ void weno_faces(Load &&ld, double (&Fh)[SEG + 1]) {
+  constexpr double K = 13.0 / 3.0;
   double P[SEG + 6], M[SEG + 6], dP[SEG + 5], dM[SEG + 5], sP[SEG + 4], sM[SEG + 4];
 #pragma unroll
   for (int k = 0; k < 5; k++) ld(k, P[k], M[k]);
@@ -65,21 +69,22 @@ __device__ __forceinline__ void weno_faces(Load &&ld, double (&Fh)[SEG + 1]) {
 #pragma unroll
   for (int k = 0; k < 3; k++) {
     const double s = dP[k + 1] - dP[k], r = dM[k + 1] - dM[k];
-    sP[k] = fma(13.0 * s, s, JANC_WENO_EPS48);
-    sM[k] = fma(13.0 * r, r, JANC_WENO_EPS48);
+    sP[k] = fma(K * s, s, JANC_WENO_EPS16);
+    sM[k] = fma(K * r, r, JANC_WENO_EPS16);
   }
 #pragma unroll
   for (int q = 0; q <= SEG; q++) {
     ld(q + 5, P[q + 5], M[q + 5]);
     dP[q + 4] = P[q + 5] - P[q + 4]; dM[q + 4] = M[q + 5] - M[q + 4];
     const double s = dP[q + 4] - dP[q + 3], r = dM[q + 4] - dM[q + 3];
-    sP[q + 3] = fma(13.0 * s, s, JANC_WENO_EPS48);
-    sM[q + 3] = fma(13.0 * r, r, JANC_WENO_EPS48);
+    sP[q + 3] = fma(K * s, s, JANC_WENO_EPS16);
+    sM[q + 3] = fma(K * r, r, JANC_WENO_EPS16);
+    double np, rp, nm, rm;
     // plus part: stencil cells q-3..q+1 (array q..q+4), upwind centre = array q+2
-    const double fp = weno5_diff(P[q + 2], dP[q], dP[q + 1], dP[q + 2], dP[q + 3], sP[q], sP[q + 1], sP[q + 2]);
+    weno5_diff(dP[q], dP[q + 1], dP[q + 2], dP[q + 3], sP[q], sP[q + 1], sP[q + 2], np, rp);
     // minus part: mirror image, cells q+2..q-2 (array q+5..q+1), centre = array q+3
-    const double fm = weno5_diff(M[q + 3], -dM[q + 4], -dM[q + 3], -dM[q + 2], -dM[q + 1], sM[q + 3], sM[q + 2], sM[q + 1]);
-    Fh[q] = fp + fm;
+    weno5_diff(-dM[q + 4], -dM[q + 3], -dM[q + 2], -dM[q + 1], sM[q + 3], sM[q + 2], sM[q + 1], nm, rm);
+    Fh[q] = fma(fma(nm, rm, np * rp), 1.0 / 6.0, P[q + 2] + M[q + 3]);
   }
 }
 
