@@ -27,9 +27,9 @@ METRIC = "fp64 cell-updates/sec (RK3 step incl. point-implicit chemistry)"
 UNIT = "cell-updates/s"
 
 # algorithmic work / traffic per cell-update, derived in DESIGN.md "Roofline arithmetic"
-WENO_OPS = 30            # DP instructions (FMA = 1) of one WENO5-JS reconstruction in difference form
-                         # (flux.cuh: differences 4 amortised, betas 6, squares 3, weights 5, candidates 3,
-                         #  numerator 3, denominator 2, reciprocal 3 + 1)
+WENO_OPS = 29            # DP instructions (FMA = 1) of one WENO5-JS reconstruction in difference form
+                         # (flux.cuh: differences 4 amortised, betas 6, squares 3, candidates 3,
+                         #  weights + numerator + denominator 9, reciprocal 3 + 1)
 
 
 def flux_ops_per_cell_stage(ndim, nvar):

@@ -26,7 +26,7 @@
 // t_2 = D3 - 3 D2; the 1/2 is folded into 1/dx.  a_k = d_k/(eps+beta_k)^2 is evaluated as 10 d_k prod_{l!=k} B_l^2 over
 // the common denominator (one reciprocal per reconstruction), and the q_k numerators re-use t_k:
 //   5 D1 - 2 D0 = 2 t_0 - D1,   D1 + 2 D2 = t_1 + D2,   4 D2 - D3 = D2 - t_2.
-// One reconstruction is 32 fp64 instructions (4 for its share of the differences, 26 below, 2 of the face sum).
+// One reconstruction is 31 fp64 instructions (4 for its share of the differences, 25 below, 2 of the face sum).
 #pragma once
 #include "common.cuh"
 
@@ -48,11 +48,11 @@ __device__ __forceinline__ void weno5_diff(double D0, double D1, double D2, doub
   const double t0 = fma(3.0, D1, -D0), t1 = D1 + D2, t2 = fma(-3.0, D2, D3);
   double b0 = fma(t0, t0, S0), b1 = fma(t1, t1, S1), b2 = fma(t2, t2, S2);
   b0 *= b0; b1 *= b1; b2 *= b2;
-  const double h = 3.0 * b0;
-  const double a0 = b1 * b2, a1 = (h + h) * b2, a2 = h * b1;      // 10 x (0.1, 0.6, 0.3) x the other two B^2
+  // 10 a_k = (b1 b2, 6 b0 b2, 3 b0 b1):  num = b1 b2 c0 + 3 b0 (2 b2 c1 + b1 c2),  den = b1 b2 + 3 b0 (2 b2 + b1)
   const double c0 = fma(2.0, t0, -D1), c1 = t1 + D2, c2 = D2 - t2;
-  num = fma(a0, c0, fma(a1, c1, a2 * c2));
-  rden = rcp_pos((a0 + a1) + a2);
+  const double a0 = b1 * b2, h = 3.0 * b0, w = b2 + b2;
+  num = fma(a0, c0, h * fma(w, c1, b1 * c2));
+  rden = rcp_pos(fma(h, w + b1, a0));
 }
 
 // Face fluxes of one pencil, streamed: ld(k, fp2, fm2) returns 2f+ and 2f- of pencil cell k-3
@@ -93,6 +93,13 @@ __device__ __forceinline__ void weno_faces(Load &&ld, double (&Fh)[SEG + 1]) {
 __device__ __forceinline__ void split2(double Um, double ud, double p, double cE, double cM, double alpha,
                                        double &fp2, double &fm2) {
   const double F = fma(fma(cE, p, Um), ud, cM * p);
+  fp2 = fma(alpha, Um, F);
+  fm2 = fma(-alpha, Um, F);
+}
+
+// the same for a component without a pressure term (cE = cM = 0): bit-for-bit split2's result
+__device__ __forceinline__ void split_adv(double Um, double ud, double alpha, double &fp2, double &fm2) {
+  const double F = Um * ud;
   fp2 = fma(alpha, Um, F);
   fm2 = fma(-alpha, Um, F);
 }
@@ -157,7 +164,8 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
         const int gx = min(o0 + xi - 3, mx0), gy = min(o1 + r % TY, in1), gz = min(o2 + r / TY, in2);
         const long long id = cell_index(P, gx, gy, gz);
         double a, b;
-        split2(Um[id], ux[id], pp[id], cEn, cM, alpha[0], a, b);
+        if (m == 1 || m == NDIM + 1) split2(Um[id], ux[id], pp[id], cEn, cM, alpha[0], a, b);
+        else split_adv(Um[id], ux[id], alpha[0], a, b);       // advected components: no pressure read
         sFp[r * C::XP + xi] = a;
         sFm[r * C::XP + xi] = b;
       }
@@ -186,7 +194,8 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
         const int gz = d == 2 ? min(o2 + zz - 3, mx2) : min(o2 + zz, in2);
         const long long id = cell_index(P, gx, gy, gz);
         double a, b;
-        split2(Um[id], ud[id], pp[id], cEn, cM, al, a, b);
+        if (m == 1 + d || m == NDIM + 1) split2(Um[id], ud[id], pp[id], cEn, cM, al, a, b);
+        else split_adv(Um[id], ud[id], al, a, b);
         sFp[(zz * EY + yy) * C::LP + x] = a;
         sFm[(zz * EY + yy) * C::LP + x] = b;
       }
@@ -371,7 +380,10 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
       const int r = tid % TY, xs = (tid / TY) * SEG;
       const int base = (r + 3) * PIT + xs;
       double Fh[SEG + 1];
-      weno_faces<SEG>([&](int k, double &a, double &b) { split2(sUm[base + k], su[base + k], sp[base + k], cEn, cM, ax, a, b); }, Fh);
+      if (m == 1 || m == 3)
+        weno_faces<SEG>([&](int k, double &a, double &b) { split2(sUm[base + k], su[base + k], sp[base + k], cEn, cM, ax, a, b); }, Fh);
+      else   // advected components (rho, transverse momentum, rho Y_k): F = U_m u, no pressure read
+        weno_faces<SEG>([&](int k, double &a, double &b) { split_adv(sUm[base + k], su[base + k], ax, a, b); }, Fh);
 #pragma unroll
       for (int i = 0; i < SEG; i++) sL[r * C::LP + xs + i] = (Fh[i] - Fh[i + 1]) * hx;
     }
@@ -391,7 +403,10 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
       const int x = tid % TX, ys = (tid / TX) * SEG;
       const int base = ys * PIT + x + 3;
       double Fh[SEG + 1];
-      weno_faces<SEG>([&](int k, double &a, double &b) { split2(sUm[base + k * PIT], sv[base + k * PIT], sp[base + k * PIT], cEn, cM, ay, a, b); }, Fh);
+      if (m == 2 || m == 3)
+        weno_faces<SEG>([&](int k, double &a, double &b) { split2(sUm[base + k * PIT], sv[base + k * PIT], sp[base + k * PIT], cEn, cM, ay, a, b); }, Fh);
+      else
+        weno_faces<SEG>([&](int k, double &a, double &b) { split_adv(sUm[base + k * PIT], sv[base + k * PIT], ay, a, b); }, Fh);
 #pragma unroll
       for (int i = 0; i < SEG; i++) sL[(ys + i) * C::LP + x] += (Fh[i] - Fh[i + 1]) * hy;
     }
