@@ -29,6 +29,7 @@
 // One reconstruction is 31 fp64 instructions (4 for its share of the differences, 25 below, 2 of the face sum).
 #pragma once
 #include "common.cuh"
+#include <type_traits>
 
 #define JANC_WENO_EPS16 1.6e-5   // 16 * 1e-6, see above
 
@@ -158,17 +159,21 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
     {
       const double cM = m == 1 ? 1.0 : 0.0;
       const double *ux = P.vel + pbase;
+      // advected components (no pressure term) are staged by their own loop: no p load, 3-instruction split flux
+      auto stage_x = [&](auto gen) {
 #pragma unroll 4
-      for (int it = tid; it < C::ROWS * (TX + 6); it += NT) {
-        const int xi = it % (TX + 6), r = it / (TX + 6);
-        const int gx = min(o0 + xi - 3, mx0), gy = min(o1 + r % TY, in1), gz = min(o2 + r / TY, in2);
-        const long long id = cell_index(P, gx, gy, gz);
-        double a, b;
-        if (m == 1 || m == NDIM + 1) split2(Um[id], ux[id], pp[id], cEn, cM, alpha[0], a, b);
-        else split_adv(Um[id], ux[id], alpha[0], a, b);       // advected components: no pressure read
-        sFp[r * C::XP + xi] = a;
-        sFm[r * C::XP + xi] = b;
-      }
+        for (int it = tid; it < C::ROWS * (TX + 6); it += NT) {
+          const int xi = it % (TX + 6), r = it / (TX + 6);
+          const int gx = min(o0 + xi - 3, mx0), gy = min(o1 + r % TY, in1), gz = min(o2 + r / TY, in2);
+          const long long id = cell_index(P, gx, gy, gz);
+          double a, b;
+          if (decltype(gen)::value) split2(Um[id], ux[id], pp[id], cEn, cM, alpha[0], a, b);
+          else split_adv(Um[id], ux[id], alpha[0], a, b);
+          sFp[r * C::XP + xi] = a;
+          sFm[r * C::XP + xi] = b;
+        }
+      };
+      if (m == 1 || m == NDIM + 1) stage_x(std::true_type{}); else stage_x(std::false_type{});
       __syncthreads();
       const int r = tid % C::ROWS, xs = (tid / C::ROWS) * SEG;
       double Fh[SEG + 1];
@@ -186,19 +191,22 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
       const double *ud = P.vel + (long long)d * P.np * P.pc + pbase;
       const double al = alpha[d];
       const int EY = d == 1 ? TY + 6 : TY, EZ = d == 2 ? TZ + 6 : TZ;     // staged extent
+      auto stage_d = [&](auto gen) {
 #pragma unroll 4
-      for (int it = tid; it < TX * EY * EZ; it += NT) {
-        const int x = it % TX, yy = (it / TX) % EY, zz = it / (TX * EY);
-        const int gx = min(o0 + x, P.n[0] - 1);
-        const int gy = d == 1 ? min(o1 + yy - 3, mx1) : min(o1 + yy, in1);
-        const int gz = d == 2 ? min(o2 + zz - 3, mx2) : min(o2 + zz, in2);
-        const long long id = cell_index(P, gx, gy, gz);
-        double a, b;
-        if (m == 1 + d || m == NDIM + 1) split2(Um[id], ud[id], pp[id], cEn, cM, al, a, b);
-        else split_adv(Um[id], ud[id], al, a, b);
-        sFp[(zz * EY + yy) * C::LP + x] = a;
-        sFm[(zz * EY + yy) * C::LP + x] = b;
-      }
+        for (int it = tid; it < TX * EY * EZ; it += NT) {
+          const int x = it % TX, yy = (it / TX) % EY, zz = it / (TX * EY);
+          const int gx = min(o0 + x, P.n[0] - 1);
+          const int gy = d == 1 ? min(o1 + yy - 3, mx1) : min(o1 + yy, in1);
+          const int gz = d == 2 ? min(o2 + zz - 3, mx2) : min(o2 + zz, in2);
+          const long long id = cell_index(P, gx, gy, gz);
+          double a, b;
+          if (decltype(gen)::value) split2(Um[id], ud[id], pp[id], cEn, cM, al, a, b);
+          else split_adv(Um[id], ud[id], al, a, b);
+          sFp[(zz * EY + yy) * C::LP + x] = a;
+          sFm[(zz * EY + yy) * C::LP + x] = b;
+        }
+      };
+      if (m == 1 + d || m == NDIM + 1) stage_d(std::true_type{}); else stage_d(std::false_type{});
       __syncthreads();
       const int x = tid % TX, rest = tid / TX;
       // d == 1: pencils along y, the other index is z;  d == 2: pencils along z, the other index is y
