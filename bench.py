@@ -27,16 +27,16 @@ METRIC = "fp64 cell-updates/sec (RK3 step incl. point-implicit chemistry)"
 UNIT = "cell-updates/s"
 
 # algorithmic work / traffic per cell-update, derived in DESIGN.md "Roofline arithmetic"
-WENO_OPS = 29            # DP instructions (FMA = 1) of one WENO5-JS reconstruction in difference form
+WENO_OPS = 25            # DP instructions (FMA = 1) of one WENO5-JS reconstruction in difference form
                          # (flux.cuh: differences 4 amortised, betas 6, squares 3, candidates 3,
-                         #  weights + numerator + denominator 9, reciprocal 3 + 1)
+                         #  weights + numerator + denominator 9)
 
 
 def flux_ops_per_cell_stage(ndim, nvar):
-    # per component and direction: split flux 2f+- (3) + 2 reconstructions + face value from the two (4) +
-    # difference, scale (2); RK update 3.  Pencil-end faces and ghost-row split fluxes (the kernel's redundancy)
+    # per component and direction: split flux 2f+- (3) + 2 reconstructions + face value from the two over one
+    # reciprocal (10) + difference, scale (2); RK update 3.  Pencil-end faces and ghost-row split fluxes (the kernel's redundancy)
     # are NOT counted.
-    return nvar * (ndim * (3 + 2 * WENO_OPS + 4 + 2) + 3)
+    return nvar * (ndim * (3 + 2 * WENO_OPS + 10 + 2) + 3)
 
 
 def chem_ops_per_cell(mech):

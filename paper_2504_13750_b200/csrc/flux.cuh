@@ -26,7 +26,8 @@
 // t_2 = D3 - 3 D2; the 1/2 is folded into 1/dx.  a_k = d_k/(eps+beta_k)^2 is evaluated as 10 d_k prod_{l!=k} B_l^2 over
 // the common denominator (one reciprocal per reconstruction), and the q_k numerators re-use t_k:
 //   5 D1 - 2 D0 = 2 t_0 - D1,   D1 + 2 D2 = t_1 + D2,   4 D2 - D3 = D2 - t_2.
-// One reconstruction is 31 fp64 instructions (4 for its share of the differences, 25 below, 2 of the face sum).
+// One reconstruction is 30 fp64 instructions (4 for its share of the differences, 21 below, half of the 10 that join
+// the two reconstructions of a face over one reciprocal).
 #pragma once
 #include "common.cuh"
 #include <type_traits>
@@ -42,10 +43,10 @@ __device__ __forceinline__ double rcp_pos(double x) {
   return fma(fma(e, e, e), r, r);
 }
 
-// 6 (q - v) = num / den of the reconstruction with differences D0..D3 about the centre value v, returned as num and
-// 1/den;  S_k = 16 eps + 13/3 (D_{k+1}-D_k)^2
+// 6 (q - v) = num / den of the reconstruction with differences D0..D3 about the centre value v (den >= 1e-18: the
+// two reconstructions of a face share one reciprocal, of the product of their denominators);  S_k = 16 eps + 13/3 (D_{k+1}-D_k)^2
 __device__ __forceinline__ void weno5_diff(double D0, double D1, double D2, double D3, double S0, double S1, double S2,
-                                           double &num, double &rden) {
+                                           double &num, double &den) {
   const double t0 = fma(3.0, D1, -D0), t1 = D1 + D2, t2 = fma(-3.0, D2, D3);
   double b0 = fma(t0, t0, S0), b1 = fma(t1, t1, S1), b2 = fma(t2, t2, S2);
   b0 *= b0; b1 *= b1; b2 *= b2;
@@ -53,7 +54,7 @@ __device__ __forceinline__ void weno5_diff(double D0, double D1, double D2, doub
   const double c0 = fma(2.0, t0, -D1), c1 = t1 + D2, c2 = D2 - t2;
   const double a0 = b1 * b2, h = 3.0 * b0, w = b2 + b2;
   num = fma(a0, c0, h * fma(w, c1, b1 * c2));
-  rden = rcp_pos(fma(h, w + b1, a0));
+  den = fma(h, w + b1, a0);
 }
 
 // Face fluxes of one pencil, streamed: ld(k, fp2, fm2) returns 2f+ and 2f- of pencil cell k-3
@@ -80,12 +81,12 @@ __device__ __forceinline__ void weno_faces(Load &&ld, double (&Fh)[SEG + 1]) {
     const double s = dP[q + 4] - dP[q + 3], r = dM[q + 4] - dM[q + 3];
     sP[q + 3] = fma(K * s, s, JANC_WENO_EPS16);
     sM[q + 3] = fma(K * r, r, JANC_WENO_EPS16);
-    double np, rp, nm, rm;
+    double np, dp, nm, dm;
     // plus part: stencil cells q-3..q+1 (array q..q+4), upwind centre = array q+2
-    weno5_diff(dP[q], dP[q + 1], dP[q + 2], dP[q + 3], sP[q], sP[q + 1], sP[q + 2], np, rp);
+    weno5_diff(dP[q], dP[q + 1], dP[q + 2], dP[q + 3], sP[q], sP[q + 1], sP[q + 2], np, dp);
     // minus part: mirror image, cells q+2..q-2 (array q+5..q+1), centre = array q+3
-    weno5_diff(-dM[q + 4], -dM[q + 3], -dM[q + 2], -dM[q + 1], sM[q + 3], sM[q + 2], sM[q + 1], nm, rm);
-    Fh[q] = fma(fma(nm, rm, np * rp), 1.0 / 6.0, P[q + 2] + M[q + 3]);
+    weno5_diff(-dM[q + 4], -dM[q + 3], -dM[q + 2], -dM[q + 1], sM[q + 3], sM[q + 2], sM[q + 1], nm, dm);
+    Fh[q] = fma(fma(nm, dp, np * dm) * rcp_pos(dp * dm), 1.0 / 6.0, P[q + 2] + M[q + 3]);
   }
 }
 
