@@ -41,7 +41,7 @@ def flux_ops_per_cell_stage(ndim, nvar):
 
 def chem_ops_per_cell(mech):
     """Algorithmic DP instructions (FMA = 1) of the point-implicit update of one cell, counted from the mechanism
-    (DESIGN.md section 6): 3 Newton iterations on e(T); per reaction 2 exponentials (25 each) + Arrhenius arguments,
+    (DESIGN.md section 6): 3 Newton iterations on e(T); per reaction 2 exponentials (23 each) + Arrhenius arguments,
     concentration products and the net rate (12); one multiply per non-zero dq_i/dX_j and one add per non-zero
     contribution to D_kj (third-body reactions touch every column); I - dt J (2 per entry); elimination n^3/3 and
     the two triangular solves n^2."""
@@ -51,7 +51,7 @@ def chem_ops_per_cell(mech):
     tb = np.asarray(mech.third_body).astype(bool) if mech.third_body is not None else np.zeros(nr, bool)
     deg = max([q for q in range(5) if np.any(np.asarray(mech.nasa)[:, q] != 0.0)] + [0])
     newton = 3 * ns * (2 * deg + 3)
-    rates = nr * (2 * 25 + 12)
+    rates = nr * (2 * 23 + 12)
     entries = updates = 0
     for i in range(nr):
         rows = int(np.count_nonzero((nu_b[i] - nu_f[i])[:n1]))

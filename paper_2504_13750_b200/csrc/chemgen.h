@@ -112,8 +112,9 @@ inline void emit_math(std::string &src, bool estrin = false) {
          "  p = fma(p, r, 1.388888888888889e-03); p = fma(p, r, 8.333333333333333e-03); p = fma(p, r, 4.1666666666666664e-02);\n"
          "  p = fma(p, r, 1.6666666666666666e-01); p = fma(p, r, 0.5); p = fma(p, r, 1.0); p = fma(p, r, 1.0);\n";
   src +=
-         "  const int n1 = n >> 1, n2 = n - n1;\n"
-         "  return p * __hiloint2double((n1 + 1023) << 20, 0) * __hiloint2double((n2 + 1023) << 20, 0);\n"
+         "  // 2^n goes straight into the exponent field: p is in [0.70, 1.42] and n in [-1021, 1023] after the clamp, so the\n"
+         "  // biased exponent stays within [1, 2046] (no fp64 instruction, no intermediate overflow)\n"
+         "  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));\n"
          "}\n"
          "__device__ __forceinline__ double rcp_nb(double x) {\n"
          "  double r;\n"
