@@ -63,8 +63,8 @@ def chem_ops_per_cell(mech):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel (stages 2 and 3; the first
 # stage reads U^n only once: 4.21e8), from the committed `ncu --set full` capture of this same command
-# (profiles/r1e_summary.md); other workloads: not captured.
-NCU_TRAFFIC_BYTES = {"cfg2_2d_channel_4096x512": 6.32e8}
+# (profiles/r1f_summary.md); other workloads: not captured.
+NCU_TRAFFIC_BYTES = {"cfg2_2d_channel_4096x512": 6.28e8}
 
 
 def flux_bytes_per_cell_stage(ndim, nvar):
@@ -302,7 +302,7 @@ def main():
         byt = flux_bytes_per_cell_stage(nd, nvar) * cells
         roof = {"kernel": "k_flux_rk2" if nd == 2 else "k_flux_rk", "bound": "alu", "achieved": ops / fl_avg / 1e12, "peak": dfma / 1e12,
                 "unit": "T fp64-instr/s (FMA=1)", "frac": ops / fl_avg / dfma, "traffic": NCU_TRAFFIC_BYTES.get(case.name),
-                "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1e_summary.md)",
+                "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1f_summary.md)",
                 "peak_source": "measured: register-resident DFMA microbenchmark in this run",
                 "avg_launch_ms": fl_avg * 1e3, "launches_timed": fl_n,
                 "hbm": {"achieved": byt / fl_avg / 1e9, "peak": hbm_peak, "unit": "GB/s",
