@@ -13,8 +13,9 @@
 //      with coalesced loads; pencils then read them row-wise (odd pitch, conflict-free).
 //   y, z: the tile extended by 3 cells along the sweep direction is staged the same way ([z][y][x], odd x pitch);
 //      lanes run along x, so pencil reads are conflict-free.
-// Pencil results (-dF/dx_d) are summed per cell in shared memory; a coalesced pass applies the RK
-// stage.  No flux array ever goes to HBM: per stage the kernel reads U^(k) (+ U^n) and writes U^(k+1).
+// Pencil results (-dF/dx_d) are summed per cell in shared memory; a coalesced pass applies the RK stage (2-D kernel: the
+// thread that walks a y pencil adds its result to the x part and applies the RK stage of its own cells, lanes along x).
+// No flux array ever goes to HBM: per stage the kernel reads U^(k) (+ U^n) and writes U^(k+1).
 //
 // WENO5 in difference form.  With D_k = v_{k+1} - v_k (k = 0..3 over v_{-2..+2}):
 //   beta_0 = 13/12 (D1-D0)^2 + 1/4 (3 D1 - D0)^2,  beta_1 = 13/12 (D2-D1)^2 + 1/4 (D1+D2)^2,
@@ -397,19 +398,17 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
       for (int i = 0; i < SEG; i++) sL[r * C::LP + xs + i] = (Fh[i] - Fh[i + 1]) * hx;
     }
     __syncthreads();
-    // U^n of this thread's output cells: requested before the y pencils, consumed after them
-    double u0v[SEG];
-    if (!same) {
-#pragma unroll
-      for (int q = 0; q < SEG; q++) {
-        const int o = tid + q * NT;
-        const int g0 = min(o0 + o % TX, P.n[0] - 1), g1 = min(o1 + o / TX, P.n[1] - 1);
-        u0v[q] = U0p[cell_index(P, g0, g1, 0) + (long long)m * P.pc];
-      }
-    }
-    {  // y pencils: lanes run over columns
+    {  // y pencils: lanes run over columns.  The thread that walks cells (x, ys..ys+SEG-1) also applies their RK stage
+       // (increment form): U^n is requested before the walk and consumed after it; loads and stores are coalesced along x.
       const double cM = m == 2 ? 1.0 : 0.0;
       const int x = tid % TX, ys = (tid / TX) * SEG;
+      const int g0 = o0 + x, gc0 = min(g0, P.n[0] - 1);
+      double u0v[SEG];
+      if (!same) {
+#pragma unroll
+        for (int i = 0; i < SEG; i++)
+          u0v[i] = U0p[cell_index(P, gc0, min(o1 + ys + i, P.n[1] - 1), 0) + (long long)m * P.pc];
+      }
       const int base = ys * PIT + x + 3;
       double Fh[SEG + 1];
       if (m == 2 || m == 3)
@@ -417,20 +416,14 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
       else
         weno_faces<SEG>([&](int k, double &a, double &b) { split_adv(sUm[base + k * PIT], sv[base + k * PIT], ay, a, b); }, Fh);
 #pragma unroll
-      for (int i = 0; i < SEG; i++) sL[(ys + i) * C::LP + x] += (Fh[i] - Fh[i + 1]) * hy;
-    }
-    __syncthreads();
-    // RK stage (increment form), coalesced
-#pragma unroll
-    for (int q = 0; q < SEG; q++) {
-      const int o = tid + q * NT;
-      const int lx = o % TX, ly = o / TX;
-      const int g0 = o0 + lx, g1 = o1 + ly;
-      if (g0 < P.n[0] && g1 < P.n[1]) {
-        const long long id = cell_index(P, g0, g1, 0) + (long long)m * P.pc;
-        const double uk = sUm[(ly + 3) * PIT + lx + 3];
-        const double u0 = same ? uk : u0v[q];
-        Uop[id] = u0 + coef * ((uk - u0) + dt * sL[ly * C::LP + lx]);
+      for (int i = 0; i < SEG; i++) {
+        const int g1 = o1 + ys + i;
+        if (g0 < P.n[0] && g1 < P.n[1]) {
+          const double L = sL[(ys + i) * C::LP + x] + (Fh[i] - Fh[i + 1]) * hy;
+          const double uk = sUm[(ys + i + 3) * PIT + x + 3];
+          const double u0 = same ? uk : u0v[i];
+          Uop[cell_index(P, g0, g1, 0) + (long long)m * P.pc] = u0 + coef * ((uk - u0) + dt * L);
+        }
       }
     }
     __syncthreads();   // everyone is done with sU[m & 1] and sL
