@@ -67,7 +67,8 @@ typedef struct {
 
 /* Create a context for one grid on CUDA device `device`; kernels go to `cuda_stream`.  JANC_EINVAL for a malformed
  * grid, including fewer than 3 cells along a direction whose sides are not both zero-gradient (the 3 ghost layers of
- * PAPER.md:295 are copies of 3 distinct interior cells under the periodic, mirror and neighbour-patch rules). */
+ * PAPER.md:295 are copies of 3 distinct interior cells under the periodic, mirror and neighbour-patch rules), or a
+ * patch of 2^31 or more padded cells (more than one B200 holds). */
 int janc_create(const janc_grid *grid, int device, void *cuda_stream, janc_ctx **out);
 
 /* Mechanism must be set before the workspace is sized (nvar depends on ns). */

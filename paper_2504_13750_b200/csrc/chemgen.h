@@ -217,8 +217,9 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
   E.line("long long t = (long long)blockIdx.x * " + I(NT) + " + threadIdx.x;");
   E.line("const bool live = t < ncell;");
   E.line("if (!live) t = ncell - 1;   // idle lanes recompute the last cell and store nothing");
-  E.line("const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;");
-  E.line("const int cj = (int)(r_ % a.n1), ck = (int)(r_ / a.n1);");
+  // a patch holds fewer than 2^31 cells (janc_create): 32-bit divisions instead of the 64-bit software routine
+  E.line("const unsigned t32 = (unsigned)t, r_ = t32 / (unsigned)a.n0; const int ci = (int)(t32 - r_ * (unsigned)a.n0);");
+  E.line("const unsigned k_ = r_ / (unsigned)a.n1; const int cj = (int)(r_ - k_ * (unsigned)a.n1), ck = (int)k_;");
   E.line("const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;");
   E.line("double *Up = a.U + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
   E.line("const long long pid = (long long)blockIdx.y * a.pc + id;");
@@ -400,8 +401,9 @@ inline std::string generate_source(const MechC &M, int ndim, bool with_math) {
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
   E.line("const long long t = (long long)blockIdx.x * 128 + threadIdx.x;");
   E.line("if (t >= ncell) return;");
-  E.line("const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;");
-  E.line("const int cj = (int)(r_ % a.n1), ck = (int)(r_ / a.n1);");
+  // a patch holds fewer than 2^31 cells (janc_create): 32-bit divisions instead of the 64-bit software routine
+  E.line("const unsigned t32 = (unsigned)t, r_ = t32 / (unsigned)a.n0; const int ci = (int)(t32 - r_ * (unsigned)a.n0);");
+  E.line("const unsigned k_ = r_ / (unsigned)a.n1; const int cj = (int)(r_ - k_ * (unsigned)a.n1), ck = (int)k_;");
   E.line("const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;");
   E.line("const double *Up = a.Uk + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
   E.line("double *Uo = a.Uout + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
@@ -479,8 +481,9 @@ inline std::string generate_prim(const MechC &M, int ndim) {
   E.line("const long long t = (long long)blockIdx.x * 256 + threadIdx.x;");
   for (int d = 0; d < ndim; d++) E.line("double s" + I(d) + " = 0.0;");
   E.line("if (t < ncell) {");
-  E.line("const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;");
-  E.line("const int cj = (int)(r_ % a.n1), ck = (int)(r_ / a.n1);");
+  // a patch holds fewer than 2^31 cells (janc_create): 32-bit divisions instead of the 64-bit software routine
+  E.line("const unsigned t32 = (unsigned)t, r_ = t32 / (unsigned)a.n0; const int ci = (int)(t32 - r_ * (unsigned)a.n0);");
+  E.line("const unsigned k_ = r_ / (unsigned)a.n1; const int cj = (int)(r_ - k_ * (unsigned)a.n1), ck = (int)k_;");
   E.line("const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;");
   E.line("const double *Up = a.U + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
   E.line("const long long pid = (long long)blockIdx.y * a.pc + id;");

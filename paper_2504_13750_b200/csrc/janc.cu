@@ -146,6 +146,7 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
     }
     P.st[d] = P.pc; P.pc *= P.P[d]; c->ncell *= P.n[d];
   }
+  if (P.pc >= (1LL << 31)) { delete c; return JANC_EINVAL; }   // per-patch cell indices are 32-bit in the generated kernels
   P.dxmin = dxmin;
   int nf = 2 * grid->ndim;
   c->level.assign(c->np, 0);
