@@ -256,7 +256,7 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
     double hc[6] = {c[5], c[0], 0.5 * c[1], c[2] / 3.0, 0.25 * c[3], 0.2 * c[4]};
     E.line("const double g" + I(k) + " = fma(" + num(c[0]) + ", lnT, " + horner(sc, 5) + ") - (" + horner(hc, 6) + ") * iT;");
   }
-  if (any_rev) E.line("const double lnC0 = log(" + num(JANC_PATM / JANC_RU) + " * iT);");
+  if (any_rev) E.line("const double lnC0 = " + num(std::log(JANC_PATM / JANC_RU)) + " - lnT;   // ln(p0 / (Ru T))");
   E.line("const double dt = a.scal[0];");
   // ---- rates of progress (eq 4.7-4.9), wdot_k = sum_i dnu_ik q_i, D_k_j = sum_i dnu_ik dq_i/dX_j
   Acc accW(ns), accD(n1 * ns);
@@ -430,7 +430,7 @@ inline std::string generate_source(const MechC &M, int ndim, bool with_math) {
     double hc[6] = {c[5], c[0], 0.5 * c[1], c[2] / 3.0, 0.25 * c[3], 0.2 * c[4]};
     E.line("const double g" + I(k) + " = fma(" + num(c[0]) + ", lnT, " + horner(sc, 5) + ") - (" + horner(hc, 6) + ") * iT;");
   }
-  if (any_rev) E.line("const double lnC0 = log(" + num(JANC_PATM / JANC_RU) + " * iT);");
+  if (any_rev) E.line("const double lnC0 = " + num(std::log(JANC_PATM / JANC_RU)) + " - lnT;   // ln(p0 / (Ru T))");
   Acc accW(ns);
   for (int i = 0; i < nr; i++) {
     const std::string si = I(i);

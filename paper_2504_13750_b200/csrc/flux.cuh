@@ -331,7 +331,8 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
   const double *Ukp = Uk + pbase * P.nvar;
   const double *U0p = U0 + pbase * P.nvar;
   double *Uop = Uout + pbase * P.nvar;
-  const long long st1 = P.st[1];
+  const int st1i = (int)P.st[1];
+  const int goff = P.G[1] * st1i + P.G[0];              // offset of interior cell (0, 0) within a field
   const double ax = slot_value(P.slots + slot_base + lev * 3 + 0), ay = slot_value(P.slots + slot_base + lev * 3 + 1);
   const double hx = 0.5 * P.invdx[lev][0], hy = 0.5 * P.invdx[lev][1];
   const int mxp = P.P[0] - 1, myp = P.P[1] - 1;     // last padded index (ragged tiles stay in the array)
@@ -350,14 +351,15 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
   }
   // copy field `fld` of an array with `fpp` fields per patch into a box
   auto load_box = [&](double *dst, const double *base, int fpp, int fld) {
+    const double *fb = base + ((long long)patch * fpp + fld) * P.pc;
 #pragma unroll 4
     for (int it = tid; it < C::BX * C::BY; it += NT) {
       const int bx = it % C::BX, by = it / C::BX;
       if (GATHER) {
         cp_async8(dst + by * PIT + bx, base + ((long long)sq[it] * fpp + fld) * P.pc + sc[it]);
-      } else {
+      } else {   // 32-bit offsets within a field (a patch holds < 2^31 padded cells, janc_create)
         const int gx = min(o0 + bx, mxp), gy = min(o1 + by, myp);
-        cp_async8(dst + by * PIT + bx, base + ((long long)patch * fpp + fld) * P.pc + (long long)gy * st1 + gx);
+        cp_async8(dst + by * PIT + bx, fb + (gy * st1i + gx));
       }
     }
   };
@@ -403,11 +405,13 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
       const double cM = m == 2 ? 1.0 : 0.0;
       const int x = tid % TX, ys = (tid / TX) * SEG;
       const int g0 = o0 + x, gc0 = min(g0, P.n[0] - 1);
+      const double *U0m = U0p + (long long)m * P.pc;
+      double *Uom = Uop + (long long)m * P.pc;
       double u0v[SEG];
       if (!same) {
 #pragma unroll
         for (int i = 0; i < SEG; i++)
-          u0v[i] = U0p[cell_index(P, gc0, min(o1 + ys + i, P.n[1] - 1), 0) + (long long)m * P.pc];
+          u0v[i] = U0m[goff + min(o1 + ys + i, P.n[1] - 1) * st1i + gc0];
       }
       const int base = ys * PIT + x + 3;
       double Fh[SEG + 1];
@@ -422,7 +426,7 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
           const double L = sL[(ys + i) * C::LP + x] + (Fh[i] - Fh[i + 1]) * hy;
           const double uk = sUm[(ys + i + 3) * PIT + x + 3];
           const double u0 = same ? uk : u0v[i];
-          Uop[cell_index(P, g0, g1, 0) + (long long)m * P.pc] = u0 + coef * ((uk - u0) + dt * L);
+          Uom[goff + g1 * st1i + g0] = u0 + coef * ((uk - u0) + dt * L);
         }
       }
     }
