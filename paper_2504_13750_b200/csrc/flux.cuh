@@ -152,10 +152,15 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
   // last loadable index along each dim (keeps ragged tiles inside the padded array)
   const int mx0 = P.n[0] + 2, mx1 = NDIM > 1 ? P.n[1] + 2 : 0, mx2 = NDIM > 2 ? P.n[2] + 2 : 0;
   const int in1 = NDIM > 1 ? P.n[1] - 1 : 0, in2 = NDIM > 2 ? P.n[2] - 1 : 0;
+  // 32-bit offsets within a field (a patch holds < 2^31 padded cells, janc_create)
+  const int s1 = NDIM > 1 ? (int)P.st[1] : 0, s2 = NDIM > 2 ? (int)P.st[2] : 0;
+  const int goff = P.G[0] + P.G[1] * s1 + P.G[2] * s2;
 
 #pragma unroll 1
   for (int m = 0; m < P.nvar; m++) {
     const double *Um = Ukp + (long long)m * P.pc;
+    const double *U0m = U0p + (long long)m * P.pc;
+    double *Uom = Uop + (long long)m * P.pc;
     const double cEn = m == NDIM + 1 ? 1.0 : 0.0;
     // ---------------- x: stage 2f+- rows, then walk
     {
@@ -167,7 +172,7 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
         for (int it = tid; it < C::ROWS * (TX + 6); it += NT) {
           const int xi = it % (TX + 6), r = it / (TX + 6);
           const int gx = min(o0 + xi - 3, mx0), gy = min(o1 + r % TY, in1), gz = min(o2 + r / TY, in2);
-          const long long id = cell_index(P, gx, gy, gz);
+          const int id = goff + gx + gy * s1 + gz * s2;
           double a, b;
           if (decltype(gen)::value) split2(Um[id], ux[id], pp[id], cEn, cM, alpha[0], a, b);
           else split_adv(Um[id], ux[id], alpha[0], a, b);
@@ -200,7 +205,7 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
           const int gx = min(o0 + x, P.n[0] - 1);
           const int gy = d == 1 ? min(o1 + yy - 3, mx1) : min(o1 + yy, in1);
           const int gz = d == 2 ? min(o2 + zz - 3, mx2) : min(o2 + zz, in2);
-          const long long id = cell_index(P, gx, gy, gz);
+          const int id = goff + gx + gy * s1 + gz * s2;
           double a, b;
           if (decltype(gen)::value) split2(Um[id], ud[id], pp[id], cEn, cM, al, a, b);
           else split_adv(Um[id], ud[id], al, a, b);
@@ -231,9 +236,9 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
       const int lx = o % TX, ly = (o / TX) % TY, lz = o / (TX * TY);
       const int g0 = o0 + lx, g1 = o1 + ly, g2 = o2 + lz;
       if (g0 < P.n[0] && g1 < P.n[1] && g2 < P.n[2]) {
-        const long long id = cell_index(P, g0, g1, g2) + (long long)m * P.pc;
-        const double u0 = U0p[id];
-        Uop[id] = u0 + coef * ((Ukp[id] - u0) + dt * sL[(lz * TY + ly) * C::LP + lx]);
+        const int id = goff + g0 + g1 * s1 + g2 * s2;
+        const double u0 = U0m[id];
+        Uom[id] = u0 + coef * ((Um[id] - u0) + dt * sL[(lz * TY + ly) * C::LP + lx]);
       }
     }
     // the next component's x pencils overwrite sL only after its staging barrier
