@@ -357,11 +357,13 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
   // copy field `fld` of an array with `fpp` fields per patch into a box
   auto load_box = [&](double *dst, const double *base, int fpp, int fld) {
     const double *fb = base + ((long long)patch * fpp + fld) * P.pc;
+    const double *fbg = base + (long long)fld * P.pc;
+    const int fppc = fpp * (int)P.pc;                   // GATHER: patches / small grids, fields of one patch < 2^31 cells
 #pragma unroll 4
     for (int it = tid; it < C::BX * C::BY; it += NT) {
       const int bx = it % C::BX, by = it / C::BX;
       if (GATHER) {
-        cp_async8(dst + by * PIT + bx, base + ((long long)sq[it] * fpp + fld) * P.pc + sc[it]);
+        cp_async8(dst + by * PIT + bx, fbg + ((long long)sq[it] * fppc + sc[it]));      // one 32 x 32 -> 64 multiply
       } else {   // 32-bit offsets within a field (a patch holds < 2^31 padded cells, janc_create)
         const int gx = min(o0 + bx, mxp), gy = min(o1 + by, myp);
         cp_async8(dst + by * PIT + bx, fb + (gy * st1i + gx));
