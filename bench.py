@@ -62,9 +62,9 @@ def chem_ops_per_cell(mech):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel (stages 2 and 3; the first
-# stage reads U^n only once: 4.21e8), from the committed `ncu --set full` capture of this same command
+# stage reads U^n only once: 4.19e8), from the committed `ncu --set full` capture of this same command
 # (profiles/r1f_summary.md); other workloads: not captured.
-NCU_TRAFFIC_BYTES = {"cfg2_2d_channel_4096x512": 6.28e8}
+NCU_TRAFFIC_BYTES = {"cfg2_2d_channel_4096x512": 6.26e8}
 
 
 def flux_bytes_per_cell_stage(ndim, nvar):
