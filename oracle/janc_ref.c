@@ -731,6 +731,16 @@ int jref_chem_cell(const jref_mech *in, double T, double rho, const double *rhoY
 
 int jref_gauss_solve(int n, double *A, double *b) { return gauss_solve(n, A, b) ? JREF_OK : JREF_ENONFINITE; }
 
+/* Pin support: run ghost_fill on the current state and return the padded arrays (ghosts included),
+ * Upad[np][nvar][pc] with pc = prod_d (n_d + 6), x fastest; Tpad[np][pc] nullable. */
+int jref_debug_ghost_fill(jref_ctx *c, double *Upad, double *Tpad) {
+  if (!c || !c->have_state || !Upad) return JREF_ESTATE;
+  ghost_fill(c, c->U);
+  memcpy(Upad, c->U, sizeof(double) * (size_t)c->np * c->nvar * c->pc);
+  if (Tpad) memcpy(Tpad, c->T, sizeof(double) * (size_t)c->np * c->pc);
+  return JREF_OK;
+}
+
 /* thread control for the timed baseline (results do not depend on it) */
 int jref_set_threads(int n) {
 #ifdef _OPENMP

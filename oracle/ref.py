@@ -100,6 +100,7 @@ class RefSolver:
             if rc:
                 raise RuntimeError(f"jref_set_blocks failed: {rc}")
         self.np_ = max(1, grid.n_patches)
+        self.ndim = grid.ndim
         self.nvar = grid.ndim + 2 + mech.ns - 1
         self.shape = (self.np_, self.nvar, grid.n[2] if grid.ndim > 2 else 1,
                       grid.n[1] if grid.ndim > 1 else 1, grid.n[0])
@@ -127,6 +128,17 @@ class RefSolver:
         U = np.empty(self.shape)
         T = np.empty((self.shape[0],) + self.shape[2:])
         self.status = lib().jref_get_state(self._h, _ptr(U), _ptr(T))
+        return U, T
+
+    def debug_ghost_fill(self):
+        """Padded U [np, nvar, Pz, Py, Px] and T [np, Pz, Py, Px] right after ghost_fill (pins only)."""
+        nd = self.ndim
+        pad = lambda n, d: n + 6 if d < nd else 1
+        P = (pad(self.shape[2], 2), pad(self.shape[3], 1), pad(self.shape[4], 0))
+        U = np.empty((self.np_, self.nvar) + P)
+        T = np.empty((self.np_,) + P)
+        rc = lib().jref_debug_ghost_fill(self._h, _ptr(U), _ptr(T))
+        assert rc == 0, rc
         return U, T
 
     def close(self):

@@ -64,6 +64,8 @@ class Blocks:
     level: np.ndarray        # [np] int32
     nbr: np.ndarray          # [np, 2*ndim] int32 (lo-x, hi-x, lo-y, hi-y, ...), -1 none
     parent: np.ndarray       # [np, 1+ndim] int32 (parent id, sub-region index per dir), -1 on level 0
+    origin: np.ndarray = None  # [np, ndim] global index of the patch's cell (0,..,0) in cells of its OWN level
+                               # (layout bookkeeping for tests and regridding; the solver never needs it)
 
 
 @dataclass
@@ -362,11 +364,13 @@ def config3(pcols=128, prows=32, npc=16, seed=1003, nsteps=50, mech=None):
     level = np.zeros(npatch, dtype=np.int32)
     nbr = -np.ones((npatch, 4), dtype=np.int32)
     parent = -np.ones((npatch, 3), dtype=np.int32)
+    origin = np.zeros((npatch, 2), dtype=np.int64)
     U = np.zeros((npatch, nvar, 1, npc, npc))
     T = np.zeros((npatch, 1, npc, npc))
     for r in range(prows):
         for c in range(pcols):
             k = r * pcols + c
+            origin[k] = [c * npc, r * npc]
             nbr[k] = [k - 1 if c > 0 else -1, k + 1 if c < pcols - 1 else -1,
                       k - pcols if r > 0 else -1, k + pcols if r < prows - 1 else -1]
             U[k, :, 0] = Ug[:, r * npc:(r + 1) * npc, c * npc:(c + 1) * npc]
@@ -387,6 +391,7 @@ def config3(pcols=128, prows=32, npc=16, seed=1003, nsteps=50, mech=None):
                     level[f] = 1
                     parent[f] = [r * pcols + c, sx, sy]
                     fy, fx = 2 * r + sy, 2 * c + sx
+                    origin[f] = [fx * npc, fy * npc]
                     nbr[f] = [fid(fy, fx - 1), fid(fy, fx + 1), fid(fy - 1, fx), fid(fy + 1, fx)]
                     h = npc // 2
                     y0, x0 = r * npc + sy * h, c * npc + sx * h
@@ -396,7 +401,7 @@ def config3(pcols=128, prows=32, npc=16, seed=1003, nsteps=50, mech=None):
     r_ = (BC_REFLECT, BC_REFLECT, 0)
     g = Grid(2, (npc, npc, 1), (1e-4, 1e-4, 1.0), r_, r_, n_patches=npatch, n_levels=2, ratio=2)
     return Case(f"cfg3_amr_{npatch}x{npc}x{npc}", g, mech, U, T, 0.2, nsteps,
-                blocks=Blocks(level, nbr, parent))
+                blocks=Blocks(level, nbr, parent, origin))
 
 
 def config4(n=256, nspheres=50, radius=8, seed=1004, nsteps=20, mech=None):
