@@ -71,7 +71,20 @@ typedef struct {
  * patch of 2^31 or more padded cells (more than one B200 holds). */
 int janc_create(const janc_grid *grid, int device, void *cuda_stream, janc_ctx **out);
 
-/* Mechanism must be set before the workspace is sized (nvar depends on ns). */
+/* Options, as text (key, value); JANC_EINVAL for an unknown key or value.  The product runs the defaults; the other
+ * values exist so that tests can reach every kernel and every host path without environment variables.
+ *   "graph"            "1" (default) | "0"   replay one captured CUDA graph per step | eager launches
+ *   "halo"             "auto" (default) | "ghost"   auto: 2-D patches of <= 16 x 16 cells and 2-D grids below 600 k cells
+ *                      gather their halo inside the flux kernel; ghost: k_ghost always materialises the ghost layers
+ * and, only before janc_set_mechanism (JANC_ESTATE afterwards), the kernel selection of that call:
+ *   "jit"              "1" (default) | "0"   mechanism-specialised kernels compiled with NVRTC | table-driven kernels
+ *   "jit_max_unknowns" integer (default 12)  largest ns-1 of the one-thread-per-cell specialised chemistry kernel
+ *   "jit_big"          "roles" (default) | "smem"   kernel for larger mechanisms
+ *   "roles"            "8" (default) | "16"  role-warps per CTA of the role-warp chemistry kernel */
+int janc_set_option(janc_ctx *, const char *key, const char *value);
+
+/* Mechanism must be set before the workspace is sized (nvar depends on ns).  A rejected mechanism (JANC_EINVAL) leaves
+ * the context unchanged. */
 int janc_set_mechanism(janc_ctx *, const janc_mech *);
 
 /* Bytes of device memory the context needs (state with ghosts, RK registers, primitives,
@@ -130,8 +143,9 @@ int janc_measure_dfma_peak(int device, void *cuda_stream, double *dfma_per_s);
 /* Which chemistry kernel the context runs: "jit" = the mechanism-specialised kernel generated and
  * compiled with NVRTC by janc_set_mechanism (csrc/chemgen.h; the counterpart of the paper's XLA JIT,
  * PAPER.md:24, :39), "reg" / "generic" = the table-driven kernels of csrc/chem.cuh (mechanisms with
- * more than 12 unknowns, NVRTC missing, or JANC_DISABLE_JIT=1 in the environment), "none" before a
- * mechanism is set.  janc_jit_log returns the NVRTC log / the reason the specialised kernel is not used. */
+ * NVRTC missing, or janc_set_option("jit", "0")), "jit-roles" / "jit-smem" = the specialised kernels for more than 12
+ * unknowns, "none" before a mechanism is set.  janc_jit_log returns the NVRTC log / the reason the specialised kernel
+ * is not used, and a note if the per-step CUDA graph could not be captured and the context fell back to eager launches. */
 const char *janc_chem_kernel(const janc_ctx *);
 const char *janc_jit_log(const janc_ctx *);
 

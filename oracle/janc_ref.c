@@ -729,6 +729,31 @@ int jref_chem_cell(const jref_mech *in, double T, double rho, const double *rhoY
   return ok ? JREF_OK : JREF_ENONFINITE;
 }
 
+/* The same per-cell update (update_aux -> solve_implicit_rate) on a list of cells: Uc[ncell][nvar]
+ * (cell-major), Tguess[ncell] -> delta[ncell][ns-1], Tout[ncell].  Cells are independent; OpenMP over cells. */
+int jref_chem_cells(const jref_mech *in, int ndim, long ncell, const double *Uc, const double *Tguess, double dt,
+                    double *delta, double *Tout) {
+  mech_t m; memset(&m, 0, sizeof m);
+  if (mech_copy(&m, in)) return JREF_EINVAL;
+  int ns = m.ns, n1 = ns - 1, nvar = ndim + 2 + n1, bad = 0;
+#pragma omp parallel
+  {
+    double *work = malloc(sizeof(double) * (size_t)(ns + m.nr + m.nr * ns + n1 * n1 + 1));
+#pragma omp for reduction(| : bad) schedule(static)
+    for (long i = 0; i < ncell; i++) {
+      double Y[64], u[3], T, p, gam, cs;
+      const double *U = Uc + i * nvar;
+      int ok = cons2prim_cell(&m, ndim, U, Tguess[i], Y, u, &T, &p, &gam, &cs);
+      ok &= chem_cell(&m, T, U[0], U + ndim + 2, dt, delta + i * n1, work);
+      Tout[i] = T;
+      if (!ok) bad |= 1;
+    }
+    free(work);
+  }
+  mech_free(&m);
+  return bad ? JREF_ENONFINITE : JREF_OK;
+}
+
 int jref_gauss_solve(int n, double *A, double *b) { return gauss_solve(n, A, b) ? JREF_OK : JREF_ENONFINITE; }
 
 /* Pin support: run ghost_fill on the current state and return the padded arrays (ghosts included),

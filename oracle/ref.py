@@ -189,6 +189,18 @@ def chem_cell(mech, T, rho, rhoY, dt):
     return rc, d
 
 
+def chem_cells(mech, ndim, Uc, Tguess, dt):
+    """Batch of independent cells: Uc [ncell, nvar], Tguess [ncell] -> (rc, delta [ncell, ns-1], T [ncell])."""
+    mh = _MechHolder(mech)
+    Uc = _f64(Uc); Tg = _f64(Tguess)
+    n = Uc.shape[0]
+    d = np.zeros((n, max(mech.ns - 1, 1))); T = np.zeros(n)
+    fn = lib().jref_chem_cells
+    fn.argtypes = [C.c_void_p, C.c_int, C.c_long, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
+    rc = fn(C.byref(mh.c), int(ndim), n, _ptr(Uc), _ptr(Tg), float(dt), _ptr(d), _ptr(T))
+    return rc, d, T
+
+
 def gauss_solve(A, b):
     A = _f64(A).copy(); b = _f64(b).copy()
     rc = lib().jref_gauss_solve(int(b.size), _ptr(A), _ptr(b))

@@ -19,7 +19,7 @@ JANC_OK, JANC_EINVAL, JANC_ENOMEM, JANC_ECUDA, JANC_ESTATE, JANC_ENONFINITE = 0,
 FLAG_NO_CHEM = 1
 FLAG_EXPLICIT_SOURCE = 2
 
-EXPORTS = ["janc_create", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
+EXPORTS = ["janc_create", "janc_set_option", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
            "janc_set_blocks", "janc_set_state", "janc_step", "janc_get_state", "janc_status",
            "janc_launch_count", "janc_debug_cons2prim", "janc_profile_step",
            "janc_measure_dfma_peak", "janc_chem_kernel", "janc_jit_log", "janc_jit_probe",
@@ -58,6 +58,7 @@ def lib():
         L.janc_bind_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
         L.janc_create.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.janc_set_mechanism.argtypes = [C.c_void_p, C.c_void_p]
+        L.janc_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_char_p]
         L.janc_set_blocks.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.janc_set_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.janc_step.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int, C.c_void_p]
@@ -129,7 +130,7 @@ class Solver:
     """janc_* context: create -> set_mechanism -> bind_workspace (torch) -> [set_blocks] -> set_state
     -> step -> get_state -> destroy.  Same call names as the C ABI."""
 
-    def __init__(self, grid, mech, blocks=None, device=0, stream=None):
+    def __init__(self, grid, mech, blocks=None, device=0, stream=None, options=None):
         import torch
         if not torch.cuda.is_available():
             raise JancError(JANC_ECUDA, "no CUDA device (libjanc has no CPU fallback)")
@@ -147,6 +148,8 @@ class Solver:
         rc = L.janc_create(C.byref(g), self.device, C.c_void_p(stream.cuda_stream), C.byref(self._h))
         if rc:
             raise JancError(rc, "janc_create")
+        for k, v in (options or {}).items():          # janc_set_option(key, value), see include/janc.h
+            self._check(L.janc_set_option(self._h, str(k).encode(), str(v).encode()), f"janc_set_option({k})")
         m, self._keep = _mech_struct(mech)
         self._check(L.janc_set_mechanism(self._h, C.byref(m)), "janc_set_mechanism")
         nbytes = L.janc_workspace_bytes(self._h)
@@ -161,6 +164,9 @@ class Solver:
         self.shape = (self.np_, self.nvar, grid.n[2] if grid.ndim > 2 else 1,
                       grid.n[1] if grid.ndim > 1 else 1, grid.n[0])
         self.tshape = (self.shape[0],) + self.shape[2:]
+
+    def set_option(self, key, value):
+        self._check(lib().janc_set_option(self._h, str(key).encode(), str(value).encode()), f"janc_set_option({key})")
 
     def chem_kernel(self):
         """'jit' (mechanism-specialised, NVRTC), 'reg' or 'generic' (table-driven kernels)."""

@@ -36,10 +36,10 @@ namespace chemgen {
 // roles (warps) per CTA: 8 roles x 3 column slots (255 registers; the default) or 16 roles x 2 slots (128 registers).
 // Measured on cfg 4: 59 ms with 8 roles, 81 ms with 16 -- the per-column publish -> consume chain, not the number of
 // resident warps, bounds the elimination, and it is longer with 16 participants.
-inline int roles_nr() {
-  const char *e = getenv("JANC_ROLES_N");              // test knob
-  return e && atoi(e) == 16 ? 16 : 8;
-}
+// The count is a per-thread setting of the generator, set by janc.cu from the context's options (janc_set_option "roles")
+// before any function of this header is called.
+inline int &roles_nr_ref() { static thread_local int v = 8; return v; }
+inline int roles_nr() { return roles_nr_ref(); }
 
 struct RolesLayout {
   int oX, oP, oN, oRN, oDL, oRHS, oF, oPIV, oIP, oXS, oNX, oR, rows;   // offsets in rows of 32 doubles

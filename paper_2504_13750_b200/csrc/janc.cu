@@ -4,12 +4,15 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <memory>
 #include <string>
 #include <vector>
 
 #include <dlfcn.h>
 #include <map>
+#include <mutex>
 #include <nvrtc.h>
+#include <set>
 
 #include "../../include/janc.h"
 #include "chem.cuh"
@@ -19,7 +22,22 @@
 #include "ghost.cuh"
 #include "prim.cuh"
 
+// janc_set_option keys (include/janc.h); defaults are what the product runs
+struct Options {
+  bool graph = true;                    // "graph": replay one captured CUDA graph per step
+  bool jit = true;                      // "jit": run-time specialised kernels (NVRTC)
+  int jit_max_unknowns = JANC_JIT_MAX_N1;   // "jit_max_unknowns": largest system of the one-thread-per-cell kernel
+  bool jit_big_smem = false;            // "jit_big" = "smem": the shared-memory kernel instead of the role-warp kernel
+  int roles = 8;                        // "roles": 8 or 16 role-warps
+  bool halo_in_kernel = true;           // "halo" = "auto": 2-D patches <= 16 x 16 / small grids gather their halo in the
+                                        //   flux kernel; "ghost": always materialise ghosts with k_ghost
+};
+
 struct janc_ctx {
+  Options opt;
+  std::set<const void *> attr_done;     // kernels whose dynamic shared-memory attribute is set on THIS context's device
+  cudaError_t launch_err = cudaSuccess; // first failed kernel launch since the last check
+  bool uses_cmech = false;              // table-driven kernels (c_mech in constant memory) are on this context's path
   janc_grid g;
   int device;
   cudaStream_t stream;
@@ -55,7 +73,13 @@ struct janc_ctx {
 };
 
 static unsigned long long g_next_id = 1;
-static unsigned long long g_mech_owner = 0;   // which context's mechanism sits in c_mech
+// The table-driven fallback kernels read the mechanism from __constant__ c_mech, one copy per device, shared by all
+// contexts of the process.  g_mech_mutex serialises every call that launches such kernels (held for the whole call);
+// g_mech_owner[device] = which context's mechanism sits in that device's c_mech.  A re-upload first drains the device.
+static std::mutex g_mech_mutex;
+static std::mutex g_jit_mutex;                // the per-process caches of compiled kernels
+#define JANC_MAX_DEVICES 64
+static unsigned long long g_mech_owner[JANC_MAX_DEVICES] = {0};
 
 #define CK(call)                                                                         \
   do {                                                                                   \
@@ -114,7 +138,7 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
   c->g = *grid;
   c->device = device;
   c->num_sms = 148;
-  { const char *ng = getenv("JANC_NO_GRAPH"); c->use_graph = !(ng && ng[0] && ng[0] != '0'); }
+  if (device >= JANC_MAX_DEVICES) { delete c; return JANC_EINVAL; }
   cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
   c->stream = (cudaStream_t)cuda_stream;
   c->np = grid->n_patches > 0 ? grid->n_patches : 1;
@@ -164,7 +188,7 @@ static void invalidate_graphs(janc_ctx *c);
 
 extern "C" void janc_destroy(janc_ctx *c) {
   if (!c) return;
-  if (g_mech_owner == c->id) g_mech_owner = 0;
+  { std::lock_guard<std::mutex> lk(g_mech_mutex); if (g_mech_owner[c->device] == c->id) g_mech_owner[c->device] = 0; }
   invalidate_graphs(c);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
   delete c;
@@ -296,13 +320,10 @@ struct JitKernels { cudaKernel_t chem = nullptr, prim = nullptr, src = nullptr; 
 
 // 0: table-driven kernel, 1: register-resident specialised kernel (one thread per cell), 2: one thread per cell
 // with the matrix in smem, 3: 8 role-warps per 32 cells with the matrix columns in registers (chemgen_roles.h)
-static int jit_chem_mode(const MechC &M) {
-  int max_n1 = JANC_JIT_MAX_N1;
-  if (const char *e = getenv("JANC_JIT_MAX_N1")) max_n1 = atoi(e);     // test knob: push small mechanisms to the big path
+static int jit_chem_mode(const MechC &M, const Options &opt) {
   if (M.ns < 2 || M.nr < 1) return 0;
-  if (M.ns - 1 <= max_n1) return 1;
-  const char *big = getenv("JANC_JIT_BIG");                            // test knob: "smem" selects mode 2
-  if (chemgen::roles_applicable(M) && !(big && strcmp(big, "smem") == 0)) return 3;
+  if (M.ns - 1 <= opt.jit_max_unknowns) return 1;
+  if (chemgen::roles_applicable(M) && !opt.jit_big_smem) return 3;
   const size_t smem = (size_t)(M.ns - 1) * M.ns * JANC_JIT_NT_BIG * sizeof(double);
   return smem <= 200 * 1024 ? 2 : 0;
 }
@@ -316,9 +337,10 @@ static void jit_setup(janc_ctx *c) {
   c->jit_src_tried = false;
   c->jit_log.clear();
   const MechC &M = c->mech;
-  const char *off = getenv("JANC_DISABLE_JIT");
-  if (off && off[0] && off[0] != '0') { c->jit_log = "disabled by JANC_DISABLE_JIT"; return; }
-  const int mode = jit_chem_mode(M);
+  c->jit_chem_mode = 0;
+  if (!c->opt.jit) { c->jit_log = "disabled by janc_set_option(\"jit\", \"0\")"; return; }
+  chemgen::roles_nr_ref() = c->opt.roles;
+  const int mode = jit_chem_mode(M, c->opt);
   const bool chem = mode != 0;
   c->jit_chem_mode = mode;
   c->jit_chem_nt = mode == 3 ? chemgen::roles_nr() * 32 : mode == 2 ? JANC_JIT_NT_BIG : JANC_JIT_NT;
@@ -328,7 +350,8 @@ static void jit_setup(janc_ctx *c) {
   if (mode == 3) src += chemgen::generate_roles(M, c->g.ndim);
   else if (chem) src += chemgen::generate(M, c->g.ndim, mode == 2);
   else c->jit_log = "chemistry: mechanism outside the specialised range; ";
-  static std::map<std::string, JitKernels> cache;          // per process; one device per process
+  static std::map<std::string, JitKernels> cache;          // per process, keyed by device + source
+  std::lock_guard<std::mutex> lk(g_jit_mutex);
   const std::string key = std::to_string(c->device) + "\n" + src;
   auto it = cache.find(key);
   if (it != cache.end()) { c->jit_kernel = it->second.chem; c->jit_prim = it->second.prim; return; }
@@ -355,11 +378,11 @@ static void jit_setup_source(janc_ctx *c) {
   if (c->jit_src || c->jit_src_tried) return;
   c->jit_src_tried = true;
   const MechC &M = c->mech;
-  const char *off = getenv("JANC_DISABLE_JIT");
-  if (off && off[0] && off[0] != '0') { c->jit_log += " source kernel: disabled by JANC_DISABLE_JIT"; return; }
+  if (!c->opt.jit) { c->jit_log += " source kernel: disabled by janc_set_option(\"jit\", \"0\")"; return; }
   if (M.ns < 2 || M.nr < 1) return;
   const std::string src = chemgen::generate_source(M, c->g.ndim, true);
   static std::map<std::string, cudaKernel_t> cache;
+  std::lock_guard<std::mutex> lk(g_jit_mutex);
   const std::string key = std::to_string(c->device) + "\n" + src;
   auto it = cache.find(key);
   if (it != cache.end()) { c->jit_src = it->second; return; }
@@ -385,14 +408,19 @@ extern "C" const char *janc_jit_log(const janc_ctx *c) { return c ? c->jit_log.c
 // Diagnostic, needs no device: emit the specialised source for a mechanism and compile it for sm_100a.
 extern "C" int janc_jit_probe(const janc_mech *m, int ndim, char *src_out, size_t cap, size_t *src_len, size_t *cubin_bytes) {
   if (!m || ndim < 1 || ndim > 3) return JANC_EINVAL;
-  static MechC M;
+  std::unique_ptr<MechC> Mp(new (std::nothrow) MechC);
+  if (!Mp) return JANC_ENOMEM;
+  MechC &M = *Mp;
   std::string err;
   int rc = fill_mech(m, M, err);
   if (rc) return rc;
+  const Options opt;
+  chemgen::roles_nr_ref() = opt.roles;
+  const int mode = jit_chem_mode(M, opt);
   std::string src = chemgen::generate_prim(M, ndim);
-  if (jit_chem_mode(M) == 3) src += chemgen::generate_roles(M, ndim);
-  else if (jit_chem_mode(M)) src += chemgen::generate(M, ndim, jit_chem_mode(M) == 2);
-  if (M.ns >= 2 && M.nr >= 1) src += chemgen::generate_source(M, ndim, jit_chem_mode(M) == 0);   // same translation unit here: helpers once
+  if (mode == 3) src += chemgen::generate_roles(M, ndim);
+  else if (mode) src += chemgen::generate(M, ndim, mode == 2);
+  if (M.ns >= 2 && M.nr >= 1) src += chemgen::generate_source(M, ndim, mode == 0);   // same translation unit here: helpers once
   if (src_len) *src_len = src.size();
   if (src_out && cap > 0) { size_t n = src.size() < cap - 1 ? src.size() : cap - 1; memcpy(src_out, src.data(), n); src_out[n] = 0; }
   if (cubin_bytes) {
@@ -407,24 +435,65 @@ extern "C" int janc_jit_probe(const janc_mech *m, int ndim, char *src_out, size_
 
 extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
   if (!c || !m) return JANC_EINVAL;
-  int rc = fill_mech(m, c->mech, c->err);
-  if (rc) return rc;
+  // fill a temporary table and commit it only on success: a rejected mechanism leaves the context as it was
+  std::unique_ptr<MechC> tmp(new (std::nothrow) MechC);
+  if (!tmp) return JANC_ENOMEM;
+  std::string err;
+  int rc = fill_mech(m, *tmp, err);
+  if (rc) { c->err = err.empty() ? "malformed mechanism" : err; return rc; }
+  if (cudaSetDevice(c->device) != cudaSuccess) return JANC_ECUDA;
+  c->mech = *tmp;
   invalidate_graphs(c);
   jit_setup(c);
   c->ns = m->ns; c->nr = m->nr;
   c->nvar = c->g.ndim + 2 + m->ns - 1;
   c->P.nvar = c->nvar; c->P.ns = m->ns;
   c->have_mech = true; c->have_ws = false; c->have_state = false;
-  if (g_mech_owner == c->id) g_mech_owner = 0;
+  // which kernels of the path read c_mech: the table-driven cons->prim and / or chemistry
+  c->uses_cmech = !c->jit_prim || (m->ns > 1 && m->nr > 0 && !c->jit_kernel);
+  { std::lock_guard<std::mutex> lk(g_mech_mutex); if (g_mech_owner[c->device] == c->id) g_mech_owner[c->device] = 0; }
   return JANC_OK;
 }
 
+// Contexts on the table-driven path hold g_mech_mutex for the whole launching call (MechLock) and make sure their
+// mechanism is the one in the device's c_mech; a re-upload drains the device first, so no kernel of another context
+// that still reads the old table is in flight.
+struct MechLock {
+  std::unique_lock<std::mutex> lk;
+  explicit MechLock(janc_ctx *c) { if (c->uses_cmech) lk = std::unique_lock<std::mutex>(g_mech_mutex); }
+};
+
 static int upload_mech(janc_ctx *c) {
-  if (g_mech_owner == c->id) return JANC_OK;
-  CK(cudaMemcpyToSymbolAsync(c_mech, &c->mech, sizeof(MechC), 0, cudaMemcpyHostToDevice, c->stream));
-  CK(cudaStreamSynchronize(c->stream));   // c->mech is pageable host memory
-  g_mech_owner = c->id;
+  if (!c->uses_cmech || g_mech_owner[c->device] == c->id) return JANC_OK;
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpyToSymbol(c_mech, &c->mech, sizeof(MechC), 0, cudaMemcpyHostToDevice));
+  g_mech_owner[c->device] = c->id;
   return JANC_OK;
+}
+
+extern "C" int janc_set_option(janc_ctx *c, const char *key, const char *value) {
+  if (!c || !key || !value) return JANC_EINVAL;
+  const std::string k = key, v = value;
+  const bool on = !(v == "0" || v == "off" || v == "false");
+  if (k == "graph") { c->opt.graph = on; c->use_graph = on; if (!on) invalidate_graphs(c); return JANC_OK; }
+  if (k == "halo") {
+    if (v != "auto" && v != "ghost") { c->err = "halo: auto | ghost"; return JANC_EINVAL; }
+    c->opt.halo_in_kernel = v == "auto"; invalidate_graphs(c); return JANC_OK;
+  }
+  // the remaining keys select kernels at janc_set_mechanism time
+  if (c->have_mech) { c->err = "option '" + k + "' must be set before janc_set_mechanism"; return JANC_ESTATE; }
+  if (k == "jit") { c->opt.jit = on; return JANC_OK; }
+  if (k == "jit_max_unknowns") { c->opt.jit_max_unknowns = atoi(value); return JANC_OK; }
+  if (k == "jit_big") {
+    if (v != "roles" && v != "smem") { c->err = "jit_big: roles | smem"; return JANC_EINVAL; }
+    c->opt.jit_big_smem = v == "smem"; return JANC_OK;
+  }
+  if (k == "roles") {
+    if (v != "8" && v != "16") { c->err = "roles: 8 | 16"; return JANC_EINVAL; }
+    c->opt.roles = atoi(value); return JANC_OK;
+  }
+  c->err = "unknown option '" + k + "'";
+  return JANC_EINVAL;
 }
 
 // ------------------------------------------------------------------ workspace
@@ -605,6 +674,26 @@ static void prof_mark(janc_ctx *c, Prof *pf, int phase) {
   pf->phase.push_back(phase);
 }
 
+// every kernel launch of the step goes through here: counts it and keeps the first failure for the calling ABI function
+static void note_launch(janc_ctx *c, cudaError_t e) {
+  if (e != cudaSuccess && c->launch_err == cudaSuccess) c->launch_err = e;
+  c->launches++;
+}
+static int take_launch_error(janc_ctx *c) {
+  if (c->launch_err == cudaSuccess) return JANC_OK;
+  c->err = std::string("kernel launch failed: ") + cudaGetErrorString(c->launch_err);
+  c->launch_err = cudaSuccess;
+  cudaGetLastError();
+  return JANC_ECUDA;
+}
+// dynamic shared-memory limit of a kernel, once per context (= per device)
+static void smem_attr(janc_ctx *c, const void *fn, size_t bytes) {
+  if (c->attr_done.count(fn)) return;
+  const cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e != cudaSuccess && c->launch_err == cudaSuccess) c->launch_err = e;
+  c->attr_done.insert(fn);
+}
+
 template <int NS>
 static void launch_prim(janc_ctx *c, const double *U, int reduce, int slot_base, double *dbgc) {
   k_prim<NS><<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, U, reduce, slot_base, dbgc);
@@ -615,8 +704,7 @@ static void do_prim(janc_ctx *c, const double *U, int reduce, int slot_base, dou
     PrimArgs a{U, P.T, P.p, P.vel, dbgc, P.slots, P.level, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2],
                P.st[0], P.st[1], P.st[2], P.pc, P.np, reduce, slot_base};
     void *args[] = {&a};
-    cudaLaunchKernel((const void *)c->jit_prim, cell_grid(c, 256, c->np), dim3(256, 1, 1), args, 0, c->stream);
-    c->launches++;
+    note_launch(c, cudaLaunchKernel((const void *)c->jit_prim, cell_grid(c, 256, c->np), dim3(256, 1, 1), args, 0, c->stream));
     prof_mark(c, pf, 0);
     return;
   }
@@ -627,7 +715,7 @@ static void do_prim(janc_ctx *c, const double *U, int reduce, int slot_base, dou
     case 20: launch_prim<20>(c, U, reduce, slot_base, dbgc); break;
     default: launch_prim<0>(c, U, reduce, slot_base, dbgc); break;
   }
-  c->launches++;
+  note_launch(c, cudaGetLastError());
   prof_mark(c, pf, 0);
 }
 
@@ -635,7 +723,7 @@ static void do_prim(janc_ctx *c, const double *U, int reduce, int slot_base, dou
 // (flux.cuh, GATHER); no ghost fill
 static bool small_grid(const janc_ctx *c) { return (long long)c->np * c->ncell < 600000; }
 static bool gather_mode(const janc_ctx *c) {
-  return c->g.ndim == 2 && ((c->P.n[0] <= 16 && c->P.n[1] <= 16) || small_grid(c));
+  return c->opt.halo_in_kernel && c->g.ndim == 2 && ((c->P.n[0] <= 16 && c->P.n[1] <= 16) || small_grid(c));
 }
 
 static void do_ghost(janc_ctx *c, double *U, Prof *pf) {
@@ -651,7 +739,7 @@ static void do_ghost(janc_ctx *c, double *U, Prof *pf) {
   dim3 grid((unsigned)((total + 255) / 256), (unsigned)c->np, 1);
   for (int lev = 0; lev < c->g.n_levels; lev++) {
     k_ghost<<<grid, 256, 0, c->stream>>>(c->P, U, lev, amax);
-    c->launches++;
+    note_launch(c, cudaGetLastError());
   }
   prof_mark(c, pf, 1);
 }
@@ -660,11 +748,7 @@ template <int NDIM, int TX, int TY, int TZ, int SEG>
 static void launch_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef) {
   using C = FluxCfg<NDIM, TX, TY, TZ, SEG>;
   const Params &P = c->P;
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(k_flux_rk<NDIM, TX, TY, TZ, SEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-    attr_done = true;
-  }
+  smem_attr(c, (const void *)k_flux_rk<NDIM, TX, TY, TZ, SEG>, C::SMEM);
   const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY) * ((P.n[2] + TZ - 1) / TZ));
   k_flux_rk<NDIM, TX, TY, TZ, SEG><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
 }
@@ -673,11 +757,7 @@ template <int TX, int TY, int SEG, bool GATHER = false>
 static void launch_flux2(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef) {
   using C = Flux2Cfg<TX, TY, SEG, GATHER>;
   const Params &P = c->P;
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(k_flux_rk2<TX, TY, SEG, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-    attr_done = true;
-  }
+  smem_attr(c, (const void *)k_flux_rk2<TX, TY, SEG, GATHER>, C::SMEM);
   const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY));
   k_flux_rk2<TX, TY, SEG, GATHER><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
 }
@@ -686,11 +766,13 @@ static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uou
   const Params &P = c->P;
   if (c->g.ndim == 1) launch_flux<1, 128, 1, 1, 4>(c, Uk, U0, Uout, slot_base, coef);
   else if (c->g.ndim == 2) {
-    if (c->P.n[0] <= 16 && c->P.n[1] <= 16) launch_flux2<16, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches: halo gathered in-kernel; 2 warps per patch
-    else if (small_grid(c)) launch_flux2<32, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // small grids: 4x the CTAs, no ghost launches
+    const bool tiny = c->P.n[0] <= 16 && c->P.n[1] <= 16;
+    if (gather_mode(c) && tiny) launch_flux2<16, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches: halo gathered in-kernel; 2 warps per patch
+    else if (gather_mode(c)) launch_flux2<32, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // small grids: 4x the CTAs, no ghost launches
+    else if (c->P.n[0] <= 32) launch_flux2<32, 16, 4, false>(c, Uk, U0, Uout, slot_base, coef);   // patches of <= 32 columns with materialised ghosts
     else launch_flux2<64, 16, 8>(c, Uk, U0, Uout, slot_base, coef);
   } else launch_flux<3, 16, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);   // 128 threads, 39 KB: 4 independent CTAs per SM overlap stage / walk
-  c->launches++;
+  note_launch(c, cudaGetLastError());
   prof_mark(c, pf, 2);
 }
 
@@ -702,8 +784,7 @@ template <int NS>
 static void launch_chem_reg(janc_ctx *c, double *U) {
   constexpr int NT = 64;
   const size_t smem = (size_t)(NS + 2 * c->nr + c->mech.ntb) * NT * sizeof(double);
-  static bool attr_done = false;
-  if (!attr_done) { cudaFuncSetAttribute(k_chem_reg<NS, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); attr_done = true; }
+  smem_attr(c, (const void *)k_chem_reg<NS, NT>, 227 * 1024);
   k_chem_reg<NS, NT><<<cell_grid(c, NT, c->np), NT, smem, c->stream>>>(c->P, U);
 }
 static void do_chem(janc_ctx *c, double *U, Prof *pf) {
@@ -716,8 +797,7 @@ static void do_chem(janc_ctx *c, double *U, Prof *pf) {
       const long long turns = (long long)grid.x * grid.y;
       grid = dim3((unsigned)(turns < c->num_sms ? turns : c->num_sms), 1, 1);
     }
-    cudaLaunchKernel((const void *)c->jit_kernel, grid, dim3(c->jit_chem_nt, 1, 1), args, c->jit_chem_smem, c->stream);
-    c->launches++;
+    note_launch(c, cudaLaunchKernel((const void *)c->jit_kernel, grid, dim3(c->jit_chem_nt, 1, 1), args, c->jit_chem_smem, c->stream));
     prof_mark(c, pf, 3);
     return;
   }
@@ -727,7 +807,7 @@ static void do_chem(janc_ctx *c, double *U, Prof *pf) {
     case 20: launch_chem<20>(c, U); break;
     default: launch_chem<0>(c, U); break;
   }
-  c->launches++;
+  note_launch(c, cudaGetLastError());
   prof_mark(c, pf, 3);
 }
 
@@ -736,8 +816,7 @@ static void do_src(janc_ctx *c, const double *Uk, double *Uout, double coef, Pro
   const Params &P = c->P;
   SrcArgs a{Uk, Uout, P.T, P.scal, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc, coef};
   void *args[] = {&a};
-  cudaLaunchKernel((const void *)c->jit_src, cell_grid(c, 128, c->np), dim3(128, 1, 1), args, 0, c->stream);
-  c->launches++;
+  note_launch(c, cudaLaunchKernel((const void *)c->jit_src, cell_grid(c, 128, c->np), dim3(128, 1, 1), args, 0, c->stream));
   prof_mark(c, pf, 3);
 }
 
@@ -748,7 +827,7 @@ static void step_once(janc_ctx *c, double cfl, double dt_fixed, int flags, Prof 
   // stage 0: update_aux on U^n (also the cfl() evaluation), dt, ghost fill, fluxes
   do_prim(c, c->A, 1, SLOT(par, 0, 0, 0), nullptr, pf);
   k_dt<<<1, 32, 0, c->stream>>>(c->P, par, cfl, dt_fixed);
-  c->launches++;
+  note_launch(c, cudaGetLastError());
   prof_mark(c, pf, 0);
   do_ghost(c, c->A, pf);
   const bool esrc = (flags & 2) && c->jit_src && c->ns > 1 && c->nr > 0;   // source inside every stage
@@ -774,7 +853,7 @@ static void step_once(janc_ctx *c, double cfl, double dt_fixed, int flags, Prof 
     for (int d = 0; d < nd; d++) nc /= r;
     dim3 grid((unsigned)((nc * c->nvar + 255) / 256), (unsigned)c->np, 1);
     k_average_down<<<grid, 256, 0, c->stream>>>(c->P, c->A);
-    c->launches++;
+    note_launch(c, cudaGetLastError());
     prof_mark(c, pf, 4);
   }
   c->parity = 1 - par;
@@ -811,15 +890,22 @@ static void run_step(janc_ctx *c, double cfl, double dt_fixed, int flags) {
     if (ok) ok = cudaGraphInstantiate(&G.exec, g, 0) == cudaSuccess;
     if (g) cudaGraphDestroy(g);
     if (!ok) {
-      cudaGetLastError();
+      const cudaError_t e = cudaGetLastError();
       G.exec = nullptr;
       c->use_graph = false;
+      c->jit_log += std::string(" [step graph: capture / instantiate failed (") + cudaGetErrorString(e) + "), eager launches from here on]";
       step_once(c, cfl, dt_fixed, flags, nullptr);
       return;
     }
     G.cfl = cfl; G.dt = dt_fixed; G.flags = flags;
   }
-  if (cudaGraphLaunch(G.exec, c->stream) != cudaSuccess) { cudaGetLastError(); c->use_graph = false; step_once(c, cfl, dt_fixed, flags, nullptr); return; }
+  if (const cudaError_t e = cudaGraphLaunch(G.exec, c->stream); e != cudaSuccess) {
+    cudaGetLastError();
+    c->use_graph = false;
+    c->jit_log += std::string(" [step graph: launch failed (") + cudaGetErrorString(e) + "), eager launches from here on]";
+    step_once(c, cfl, dt_fixed, flags, nullptr);
+    return;
+  }
   c->launches += G.launches;
   c->parity = 1 - par;
 }
@@ -841,6 +927,7 @@ extern "C" int janc_step(janc_ctx *c, int nsteps, double cfl, double dt_fixed, i
     return JANC_ESTATE;
   }
   CK(cudaSetDevice(c->device));
+  MechLock mech_lock(c);
   rc = upload_mech(c);
   if (rc) return rc;
   double t0 = 0.0;
@@ -849,6 +936,7 @@ extern "C" int janc_step(janc_ctx *c, int nsteps, double cfl, double dt_fixed, i
     CK(cudaStreamSynchronize(c->stream));
   }
   for (int s = 0; s < nsteps; s++) run_step(c, cfl, dt_fixed, flags);
+  if ((rc = take_launch_error(c)) != JANC_OK) return rc;
   CK(cudaGetLastError());
   if (t_advanced) {
     double t1 = 0.0;
@@ -865,10 +953,12 @@ extern "C" int janc_profile_step(janc_ctx *c, double cfl, double dt_fixed, float
   if (rc) return rc;
   if (!ms_out) return JANC_EINVAL;
   CK(cudaSetDevice(c->device));
+  MechLock mech_lock(c);
   rc = upload_mech(c);
   if (rc) return rc;
   Prof pf;
   step_once(c, cfl, dt_fixed, 0, &pf);
+  if ((rc = take_launch_error(c)) != JANC_OK) { for (auto e : pf.ev) cudaEventDestroy(e); return rc; }
   CK(cudaStreamSynchronize(c->stream));
   for (int q = 0; q < 6; q++) { ms_out[q] = 0.f; if (n_out) n_out[q] = 0; }
   for (size_t e = 1; e < pf.ev.size(); e++) {
@@ -889,9 +979,11 @@ extern "C" int janc_debug_cons2prim(janc_ctx *c, double *T, double *p, double *c
   int rc = check_ready(c);
   if (rc) return rc;
   CK(cudaSetDevice(c->device));
+  MechLock mech_lock(c);
   rc = upload_mech(c);
   if (rc) return rc;
   do_prim(c, c->A, 0, 0, c->dbgc, nullptr);
+  if ((rc = take_launch_error(c)) != JANC_OK) return rc;
   const size_t nT = (size_t)c->np * c->ncell;
   double *srcs[3] = {c->P.T, c->P.p, c->dbgc};
   double *dsts[3] = {T, p, cs};

@@ -469,3 +469,93 @@ def untile(case_tiled: Case, U, px, py):
         for c in range(px):
             out[0, :, 0, r * ty:(r + 1) * ty, c * tx:(c + 1) * tx] = U[r * px + c, :, 0]
     return out
+
+
+def refine_uniform(case: Case, tile, refine):
+    """Re-express a uniform-grid case (ndim 1, 2 or 3) as a two-level block list: the grid is cut into level-0
+    patches of `tile` cells and every patch with refine[pz, py, px] True gets 2^ndim level-1 children (its fixed
+    sub-regions) holding the one-to-four injection of its data.  Periodic sides
+    become wrap-around neighbour links on both levels.  Patch order: level 0 x-fastest, then the children of each
+    refined patch, sub-region x-fastest."""
+    g = case.grid
+    nd = g.ndim
+    assert g.n_patches == 0
+    n = [g.n[d] if d < nd else 1 for d in range(3)]
+    t = [tile[d] if d < nd else 1 for d in range(3)]
+    assert all(n[d] % t[d] == 0 and (t[d] % 2 == 0 or d >= nd) for d in range(3))
+    pc = [n[d] // t[d] for d in range(3)]
+    refine = np.asarray(refine, dtype=bool).reshape(pc[2], pc[1], pc[0])
+    per = [d < nd and g.bc_lo[d] == BC_PERIODIC for d in range(3)]
+    n0 = pc[0] * pc[1] * pc[2]
+    sub = [2 if d < nd else 1 for d in range(3)]
+    fine_id = -np.ones((pc[2], pc[1], pc[0], sub[2], sub[1], sub[0]), dtype=np.int64)
+    nxt = n0
+    for z, y, x in itertools.product(range(pc[2]), range(pc[1]), range(pc[0])):
+        if refine[z, y, x]:
+            for sz, sy, sx in itertools.product(range(sub[2]), range(sub[1]), range(sub[0])):
+                fine_id[z, y, x, sz, sy, sx] = nxt
+                nxt += 1
+    npatch = nxt
+    nvar = case.nvar
+    level = np.zeros(npatch, dtype=np.int32)
+    nbr = -np.ones((npatch, 2 * nd), dtype=np.int32)
+    parent = -np.ones((npatch, 1 + nd), dtype=np.int32)
+    origin = np.zeros((npatch, nd), dtype=np.int64)
+    U = np.zeros((npatch, nvar, t[2], t[1], t[0]))
+    T = np.zeros((npatch, t[2], t[1], t[0]))
+
+    def wrap(c, cnt):
+        """patch coordinates -> wrapped coordinates or None when outside a non-periodic side"""
+        out = []
+        for d in range(3):
+            v = c[d]
+            if v < 0 or v >= cnt[d]:
+                if not per[d]:
+                    return None
+                v %= cnt[d]
+            out.append(v)
+        return out
+
+    for z, y, x in itertools.product(range(pc[2]), range(pc[1]), range(pc[0])):
+        k = (z * pc[1] + y) * pc[0] + x
+        c = [x, y, z]
+        origin[k] = [c[d] * t[d] for d in range(nd)]
+        for d in range(nd):
+            for side in (0, 1):
+                cc = list(c); cc[d] += 2 * side - 1
+                w = wrap(cc, pc)
+                nbr[k, 2 * d + side] = -1 if w is None else (w[2] * pc[1] + w[1]) * pc[0] + w[0]
+        sl = (slice(z * t[2], (z + 1) * t[2]), slice(y * t[1], (y + 1) * t[1]), slice(x * t[0], (x + 1) * t[0]))
+        U[k] = case.U[0][(slice(None),) + sl]
+        T[k] = case.T[0][sl]
+    fcnt = [pc[d] * sub[d] for d in range(3)]
+    for z, y, x in itertools.product(range(pc[2]), range(pc[1]), range(pc[0])):
+        if not refine[z, y, x]:
+            continue
+        k = (z * pc[1] + y) * pc[0] + x
+        for sz, sy, sx in itertools.product(range(sub[2]), range(sub[1]), range(sub[0])):
+            f = fine_id[z, y, x, sz, sy, sx]
+            s3 = [sx, sy, sz]
+            fc = [2 * x + sx if nd > 0 else 0, (2 * y + sy) if nd > 1 else 0, (2 * z + sz) if nd > 2 else 0]
+            level[f] = 1
+            parent[f] = [k] + s3[:nd]
+            origin[f] = [fc[d] * t[d] for d in range(nd)]
+            for d in range(nd):
+                for side in (0, 1):
+                    cc = list(fc); cc[d] += 2 * side - 1
+                    w = wrap(cc, fcnt)
+                    if w is not None:
+                        nbr[f, 2 * d + side] = fine_id[w[2] // sub[2], w[1] // sub[1], w[0] // sub[0],
+                                                       w[2] % sub[2], w[1] % sub[1], w[0] % sub[0]]
+            h = [t[d] // sub[d] for d in range(3)]
+            sl = tuple(slice(s3[d] * h[d], (s3[d] + 1) * h[d]) for d in (2, 1, 0))
+            blockU = U[k][(slice(None),) + sl]
+            blockT = T[k][sl]
+            for ax, d in ((1, 2), (2, 1), (3, 0)):
+                blockU = np.repeat(blockU, sub[d], axis=ax)
+                blockT = np.repeat(blockT, sub[d], axis=ax - 1)
+            U[f] = blockU
+            T[f] = blockT
+    g2 = Grid(nd, tuple(t), g.dx, g.bc_lo, g.bc_hi, n_patches=npatch, n_levels=2, ratio=2)
+    return Case(case.name + "_2lev", g2, case.mech, U, T, case.cfl, case.nsteps,
+                blocks=Blocks(level, nbr, parent, origin))

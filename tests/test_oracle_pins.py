@@ -672,6 +672,84 @@ def test_two_level_ghosts_hold_the_cell_that_contains_their_centre(ref, mech9):
             assert Up[p, 0, 0, j + 3, i + 3] == f0(Xm, Ym)
 
 
+def _ghost_expect(x, N, bc_lo, bc_hi):
+    """global index of the interior cell a position beyond a physical side copies, and whether it is a mirror"""
+    if x < 0:
+        return {I.BC_PERIODIC: x + N, I.BC_REFLECT: -1 - x, I.BC_OUTFLOW: 0}[bc_lo], bc_lo == I.BC_REFLECT
+    if x >= N:
+        return {I.BC_PERIODIC: x - N, I.BC_REFLECT: 2 * N - 1 - x, I.BC_OUTFLOW: N - 1}[bc_hi], bc_hi == I.BC_REFLECT
+    return x, False
+
+
+@pytest.mark.parametrize("nd", [1, 3])
+def test_two_level_ghosts_1d_and_3d_block_lists(ref, nd):
+    """The same global-coordinate pin as above for 1-D and 3-D two-level block lists (inputs.refine_uniform) with a
+    mix of periodic, slip-wall and zero-gradient sides: every face ghost of every patch holds the value of the cell
+    (of its own level if that position is refined or it is a level-0 patch, else of level 0) that the neighbour /
+    coarse-parent / physical-BC rule points at, computed here from patch origins only."""
+    if nd == 1:
+        base = I.config0(n=64); tile = (8,); mask = np.zeros(8, bool); mask[[0, 3, 4]] = True
+        bc_lo, bc_hi = (I.BC_REFLECT, 0, 0), (I.BC_OUTFLOW, 0, 0)
+    else:
+        base = I.config4(n=16, nspheres=1, radius=3); tile = (8, 4, 8)
+        mask = np.zeros((2, 4, 2), bool); mask[0, 1, 0] = mask[1, 1, 0] = mask[1, 2, 1] = mask[0, 0, 1] = mask[1, 3, 1] = True
+        bc_lo, bc_hi = (I.BC_PERIODIC, I.BC_REFLECT, I.BC_OUTFLOW), (I.BC_PERIODIC, I.BC_OUTFLOW, I.BC_REFLECT)
+    base.grid.bc_lo, base.grid.bc_hi = bc_lo, bc_hi
+    c = I.refine_uniform(base, tile, mask)
+    N0 = [base.grid.n[d] for d in range(nd)]
+    lev, org, nbr = c.blocks.level, c.blocks.origin, c.blocks.nbr
+    t3 = list(tile) + [1] * (3 - nd)
+    w = [1.0, 300.0, 90000.0]
+    f0 = lambda X: 1.0 + sum(w[d] * X[d] for d in range(nd))
+    f1 = lambda x: 5.0e7 + sum(2 * w[d] * x[d] for d in range(nd))
+    refined = set()
+    for p in np.nonzero(lev == 1)[0]:
+        refined.add(tuple(org[p] // np.array(tile)))            # fine-patch coordinates present on level 1
+    U = np.zeros_like(c.U)
+    kk, jj, ii = np.meshgrid(np.arange(t3[2]), np.arange(t3[1]), np.arange(t3[0]), indexing="ij")
+    loc = [ii, jj, kk]
+    for p in range(len(lev)):
+        f = f1 if lev[p] else f0
+        val = f([org[p, d] + loc[d] for d in range(nd)])
+        for v in range(c.nvar):
+            U[p, v] = (v + 1) * val
+    s = ref.RefSolver(c.grid, c.mech, c.blocks)
+    s.set_state(U, c.T)
+    Up, _ = s.debug_ghost_fill()
+    s.close()
+    G = [3 if d < nd else 0 for d in range(3)]
+    kinds = set()
+    rng = np.random.default_rng(5)
+    for p in range(len(lev)):
+        L = int(lev[p]); N = [N0[d] * (2 ** L) for d in range(nd)]
+        for d in range(nd):
+            for side in (0, 1):
+                for g in (1, 2, 3):
+                    for _ in range(6):
+                        i = [int(rng.integers(0, t3[e])) for e in range(3)]
+                        i[d] = -g if side == 0 else t3[d] - 1 + g
+                        x = [int(org[p, e]) + i[e] for e in range(nd)]
+                        src, mirror = _ghost_expect(x[d], N[d], bc_lo[d], bc_hi[d])
+                        xs = list(x); xs[d] = src
+                        if L == 0:
+                            want = f0(xs); kinds.add("l0-phys" if src != x[d] else "l0-nbr")
+                        else:
+                            outside = x[d] < 0 or x[d] >= N[d]
+                            periodic = (bc_lo[d] if x[d] < 0 else bc_hi[d]) == I.BC_PERIODIC
+                            if outside and not periodic:      # wall / zero-gradient side: own-level interior cell
+                                want = f1(xs); kinds.add("l1-phys")
+                            elif tuple(xs[e] // tile[e] for e in range(nd)) in refined:
+                                want = f1(xs); kinds.add("l1-nbr")
+                            else:                             # coarse-fine face (possibly across a periodic wrap)
+                                want = f0([q // 2 for q in xs]); kinds.add("l1-coarse")
+                        sign = np.ones(c.nvar)
+                        if mirror:
+                            sign[1 + d] = -1.0
+                        got = Up[(p, slice(None)) + tuple(i[e] + G[e] for e in (2, 1, 0))]
+                        assert np.array_equal(got, sign * (np.arange(c.nvar) + 1) * want), (p, d, side, g, i, got[0], want)
+    assert {"l0-nbr", "l0-phys", "l1-nbr", "l1-coarse", "l1-phys"} <= kinds, kinds
+
+
 def _mirror_case(mech, n, m, seed, axis):
     """Random smooth reflecting box n x m and its even extension across the `axis` wall to a periodic box of
     twice the length (rho, E, rho Y, tangential momentum even; wall-normal momentum odd)."""
