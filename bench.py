@@ -61,10 +61,12 @@ def chem_ops_per_cell(mech):
     return newton + rates + entries + updates + 2 * n1 * n1 + n1 ** 3 // 3 + n1 * n1
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel (stages 2 and 3; the first
-# stage reads U^n only once: 4.19e8), from the committed `ncu --set full` capture of this same command
-# (profiles/r1f_summary.md); other workloads: not captured.
-NCU_TRAFFIC_BYTES = {"cfg2_2d_channel_4096x512": 6.26e8}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (flux: stages 2 and 3; the first stage reads U^n only
+# once) from the committed `ncu --set full` captures named in profiles/*_summary.md; None where no capture exists.
+NCU_TRAFFIC_BYTES = {
+    ("cfg2_2d_channel_4096x512", "flux"): 6.26e8,       # profiles/r1f_summary.md
+}
+NCU_TRAFFIC_SOURCE = "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch (profiles/*_summary.md)"
 
 
 def flux_bytes_per_cell_stage(ndim, nvar):
@@ -125,19 +127,34 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(self.rows)}
 
 
+def crop_case(case, nx2d, ny2d, n3d=32):
+    """A bounded sample of a workload for the CPU oracle: 2-D uniform grids are cropped to their first nx2d x ny2d
+    cells (the driver section and the ambient gas next to it), 3-D grids to the aligned n3d^3 sub-cube that holds the
+    most hot cells; 1-D and block-list cases are small enough to run whole."""
+    g = case.grid
+    if g.n_patches == 0 and g.ndim == 2:
+        nx, ny = min(g.n[0], nx2d), min(g.n[1], ny2d)
+        U = np.ascontiguousarray(case.U[:, :, :, :ny, :nx]); T = np.ascontiguousarray(case.T[:, :, :ny, :nx])
+        crop = I.Case(case.name + "_crop", I.Grid(2, (nx, ny, 1), g.dx, g.bc_lo, g.bc_hi), case.mech, U, T, case.cfl, 1)
+        return crop, f"{case.name} cropped to {nx}x{ny} cells (columns 0..{nx - 1}, rows 0..{ny - 1})"
+    if g.n_patches == 0 and g.ndim == 3 and g.n[0] > n3d:
+        n = n3d
+        nb = g.n[0] // n
+        hot = (case.T[0] > 1000.0).reshape(nb, n, nb, n, nb, n).sum(axis=(1, 3, 5))
+        kz, ky, kx = np.unravel_index(int(np.argmax(hot)), hot.shape)
+        sl = (slice(kz * n, (kz + 1) * n), slice(ky * n, (ky + 1) * n), slice(kx * n, (kx + 1) * n))
+        U = np.ascontiguousarray(case.U[(slice(None), slice(None)) + sl]); T = np.ascontiguousarray(case.T[(slice(None),) + sl])
+        crop = I.Case(case.name + "_crop", I.Grid(3, (n, n, n), g.dx, g.bc_lo, g.bc_hi), case.mech, U, T, case.cfl, 1)
+        return crop, (f"{case.name} cropped to the {n}^3 sub-cube at z,y,x = {kz * n},{ky * n},{kx * n} "
+                      f"({int(hot[kz, ky, kx])} hot cells), periodic")
+    return case, f"{case.name} (whole)"
+
+
 def oracle_throughput(case, budget_s=15.0):
     """The oracle as it stands, on a bounded sample of the workload (cropped IC), host cores."""
     from oracle import ref
     ref.build()
-    g = case.grid
-    if g.n_patches > 0 or g.ndim != 2:
-        crop = case          # small / block cases: run as they are for a couple of steps
-        desc = f"{case.name} (whole)"
-    else:
-        nx, ny = min(g.n[0], 512), min(g.n[1], 256)
-        U = np.ascontiguousarray(case.U[:, :, :, :ny, :nx]); T = np.ascontiguousarray(case.T[:, :, :ny, :nx])
-        crop = I.Case(case.name + "_crop", I.Grid(2, (nx, ny, 1), g.dx, g.bc_lo, g.bc_hi), case.mech, U, T, case.cfl, 1)
-        desc = f"{case.name} cropped to {nx}x{ny} cells (columns 0..{nx - 1}, rows 0..{ny - 1})"
+    crop, desc = crop_case(case, 512, 256)
     s = ref.RefSolver(crop.grid, crop.mech, crop.blocks)
     s.set_state(crop.U, crop.T)
     cells = crop.cells
@@ -157,19 +174,8 @@ def run_reference(args, rank, world):
     case = make_case(args.workload)
     from oracle import ref
     ref.build()
-    g = case.grid
-    if g.n_patches == 0 and g.ndim == 2:
-        nx, ny = min(g.n[0], 512), min(g.n[1], 128)
-        U = np.ascontiguousarray(case.U[:, :, :, :ny, :nx]); T = np.ascontiguousarray(case.T[:, :, :ny, :nx])
-        crop = I.Case(case.name + "_crop", I.Grid(2, (nx, ny, 1), g.dx, g.bc_lo, g.bc_hi), case.mech, U, T, case.cfl, 1)
-        desc = f"{case.name} cropped to {nx}x{ny} cells per step"
-    elif g.n_patches == 0 and g.ndim == 3:
-        n = min(g.n[0], 32)
-        U = np.ascontiguousarray(case.U[:, :, :n, :n, :n]); T = np.ascontiguousarray(case.T[:, :n, :n, :n])
-        crop = I.Case(case.name + "_crop", I.Grid(3, (n, n, n), g.dx, g.bc_lo, g.bc_hi), case.mech, U, T, case.cfl, 1)
-        desc = f"{case.name} cropped to {n}^3 cells per step"
-    else:
-        crop, desc = case, f"{case.name} (whole)"
+    crop, desc = crop_case(case, 512, 128)
+    desc += " per step"
     s = ref.RefSolver(crop.grid, crop.mech, crop.blocks)
     s.set_state(crop.U, crop.T)
     for _ in range(args.warmup):
@@ -192,14 +198,104 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
+def chem_bytes_per_cell(ndim, nvar, ns):
+    # read U (nvar) + T guess, write rho Y_1..ns-1 + T
+    return (nvar + 1 + ns) * 8
+
+
+def measure(binding, case, K, W, local, world, barrier, do_e2e=True):
+    """One workload on this rank's GPU: K timed steps with the state resident in HBM, K profiled steps (per-kernel
+    device time, CUDA events on the library's stream), and (do_e2e) the end-to-end loop with pinned host buffers."""
+    import torch
+    dev = f"cuda:{local}"
+    s = binding.Solver(case.grid, case.mech, case.blocks, device=local)
+    out = {"chem_kernel": s.chem_kernel()}
+    Ud = torch.from_numpy(case.U).to(dev); Td = torch.from_numpy(case.T).to(dev)
+    s.set_state(Ud, Td)
+    for _ in range(W):
+        s.step(1, cfl=case.cfl, sync=False)
+    assert s.status_sync() == 0, "device flag raised during warm-up"
+    l0 = s.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(K):
+        s.step(1, cfl=case.cfl, sync=False)
+    e1.record()
+    barrier()
+    out["ms"] = e0.elapsed_time(e1)
+    out["launches"] = s.launch_count() - l0
+    assert s.status_sync() == 0, "device flag raised during the timed region"
+    phases = {}
+    for _ in range(K):
+        pr = s.profile_step(cfl=case.cfl)
+        for k, (t, n) in pr.items():
+            a = phases.setdefault(k, [0.0, 0]); a[0] += t; a[1] += n
+    out["phases"] = phases
+    if do_e2e:
+        del Ud, Td
+        Uh = torch.from_numpy(case.U).pin_memory(); Th = torch.from_numpy(case.T).pin_memory()
+        Uo = torch.empty_like(Uh).pin_memory()
+        Ke = max(1, min(K, 5))
+        s.set_state(Uh.numpy(), Th.numpy()); s.step(1, cfl=case.cfl, sync=False); s.get_state_into(Uo.numpy())
+        barrier()
+        e0.record()
+        for _ in range(Ke):
+            s.set_state(Uh.numpy(), Th.numpy())
+            s.step(1, cfl=case.cfl, sync=False)
+            rc = s.get_state_into(Uo.numpy())
+        e1.record()
+        barrier()
+        assert rc == 0
+        out["ms_e2e"] = e0.elapsed_time(e1); out["Ke"] = Ke
+        out["h2d"] = int(Uh.numel() * 8 + Th.numel() * 8); out["d2h"] = int(Uo.numel() * 8)
+    s.close()
+    return out
+
+
+def rooflines(case, m, K, dfma, hbm_peak, hbm_src):
+    """Per-kernel roofline entries of one measured workload: algorithmic fp64 instructions and
+    bytes per launch / the kernel's average launch duration (CUDA events, m["phases"]) against the DFMA rate measured
+    in this run and the HBM copy bandwidth of MEASURED_PEAKS.json."""
+    g, cells = case.grid, case.cells
+    nd, nvar, ns = g.ndim, case.nvar, case.mech.ns
+    ph = m["phases"]
+    ent = {}
+    fl_ms, fl_n = ph["flux_rk"]
+    if fl_n:
+        avg = fl_ms / fl_n * 1e-3
+        ops = flux_ops_per_cell_stage(nd, nvar) * cells
+        byt = flux_bytes_per_cell_stage(nd, nvar) * cells
+        ent["flux"] = {"kernel": "k_flux_rk2" if nd == 2 else "k_flux_rk", "bound": "alu", "achieved": ops / avg / 1e12,
+                       "peak": dfma / 1e12, "unit": "T fp64-instr/s (FMA=1)", "frac": ops / avg / dfma,
+                       "traffic": NCU_TRAFFIC_BYTES.get((case.name, "flux")), "avg_launch_ms": avg * 1e3,
+                       "launches_timed": fl_n, "ms_per_step": fl_ms / K,
+                       "hbm": {"achieved": byt / avg / 1e9, "peak": hbm_peak, "unit": "GB/s", "frac": byt / avg / 1e9 / hbm_peak,
+                               "peak_source": hbm_src}}
+    ch_ms, ch_n = ph["chem"]
+    if ch_n:
+        avg = ch_ms / ch_n * 1e-3
+        ops = chem_ops_per_cell(case.mech)
+        byt = chem_bytes_per_cell(nd, nvar, ns) * cells
+        ent["chem"] = {"kernel": "k_chem_jit (%s)" % m["chem_kernel"], "bound": "alu", "ops_per_cell": ops,
+                       "achieved": ops * cells / avg / 1e12, "peak": dfma / 1e12, "unit": "T fp64-instr/s (FMA=1)",
+                       "frac": ops * cells / avg / dfma, "traffic": NCU_TRAFFIC_BYTES.get((case.name, "chem")),
+                       "avg_launch_ms": avg * 1e3, "launches_timed": ch_n, "ms_per_step": ch_ms / K,
+                       "hbm": {"achieved": byt / avg / 1e9, "peak": hbm_peak, "unit": "GB/s", "frac": byt / avg / 1e9 / hbm_peak,
+                               "peak_source": hbm_src}}
+    return ent
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"],
+                    help="headline workload; default = the largest single-GPU config of BASELINE.json (configs[4])")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (N = 1 only)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -220,100 +316,42 @@ def main():
         dist.barrier()
     binding.lib()
 
-    # replicas only (DESIGN.md "Multi-GPU"): every rank advances its own independent problem
-    case = make_case(args.workload, rank)
-    cells = case.cells
-    K, W = args.steps, max(args.warmup, 3)
-    s = binding.Solver(case.grid, case.mech, case.blocks, device=local)
-    chem_kernel = s.chem_kernel()
-    dev = f"cuda:{local}"
-    Ud = torch.from_numpy(case.U).to(dev); Td = torch.from_numpy(case.T).to(dev)
-    s.set_state(Ud, Td)
-    for _ in range(W):
-        s.step(1, cfl=case.cfl, sync=False)
-    assert s.status_sync() == 0, "device flag raised during warm-up"
-
     def barrier():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
             torch.cuda.synchronize()
 
+    # replicas only (DESIGN.md "Multi-GPU"): every rank advances its own independent problem
+    case = make_case(args.workload, rank)
+    K, W = args.steps, max(args.warmup, 3)
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
         sampler.start()
-    # ---- timed region 1: device-resident (inputs already in HBM)
-    l0 = s.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    for _ in range(K):
-        s.step(1, cfl=case.cfl, sync=False)
-    e1.record()
-    barrier()
-    ms = e0.elapsed_time(e1)
-    launches = s.launch_count() - l0
-    assert s.status_sync() == 0, "device flag raised during the timed region"
-
-    # ---- per-kernel-phase device time over K more steps (CUDA events on the library's stream)
-    phases = {}
-    for _ in range(K):
-        pr = s.profile_step(cfl=case.cfl)
-        for k, (t, n) in pr.items():
-            a = phases.setdefault(k, [0.0, 0]); a[0] += t; a[1] += n
-    if sampler:
+    m = measure(binding, case, K, W, local, world, barrier)
+    if sampler:           # clocks are sampled over the event-timed, the per-kernel and the end-to-end regions
         sampler.stop_flag = True
         sampler.join()
-
-    # ---- timed region 2: end to end through the C ABI with HOST buffers (pinned), copies inside
-    Uh = torch.from_numpy(case.U).pin_memory(); Th = torch.from_numpy(case.T).pin_memory()
-    Uo = torch.empty_like(Uh).pin_memory()
-    Ke = max(1, min(K, 5))
-    s.set_state(Uh.numpy(), Th.numpy()); s.step(1, cfl=case.cfl, sync=False); s.get_state_into(Uo.numpy())
-    barrier()
-    e0.record()
-    for _ in range(Ke):
-        s.set_state(Uh.numpy(), Th.numpy())
-        s.step(1, cfl=case.cfl, sync=False)
-        rc = s.get_state_into(Uo.numpy())
-    e1.record()
-    barrier()
-    ms_e2e = e0.elapsed_time(e1)
-    assert rc == 0
-
-    ms, ms_e2e = max_over_ranks([ms, ms_e2e], dev, world)
-    s.close()
+    dev = f"cuda:{local}"
+    ms, ms_e2e = max_over_ranks([m["ms"], m["ms_e2e"]], dev, world)
 
     if rank == 0:
-        g = case.grid
-        nd, nvar = g.ndim, case.nvar
+        cells, nvar = case.cells, case.nvar
         peaks = {}
         try:
             peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
         except Exception:
             pass
         hbm_peak = peaks.get("hbm_gbs", 6650.0)
-        hbm_src = "measured (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback"
+        hbm_src = "measured (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md)"
         dfma = binding.measure_dfma_peak(local)                      # DP instructions/s, measured now
-        # dominant kernel: the fused flux+divergence+RK kernel, 3 launches per step
-        fl_ms, fl_n = phases["flux_rk"]
-        fl_avg = fl_ms / max(fl_n, 1) * 1e-3
-        ops = flux_ops_per_cell_stage(nd, nvar) * cells
-        byt = flux_bytes_per_cell_stage(nd, nvar) * cells
-        roof = {"kernel": "k_flux_rk2" if nd == 2 else "k_flux_rk", "bound": "alu", "achieved": ops / fl_avg / 1e12, "peak": dfma / 1e12,
-                "unit": "T fp64-instr/s (FMA=1)", "frac": ops / fl_avg / dfma, "traffic": NCU_TRAFFIC_BYTES.get(case.name),
-                "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1f_summary.md)",
-                "peak_source": "measured: register-resident DFMA microbenchmark in this run",
-                "avg_launch_ms": fl_avg * 1e3, "launches_timed": fl_n,
-                "hbm": {"achieved": byt / fl_avg / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                        "frac": byt / fl_avg / 1e9 / hbm_peak, "peak_source": hbm_src}}
-        ch_ms, ch_n = phases["chem"]
-        if ch_n > 0:      # the chemistry kernel's achieved FP64 fraction (north_star asks for it)
-            ch_ops = chem_ops_per_cell(case.mech)
-            ch_avg = ch_ms / ch_n * 1e-3
-            roof["chem"] = {"kernel": "k_chem_jit (%s)" % chem_kernel, "bound": "alu", "ops_per_cell": ch_ops,
-                            "achieved": ch_ops * cells / ch_avg / 1e12, "peak": dfma / 1e12, "unit": "T fp64-instr/s (FMA=1)",
-                            "frac": ch_ops * cells / ch_avg / dfma, "avg_launch_ms": ch_avg * 1e3}
+        ent = rooflines(case, m, K, dfma, hbm_peak, hbm_src)
+        # the dominant kernel of the step = the one with the most device time per step
+        dom = max(ent, key=lambda k: ent[k]["ms_per_step"])
+        roof = dict(ent[dom])
+        roof["traffic_unit"] = NCU_TRAFFIC_SOURCE
+        roof["peak_source"] = "measured: register-resident DFMA microbenchmark in this run"
+        roof["kernels"] = {k: v for k, v in ent.items() if k != dom}
         line = {"metric": METRIC, "value": cells * world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
                 "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
@@ -322,13 +360,36 @@ def main():
                            "l2": "state %.0f MB per register > 126 MB L2" % (cells * nvar * 8 / 1e6)
                                  if cells * nvar * 8 > 126e6 else "state fits L2 (no flush; noted)"},
                 "clocks": sampler.summary(),
-                "e2e": {"value": cells * world * Ke / (ms_e2e * 1e-3), "unit": UNIT,
-                        "h2d_bytes_per_step": int(Uh.numel() * 8 + Th.numel() * 8), "d2h_bytes_per_step": int(Uo.numel() * 8),
-                        "steps": Ke},
-                "gpu_launches": int(launches),
+                "e2e": {"value": cells * world * m["Ke"] / (ms_e2e * 1e-3), "unit": UNIT,
+                        "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"], "steps": m["Ke"]},
+                "gpu_launches": int(m["launches"]),
                 "roofline": roof,
-                "phases_ms_per_step": {k: v[0] / K for k, v in phases.items()},
+                "phases_ms_per_step": {k: v[0] / K for k, v in m["phases"].items()},
                 "context": {"paper_a100_cell_updates_per_s": 2.0e7, "note": "PAPER.md:448, other hardware and mechanism"}}
+        if world == 1 and not args.no_per_config:
+            # every BASELINE config at full size on this GPU (north_star: "throughput per config")
+            per = {}
+            for wl in ("cfg0", "cfg1", "cfg2", "cfg3", "cfg4"):
+                if wl == args.workload:
+                    c2, m2, K2 = case, m, K
+                else:
+                    c2 = make_case(wl, rank)
+                    K2 = K
+                    m2 = measure(binding, c2, K2, W, local, world, barrier, do_e2e=False)
+                e2 = rooflines(c2, m2, K2, dfma, hbm_peak, hbm_src)
+                step_ms = m2["ms"] / K2
+                algo_bytes = (3 * ((c2.nvar + 3 + c2.grid.ndim) * 8 + flux_bytes_per_cell_stage(c2.grid.ndim, c2.nvar))
+                              + chem_bytes_per_cell(c2.grid.ndim, c2.nvar, c2.mech.ns)) * c2.cells
+                per[wl] = {"workload": c2.name, "cells": c2.cells, "value": c2.cells * K2 / (m2["ms"] * 1e-3),
+                           "ms_per_step": step_ms, "gpu_launches_per_step": m2["launches"] / K2,
+                           "phases_ms_per_step": {k: v[0] / K2 for k, v in m2["phases"].items()},
+                           "flux": {k: e2["flux"][k] for k in ("kernel", "frac", "avg_launch_ms", "traffic")} if "flux" in e2 else None,
+                           "flux_hbm_frac": e2["flux"]["hbm"]["frac"] if "flux" in e2 else None,
+                           "chem": {k: e2["chem"][k] for k in ("kernel", "frac", "avg_launch_ms", "traffic")} if "chem" in e2 else None,
+                           "hbm": {"achieved": algo_bytes / (step_ms * 1e-3) / 1e9, "frac": algo_bytes / (step_ms * 1e-3) / 1e9 / hbm_peak,
+                                   "unit": "GB/s", "note": "algorithmic bytes of the whole step / step time"}}
+                del c2
+            line["per_config"] = per
         if not args.no_cpu_baseline and world >= 1:
             cb, _, _ = oracle_throughput(case)
             line["cpu_baseline"] = cb
