@@ -80,7 +80,9 @@ int janc_create(const janc_grid *grid, int device, void *cuda_stream, janc_ctx *
  *   "jit"              "1" (default) | "0"   mechanism-specialised kernels compiled with NVRTC | table-driven kernels
  *   "jit_max_unknowns" integer (default 12)  largest ns-1 of the one-thread-per-cell specialised chemistry kernel
  *   "jit_big"          "roles" (default) | "smem"   kernel for larger mechanisms
- *   "roles"            "8" (default) | "16"  role-warps per CTA of the role-warp chemistry kernel */
+ *   "roles"            "8" (default) | "16"  role-warps per CTA of the role-warp chemistry kernel
+ *   "roles_lu"         "rows" (default) | "columns"  its linear solve: LU with one row per lane inside a warp |
+ *                      column-distributed Gauss-Jordan across the role warps */
 int janc_set_option(janc_ctx *, const char *key, const char *value);
 
 /* Mechanism must be set before the workspace is sized (nvar depends on ns).  A rejected mechanism (JANC_EINVAL) leaves

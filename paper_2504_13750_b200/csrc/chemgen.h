@@ -87,7 +87,7 @@ inline std::string xprod(const std::string &pre, const int *cnt, int ns, int ski
 //           denormal pivot gives inf / nan, which the callers' isfinite checks flag).
 inline void emit_math(std::string &src, bool estrin = false) {
   src += "__device__ __forceinline__ double exp_nb(double x) {\n"
-         "  x = fmin(fmax(x, -708.0), 709.0);\n"
+         "  x = x < -708.0 ? -708.0 : (x > 709.0 ? 709.0 : x);     // two compares + selects (fmin / fmax carry NaN handling)\n"
          "  const double t = fma(x, 1.4426950408889634, 6755399441055744.0);\n"
          "  const int n = __double2loint(t);\n"
          "  const double nf = t - 6755399441055744.0;\n"

@@ -40,9 +40,14 @@ namespace chemgen {
 // before any function of this header is called.
 inline int &roles_nr_ref() { static thread_local int v = 8; return v; }
 inline int roles_nr() { return roles_nr_ref(); }
+// elimination variant (janc_set_option "roles_lu"): true = the system is transposed through shared memory and
+// factorised with one ROW per lane inside a warp (no inter-warp synchronisation), false = the column-distributed
+// Gauss-Jordan across the role warps
+inline bool &roles_lu_rows_ref() { static thread_local bool v = true; return v; }
 
 struct RolesLayout {
-  int oX, oP, oN, oRN, oDL, oRHS, oF, oPIV, oIP, oXS, oNX, oR, rows;   // offsets in rows of 32 doubles
+  int oX, oP, oN, oRN, oDL, oRHS, oF, oPIV, oIP, oXS, oNX, oR, oPB, rows;   // offsets in rows of 32 doubles
+  int rstr, pbs;                                                   // row-LU: row stride of the transposed system, pivot-row buffer stride per cell (doubles)
   size_t ntd, nti;                                                 // table sizes (doubles, ints) behind the rows
   size_t smem() const { return (size_t)rows * 32 * sizeof(double) + ntd * sizeof(double) + nti * sizeof(int); }
 };
@@ -90,8 +95,15 @@ inline RolesLayout roles_layout(const MechC &M, int ndim) {
   L.oNX = o; o += ndim + 2 + n1 + 1;         // U (nvar rows) and T of the NEXT turn's cells, prefetched with cp.async
   // one region, three lives: M k_f, M k_b, q per reaction (until the assembly barrier); the multipliers of every
   // column (elimination: nothing is reused, so the roles may run several columns apart); the whole system (slow path)
-  L.oR = o; o += std::max(3 * nr, n1 * (n1 + 1));
+  // row-LU: the system transposed to [row][column][cell] with the row stride padded so that the lanes of a half-warp
+  // (16 / NR cells x NR rows) read 16 distinct 8-byte banks
+  L.rstr = (n1 + 1) * 32 + 16 / roles_nr();
+  { int usz = 0; for (int c = 0; c < n1; c++) usz += (n1 + 1 - c + 1) / 2 * 2;   // triangular U store per cell, even row lengths,
+    L.pbs = usz + (n1 + 2) / 2 * 2 + 4; }                                          // + the overrun of fixed-length row writes
+
+  L.oR = o; o += std::max(std::max(3 * nr, n1 * (n1 + 1)), roles_lu_rows_ref() ? (n1 * L.rstr + 31) / 32 : 0);
   L.oF = L.oR;
+  L.oPB = o; if (roles_lu_rows_ref()) o += L.pbs;                        // U store: pbs doubles per cell x 32 cells
   L.rows = o;
   L.ntd = roles_table_doubles(M);
   L.nti = roles_table_ints(M);
@@ -112,8 +124,9 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   std::vector<std::vector<int>> cf(nr, std::vector<int>(ns, 0)), cb(nr, std::vector<int>(ns, 0)), dnu(nr, std::vector<int>(ns, 0));
   const RolesDims DM = roles_dims(M);
   const int maxof = DM.maxof, maxob = DM.maxob;
-  bool any_rev = false;
+  bool any_rev = false, all_rev = true;
   for (int i = 0; i < nr; i++) {
+    if (!M.rev[i]) all_rev = false;
     for (int e = 0; e < M.nreac[i]; e++) cf[i][M.reac[i][e]]++;
     for (int e = 0; e < M.nprod[i]; e++) cb[i][M.prod[i][e]]++;
     for (int k = 0; k < ns; k++) dnu[i][k] = cb[i][k] - cf[i][k];
@@ -192,6 +205,8 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   // =========================================================================== kernel
   src += "#define SM(r) sm_[(r) * 32 + lane]\n";
   src += "#define BAR() asm volatile(\"bar.sync 0;\" ::: \"memory\")\n";
+  src += "#define PST2(p, a, x, y) asm volatile(\"{ .reg .pred q; setp.ne.s32 q, %0, 0; @q st.shared.v2.f64 [%1], {%2, %3}; }\" :: \"r\"(p), \"r\"(a), \"d\"(x), \"d\"(y) : \"memory\")\n";
+  src += "#define PST1(p, a, x) asm volatile(\"{ .reg .pred q; setp.ne.s32 q, %0, 0; @q st.shared.f64 [%1], %2; }\" :: \"r\"(p), \"r\"(a), \"d\"(x) : \"memory\")\n";
   src += "#define AWAIT(id) asm volatile(\"barrier.sync %0, " + I(NR * 32) + ";\" :: \"r\"(id) : \"memory\")\n";
   src += "#define PUBLISH(id) do { asm volatile(\"barrier.arrive %0, " + I(NR * 32) + ";\" :: \"r\"(id) : \"memory\"); } while (0)\n";
   // the next turn's inputs: (nvar + 1) x 32 doubles, one 8-byte cp.async each, spread over the CTA
@@ -302,7 +317,10 @@ inline std::string generate_roles(const MechC &M, int ndim) {
         for (int q = NKB - 2; q >= 3; q--) pol = "fma(T, " + pol + ", d" + S + "[" + I(q) + "])";
         lk = "fma(T, " + pol + ", " + lk + ")";
       }
-      E.line("    const double kb" + S + " = (c_fl[i" + S + "] & 1) ? exp_nb(" + lk + ") : 0.0;");
+      // branch-free (a branch per reaction keeps the compiler from interleaving the exponential chains of the
+      // reactions of one trip): irreversible reactions multiply a finite exponential by zero
+      if (all_rev) E.line("    const double kb" + S + " = exp_nb(" + lk + ");");
+      else E.line("    const double kb" + S + " = exp_nb(" + lk + ") * (double)(c_fl[i" + S + "] & 1);");
     } else {
       E.line("    const double kb" + S + " = 0.0;");
     }
@@ -313,9 +331,14 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     if (tb) {
       E.line("    const int tb_ = (c_fl[i" + S + "] >> 1) - 1;");
       E.line("    const double *ef = c_eff + tb_ * " + I(ns) + ";");
-      E.line("    double Mi = ef[0] * SM(" + I(L.oX) + ");");
-      E.line("    #pragma unroll");
-      E.line("    for (int j = 1; j < " + I(ns) + "; j++) Mi = fma(ef[j], SM(" + I(L.oX) + " + j), Mi);");
+      // four partial sums: the ns-term chain of dependent FMAs would be the longest path of the trip
+      E.line("    double Mi, Mi1 = 0.0, Mi2 = 0.0, Mi3 = 0.0;");
+      E.line("    Mi = ef[0] * SM(" + I(L.oX) + ");");
+      for (int j = 1; j < ns; j++) {
+        const std::string acc = (j % 4 == 0) ? "Mi" : "Mi" + I(j % 4);
+        E.line("    " + acc + " = fma(ef[" + I(j) + "], SM(" + I(L.oX + j) + "), " + acc + ");");
+      }
+      E.line("    Mi = (Mi + Mi1) + (Mi2 + Mi3);");
       E.line("    SM(" + I(L.oRN) + " + tb_) = rn" + S + ";");
       E.line("    SM(" + I(L.oR) + " + i" + S + ") = Mi * kf" + S + "; SM(" + I(L.oR + nr) + " + i" + S + ") = Mi * kb" + S + "; SM(" + I(L.oR + 2 * nr) + " + i" + S + ") = Mi * rn" + S + ";");
     } else {
@@ -393,11 +416,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
         const std::string cfs = row(L.oR + i), cbs = row(L.oR + nr + i);
         if (cf[i][j] > 0) dq = (cf[i][j] > 1 ? num((double)cf[i][j]) + " * " : std::string("")) + xprod(cfs, cf[i].data(), ns, j);
         if (rev && cb[i][j] > 0) dq += (dq.empty() ? "-" : " - ") + (cb[i][j] > 1 ? num((double)cb[i][j]) + " * " : std::string("")) + xprod(cbs, cb[i].data(), ns, j);
-        if (tb) {
-          const double a = M.eff[M.tbi[i]][j];
-          const std::string rn = row(L.oRN + M.tbi[i]);
-          if (a != 0.0) dq = dq.empty() ? num(a) + " * " + rn : "fma(" + num(a) + ", " + rn + ", " + dq + ")";
-        }
+        (void)tb;     // the efficiency term a_ij r_i of a third-body reaction touches every column: shared code below
         if (dq.empty()) continue;
         bool any = false;
         for (int k = 0; k < n1; k++) any = any || dnu[i][k] != 0;
@@ -412,11 +431,39 @@ inline std::string generate_roles(const MechC &M, int ndim) {
         }
         E.line("  }");
       }
-      if (j == n1)
-        for (int k = 0; k < n1; k++) E.line("  " + row(L.oDL + k) + " = " + A(s, k) + " * " + num(M.invW[n1]) + ";");
     }
     E.line("} break;");
   }
+  E.line("}");
+  // ---- third-body efficiencies (eq 4.7): D_kj += dnu_ik a_ij r_i for EVERY column j.  The same code for every role
+  //      (a_ij comes from the table, indexed by the role's columns), so its instructions are fetched once for the
+  //      eight warps: role-specific straight-line code streams from L2 at well under one instruction per clock.
+  if (M.ntb > 0) {
+    E.line("{");
+    for (int s = 0; s < NSL; s++)
+      E.line("  const double *ef" + I(s) + " = c_eff + (k" + I(s) + " <= " + I(n1) + " ? k" + I(s) + " : 0);");
+    for (int i = 0; i < nr; i++) {
+      if (!M.tb[i]) continue;
+      bool any = false;
+      for (int k = 0; k < n1; k++) any = any || dnu[i][k] != 0;
+      if (!any) continue;
+      const int q = M.tbi[i];
+      E.line("  { const double rn = " + row(L.oRN + q) + ";");
+      for (int s = 0; s < NSL; s++) E.line("    const double t" + I(s) + " = ef" + I(s) + "[" + I(q * ns) + "] * rn;");
+      for (int k = 0; k < n1; k++) {
+        if (dnu[i][k] == 0) continue;
+        for (int s = 0; s < NSL; s++) {
+          if (dnu[i][k] == 1) E.line("    " + A(s, k) + " += t" + I(s) + ";");
+          else if (dnu[i][k] == -1) E.line("    " + A(s, k) + " -= t" + I(s) + ";");
+          else E.line("    " + A(s, k) + " = fma(" + num((double)dnu[i][k]) + ", t" + I(s) + ", " + A(s, k) + ");");
+        }
+      }
+      E.line("  }");
+    }
+    E.line("}");
+  }
+  E.line("if (w == " + I(wN) + ") {");
+  for (int k = 0; k < n1; k++) E.line("  " + row(L.oDL + k) + " = " + A(sN, k) + " * " + num(M.invW[n1]) + ";");
   E.line("}");
   E.line("BAR();");
   // ---- A = I - dt J,  J_kl = W_k (D_kl / W_l - D_kN / W_N);  column N becomes rhs = dt W_k wdot_k  (eq 4.12-4.13, A11)
@@ -435,6 +482,211 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     }
   }
   E.line("}");
+  if (roles_lu_rows_ref()) {
+  // ---- LU with one ROW per lane.  The columns the roles assembled are transposed through shared memory
+  //      ([row][column][cell]); then NR adjacent lanes of a warp own one cell: lane group index g_ holds rows g_, g_ + NR,
+  //      ... (n1 + 1 entries each, in registers, static indices: the column loop is unrolled).  Step c: the lanes that
+  //      hold row c publish its entries c..n1 to a small per-cell buffer, everybody reads them back (broadcast), rows
+  //      below take  a_rj -= (a_rc / a_cc) a_cj.  A warp owns its 32 / NR cells from here to the solution: no barrier,
+  //      no named barrier, only __syncwarp.  Fast path = no row swap needed (the diagonal entry is the first row of
+  //      maximal |a_rc|, r >= c: the oracle's rule); if any cell of the CTA needs one, the system -- still untouched in
+  //      shared memory -- is solved by the generic pivoted loop below.
+  const int RS = (n1 + NR - 1) / NR;                                   // row slots per lane
+  const int NC1 = n1 + 1;
+  auto R = [](int t, int j) { return "R" + I(t) + "_" + I(j); };
+  // transposed store of the columns this role assembled
+  E.line("{");
+  for (int s = 0; s < NSL; s++) {
+    E.line("  if (k" + I(s) + " <= " + I(n1) + ") { double *mt_ = sm_ + " + I(L.oR * 32) + " + k" + I(s) + " * 32 + lane;");
+    for (int k = 0; k < n1; k++) E.line("    mt_[" + I(k * L.rstr) + "] = " + A(s, k) + ";");
+    E.line("  }");
+  }
+  E.line("}");
+  E.line("BAR();");
+  // The column loop is ROLLED (the whole kernel has to stay close to the 32 KB instruction cache: straight-line code
+  // streams from L2 at half an instruction per clock): after step c every row drops its column c, i.e. the update
+  // writes column j into register j - 1, so the pivot column is always physical column 0 and the body is the same for
+  // every c.  A row that has served as pivot row is frozen in shared memory (U store, triangular, per cell), where the
+  // back-substitution reads it; its registers shift on as dead values.  The loop is cut into phases with fewer
+  // physical columns and fewer live row slots.
+  E.line("int bad = 0;");
+  E.line("{");
+  E.line("  const int g_ = threadIdx.x % " + I(NR) + ", cell_ = threadIdx.x / " + I(NR) + ";");
+  E.line("  const double *mr_ = sm_ + " + I(L.oR * 32) + " + g_ * " + I(L.rstr) + " + cell_;");
+  E.line("  double *us_ = sm_ + " + I(L.oPB * 32) + " + cell_ * " + I(L.pbs) + ";     // U rows of this cell, row c at uoff(c)");
+  for (int t = 0; t < RS; t++) {
+    const bool part = NR * t + NR - 1 >= n1;                           // some lanes of this slot hold no row: zeros
+    for (int j = 0; j < NC1; j++)
+      E.line("  double " + R(t, j) + " = " + (part ? "g_ + " + I(NR * t) + " < " + I(n1) + " ? " : std::string("")) +
+             "mr_[" + I(NR * t * L.rstr + j * 32) + "]" + (part ? " : 0.0" : "") + ";");
+  }
+  {
+    std::string d = "  double ";
+    for (int t = 0; t < RS; t++) d += "IP" + I(t) + " = 0.0, XS" + I(t) + " = 0.0" + (t + 1 < RS ? ", " : ";");
+    E.line(d);
+  }
+  // The loop is software-pipelined: step c first updates the slot that holds row c + 1, publishes that row (with the
+  // reciprocal of its diagonal entry, computed while the rest of the row is still being updated) and issues the loads of
+  // step c + 1; the other slots are updated behind it, so the store -> load -> multiply chain of the next step is off
+  // the critical path.  Two register sets (qa / qb) alternate; the loop body is two steps.
+  // Phases [cs, ce): constant slot of the pivot row, constant slot of the next pivot row, constant set of live slots,
+  // ncols = NC1 - cs physical columns.
+  std::vector<int> cuts;
+  {
+    std::vector<char> cut(n1 + 1, 0);
+    cut[0] = cut[n1] = 1;
+    for (int t = 0; t < RS; t++) {
+      if (NR * t < n1) cut[NR * t] = 1;                                // pivot slot changes
+      if (NR * t + NR - 1 < n1) cut[NR * t + NR - 1] = 1;              // next-pivot slot changes, slot t goes dead
+    }
+    int last = 0;
+    for (int c = 1; c <= n1; c++) {
+      if (!cut[c]) continue;
+      if (c - last >= 6) { int mid = last + (c - last) / 2; mid -= (mid - last) % 2; cut[mid] = 1; }   // fewer columns in the second half
+      last = c;
+    }
+    for (int c = 0; c <= n1; c++) if (cut[c]) cuts.push_back(c);
+  }
+  {
+    std::string d = "  double2 ";
+    for (int j = 0; j < NC1; j += 2) d += "qa" + I(j) + ", qb" + I(j) + (j + 2 < NC1 ? ", " : ";");
+    E.line(d);
+    E.line("  double ipa, ipb;");
+  }
+  auto Q = [&](int b, int j) { return std::string(b ? "qb" : "qa") + I(j & ~1) + ((j & 1) ? ".y" : ".x"); };
+  auto IPB = [&](int b) { return std::string(b ? "ipb" : "ipa"); };
+  const int ipoff = L.pbs - 2;
+  // publish row `cx` (held in slot t, nv valid entries) from the lanes g_ == cx % NR: predicated stores (inline PTX; as
+  // an `if` the compiler branches around them and sinks the reciprocal's Newton steps into the branch, where nothing
+  // overlaps them), then -- after whatever the caller puts in between -- the loads into register set b
+  auto publish = [&](const std::string &cx, int t, int nv, const std::string &ind) {
+    const int nv2 = (nv + 1) / 2 * 2;
+    E.line(ind + "{ const unsigned ua_ = (unsigned)__cvta_generic_to_shared(us_ + uo_);");
+    E.line(ind + "  const double ipn_ = rcp_nb(" + R(t, 0) + ");");
+    E.line(ind + "  const int own_ = g_ == (" + cx + ") % " + I(NR) + ";");
+    for (int j = 0; j < nv2; j += 2)
+      E.line(ind + "  PST2(own_, ua_ + " + I(j * 8) + ", " + R(t, j) + ", " + (j + 1 < nv ? R(t, j + 1) : std::string("0.0")) + ");");
+    E.line(ind + "  PST1(own_, (unsigned)__cvta_generic_to_shared(us_ + " + I(ipoff) + " + ((" + cx + ") & 1)), ipn_);");
+    E.line(ind + "}");
+  };
+  auto load = [&](const std::string &cx, int b, int nv, const std::string &ind) {
+    const int nv2 = (nv + 1) / 2 * 2;
+    E.line(ind + "__syncwarp();");
+    E.line(ind + "{ const double *ur_ = us_ + uo_;");
+    for (int j = 0; j < nv2; j += 2) E.line(ind + "  " + std::string(b ? "qb" : "qa") + I(j) + " = *(const double2 *)(ur_ + " + I(j) + ");");
+    E.line(ind + "  " + IPB(b) + " = us_[" + I(ipoff) + " + ((" + cx + ") & 1)];");
+    E.line(ind + "}");
+  };
+  auto update_slot = [&](const std::string &cx, int t, int b, int ncols, const std::string &ind) {
+    E.line(ind + "{ const bool act = g_ + " + I(NR * t) + " > " + cx + "; const double l_ = act ? " + R(t, 0) + " * " + IPB(b) + " : 0.0;");
+    E.line(ind + "  bad |= (int)(act & (fabs(" + R(t, 0) + ") > fabs(" + Q(b, 0) + ")));");
+    for (int j = 1; j < ncols; j++) E.line(ind + "  " + R(t, j - 1) + " = fma(-l_, " + Q(b, j) + ", " + R(t, j) + ");");
+    E.line(ind + "}");
+  };
+  // one elimination step with the pivot row in register set b; the next row goes to set 1 - b
+  auto step = [&](const std::string &cx, int cs, int ce, int b, bool has_next, const std::string &ind) {
+    const int ncols = NC1 - cs, t0 = cs / NR, t1 = (cs + 1) / NR < RS ? (cs + 1) / NR : RS - 1;
+    (void)ce;
+    E.line(ind + "uo_ += ((" + I(NC1) + " - (" + cx + ") + 1) >> 1) << 1;     // offset of row c + 1 (row lengths rounded up to even)");
+    // slots other than the next pivot row's: the first one goes between the publishing stores' operands (the
+    // reciprocal chain) and the stores' consumers, the rest behind the loads of the next row
+    std::vector<int> others;
+    for (int t = 0; t < RS; t++) {
+      if (NR * t + NR - 1 <= cs) continue;                             // every row of the slot is <= c throughout the phase
+      if (has_next && t == t1) continue;
+      others.push_back(t);
+    }
+    size_t done = 0;
+    if (has_next) {
+      update_slot(cx, t1, b, ncols, ind);
+      publish("(" + cx + ") + 1", t1, ncols - 1, ind);
+      if (others.size() > 1) update_slot(cx, others[done++], b, ncols, ind);
+      load("(" + cx + ") + 1", 1 - b, ncols - 1, ind);
+    }
+    E.line(ind + "bad |= !(fabs(" + Q(b, 0) + ") > 0.0);");
+    E.line(ind + "if (g_ == (" + cx + ") % " + I(NR) + ") IP" + I(t0) + " = " + IPB(b) + ";");
+    for (; done < others.size(); done++) update_slot(cx, others[done], b, ncols, ind);
+  };
+  E.line("  int uo_ = 0;");
+  publish("0", 0, NC1, "  ");
+  load("0", 0, NC1, "  ");
+  int cur = 0;                                                         // register set that holds the pivot row at the phase start
+  for (size_t ph = 0; ph + 1 < cuts.size(); ph++) {
+    const int cs = cuts[ph], ce = cuts[ph + 1];
+    if (cs >= ce) continue;
+    const int npair = (ce - cs) / 2;
+    const bool last_phase = ce == n1;
+    // the very last step (c = n1 - 1) has no next row: keep it out of the paired loop
+    int pairs = npair, rem = (ce - cs) % 2;
+    if (last_phase && rem == 0) { pairs -= 1; rem = 2; }
+    if (pairs > 0) {
+      E.line("  #pragma unroll 1");
+      E.line("  for (int c = " + I(cs) + "; c < " + I(cs + 2 * pairs) + "; c += 2) {");
+      step("c", cs, ce, cur, true, "    ");
+      step("c + 1", cs, ce, 1 - cur, true, "    ");
+      E.line("  }");
+    }
+    int c = cs + 2 * pairs;
+    for (; c < ce; c++) {
+      step(I(c), cs, ce, cur, c + 1 < n1, "  ");
+      cur = 1 - cur;
+    }
+  }
+  // back-substitution from the U store: row r holds u_r,r .. u_r,n1-1, rhs_r at ur(r)[0 .. n1 - r]
+  E.line("  bool okx = true;");
+  {
+    // offset of row r: sum_{i<r} roundup_even(NC1 - i)
+    const std::string odd = (NC1 % 2 == 0) ? "(r >> 1)" : "((r + 1) >> 1)";
+    E.line("  auto uoff = [](int r) { return r * " + I(NC1) + " - ((r * (r - 1)) >> 1) + " + odd + "; };");
+  }
+  for (int t = 0; t < RS; t++) {
+    E.line("  const int r" + I(t) + " = g_ + " + I(NR * t) + ", o" + I(t) + " = uoff(r" + I(t) + " < " + I(n1) + " ? r" + I(t) + " : 0);");
+    E.line("  double Y" + I(t) + " = r" + I(t) + " < " + I(n1) + " ? us_[o" + I(t) + " + " + I(n1) + " - r" + I(t) + "] : 0.0;");
+  }
+  // one loop per row slot of the pivot row (the slot index is then static: no selects)
+  for (int t = 0; t < RS; t++) E.line("  const double *p" + I(t) + " = us_ + o" + I(t) + " - r" + I(t) + ";     // u_r,c of this lane's row at p[c]");
+  for (int to = RS - 1; to >= 0; to--) {
+    const int chi = std::min(n1 - 1, NR * to + NR - 1), clo = NR * to;
+    E.line("  #pragma unroll 1");
+    E.line("  for (int c = " + I(chi) + "; c >= " + I(clo) + "; c--) {");
+    E.line("    const int go = c - " + I(clo) + ";");
+    E.line("    double x_ = Y" + I(to) + " * IP" + I(to) + ";");
+    E.line("    x_ = __shfl_sync(0xffffffffu, x_, (lane & " + I(~(NR - 1) & 31) + ") | go);");
+    E.line("    if (g_ == go) XS" + I(to) + " = x_;");
+    for (int t = 0; t <= to; t++)                                        // rows of higher slots are all > c
+      E.line("    if (r" + I(t) + " < c) Y" + I(t) + " = fma(-p" + I(t) + "[c], x_, Y" + I(t) + ");");
+    E.line("  }");
+  }
+  for (int t = 0; t < RS; t++)
+    E.line("  if (r" + I(t) + " < " + I(n1) + ") { if (!isfinite(XS" + I(t) + ")) okx = false; sm_[(" + I(L.oXS) + " + r" + I(t) + ") * 32 + cell_] = XS" + I(t) + "; }");
+  E.line("  if (!okx) bad |= 2;     // non-finite solution: let the pivoted path decide (it raises the flag)");
+  E.line("}");
+  E.line("if (__syncthreads_or(bad)) {");
+  // ---- slow path: generic partial pivoting on the untouched system in shared memory (lane = cell, roles split the columns)
+  E.line("  #define SMA(r, c) sm_[" + I(L.oR * 32) + " + (r) * " + I(L.rstr) + " + (c) * 32 + lane]");
+  E.line("  #pragma unroll 1");
+  E.line("  for (int c = 0; c < " + I(n1) + "; c++) {");
+  E.line("    int piv = c; double best = fabs(SMA(c, c));");
+  E.line("    for (int r = c + 1; r < " + I(n1) + "; r++) { const double v = fabs(SMA(r, c)); if (v > best) { best = v; piv = r; } }");
+  E.line("    if (!(best > 0.0)) ok = false;");
+  E.line("    BAR();   // every role has chosen the pivot of column c before anyone swaps it");
+  for (int s = 0; s < NSL; s++)
+    E.line("    if (k" + I(s) + " >= c && k" + I(s) + " <= " + I(n1) + " && piv != c) { const double x_ = SMA(c, k" + I(s) + "); SMA(c, k" + I(s) + ") = SMA(piv, k" + I(s) + "); SMA(piv, k" + I(s) + ") = x_; }");
+  E.line("    BAR();");
+  E.line("    const double ip = 1.0 / SMA(c, c);     // column c is not written by the sweep below (only columns > c)");
+  for (int s = 0; s < NSL; s++) {
+    E.line("    if (k" + I(s) + " > c && k" + I(s) + " <= " + I(n1) + ") { const double pj = SMA(c, k" + I(s) + ");");
+    E.line("      for (int r = 0; r < " + I(n1) + "; r++) if (r != c) SMA(r, k" + I(s) + ") = fma(-(SMA(r, c) * ip), pj, SMA(r, k" + I(s) + ")); }");
+  }
+  E.line("    if (w == 0) SM(" + I(L.oIP) + " + c) = ip;");
+  E.line("    BAR();");
+  E.line("  }");
+  E.line("  if (w == " + I(wN) + ") {");
+  E.line("    for (int k = 0; k < " + I(n1) + "; k++) { const double x_ = SMA(k, " + I(n1) + ") * SM(" + I(L.oIP) + " + k); if (!isfinite(x_)) ok = false; SM(" + I(L.oXS) + " + k) = x_; }");
+  E.line("  }");
+  E.line("  #undef SMA");
+  E.line("}");
+  } else {
   // ---- Gauss-Jordan elimination, column-distributed, one-column look-ahead (see the header); L is not kept: the
   //      right-hand side is column n1 of the system.  The column loop is a real loop (compact code, warm in the
   //      instruction cache): the update writes row p + 1 into row p, so the pivot row is always physical row 0
@@ -532,6 +784,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("  }");
   E.line("  #undef SMA");
   E.line("}");
+  }
   E.line("BAR();");
   for (int s = 0; s < NSL; s++)
     E.line("if (live && k" + I(s) + " < " + I(n1) + ") Up[(long long)(" + I(ndim + 2) + " + k" + I(s) + ") * a.pc] = ry" + I(s) +
@@ -540,7 +793,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("asm volatile(\"cp.async.wait_all;\" ::: \"memory\");");
   E.line("BAR();   // shared rows are reused by the next turn; the prefetched inputs are visible to every role");
   E.line("}");
-  src += "}\n#undef SM\n#undef BAR\n#undef AWAIT\n#undef PUBLISH\n";
+  src += "}\n#undef PST2\n#undef PST1\n#undef SM\n#undef BAR\n#undef AWAIT\n#undef PUBLISH\n";
   return src;
 }
 
