@@ -168,7 +168,7 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
       const double *ux = P.vel + pbase;
       // advected components (no pressure term) are staged by their own loop: no p load, 3-instruction split flux
       auto stage_x = [&](auto gen) {
-#pragma unroll 4
+#pragma unroll 12
         for (int it = tid; it < C::ROWS * (TX + 6); it += NT) {
           const int xi = it % (TX + 6), r = it / (TX + 6);
           const int gx = min(o0 + xi - 3, mx0), gy = min(o1 + r % TY, in1), gz = min(o2 + r / TY, in2);
@@ -199,7 +199,7 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
       const double al = alpha[d];
       const int EY = d == 1 ? TY + 6 : TY, EZ = d == 2 ? TZ + 6 : TZ;     // staged extent
       auto stage_d = [&](auto gen) {
-#pragma unroll 4
+#pragma unroll 12
         for (int it = tid; it < TX * EY * EZ; it += NT) {
           const int x = it % TX, yy = (it / TX) % EY, zz = it / (TX * EY);
           const int gx = min(o0 + x, P.n[0] - 1);
