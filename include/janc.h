@@ -74,6 +74,8 @@ int janc_create(const janc_grid *grid, int device, void *cuda_stream, janc_ctx *
 /* Options, as text (key, value); JANC_EINVAL for an unknown key or value.  The product runs the defaults; the other
  * values exist so that tests can reach every kernel and every host path without environment variables.
  *   "graph"            "1" (default) | "0"   replay one captured CUDA graph per step | eager launches
+ *   "tma"              "1" (default) | "0"   2-D grids above 600 k cells with an even padded width: tiles staged with
+ *                      cp.async.bulk.tensor (TMA) | with 8-byte cp.async
  *   "halo"             "auto" (default) | "ghost"   auto: 2-D patches of <= 16 x 16 cells and 2-D grids below 600 k cells
  *                      gather their halo inside the flux kernel; ghost: k_ghost always materialises the ghost layers
  * and, only before janc_set_mechanism (JANC_ESTATE afterwards), the kernel selection of that call:

@@ -442,3 +442,144 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
     cp_async_commit();
   }
 }
+
+// ------------------------------------------------------------------------------------------------
+// TMA variant of the 2-D kernel (uniform grids and patches with materialised ghosts): the tile + 3 ghost layers of
+// p, u, v and of every component U_m arrive as ONE cp.async.bulk.tensor box each (a 3-D tensor map {Px, Py, fields}
+// over the padded arrays; a box that sticks out of the array is zero-filled, and only cells outside the grid ever see
+// those zeros), signalled through an mbarrier.  The box is dense (pitch = TX + 6 doubles): the per-element index math
+// of the cp.async loads (a fifth of the kernel's instructions) disappears, in exchange x pencils (lanes = rows) read
+// with a 2-way bank conflict.  Requires an even padded width (global strides are multiples of 16 bytes).
+#include <cuda.h>
+
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
+  asm volatile("mbarrier.init.shared.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+  asm volatile(
+      "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n" ::"r"(
+          (unsigned)__cvta_generic_to_shared(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(double *dst, const CUtensorMap *map, unsigned long long *bar, int x, int y, int z) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(dst)),
+               "l"(map), "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(x), "r"(y), "r"(z)
+               : "memory");
+}
+
+template <int TX, int TY, int SEG>
+struct Flux2TmaCfg {
+  static constexpr int NT = TX * TY / SEG;
+  static constexpr int BX = TX + 6, BY = TY + 6;
+  static constexpr int PIT = BX;                                          // dense box
+  static constexpr int BOX = (BX * BY * 8 + 127) / 128 * 16;              // doubles, padded to 128 bytes
+  static constexpr int LP = TX | 1;
+  static constexpr unsigned BOX_BYTES = BX * BY * 8;
+  static constexpr size_t SMEM = (size_t)(5 * BOX + TY * LP) * sizeof(double) + 64;
+  static constexpr int MINB = NT >= 128 ? 3 : 512 / NT;                   // resident CTAs the register allocation aims at
+  static_assert(TX % SEG == 0 && TY % SEG == 0 && (BX * 8) % 16 == 0, "tile");
+};
+
+template <int TX, int TY, int SEG>
+__global__ void __launch_bounds__(TX * TY / SEG, Flux2TmaCfg<TX, TY, SEG>::MINB)
+k_flux_rk2_tma(Params P, const double *U0, double *Uout, int slot_base, double coef, int same_i,
+               const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapP,
+               const __grid_constant__ CUtensorMap mapV) {
+  using C = Flux2TmaCfg<TX, TY, SEG>;
+  constexpr int NT = C::NT, PIT = C::PIT;
+  extern __shared__ __align__(128) double flux_smem[];
+  double *sp = flux_smem, *su = sp + C::BOX, *sv = su + C::BOX, *sU = sv + C::BOX, *sL = sU + 2 * C::BOX;
+  unsigned long long *bars = (unsigned long long *)(sL + TY * C::LP);     // [0], [1]: U buffers (the first also p, u, v)
+
+  const int tid = threadIdx.x;
+  const int patch = blockIdx.y;
+  const int lev = P.level[patch];
+  const int ntx = (P.n[0] + TX - 1) / TX;
+  const int o0 = (blockIdx.x % ntx) * TX, o1 = (blockIdx.x / ntx) * TY;
+  const double dt = P.scal[0];
+  const long long pbase = (long long)patch * P.pc;
+  const double *U0p = U0 + pbase * P.nvar;
+  double *Uop = Uout + pbase * P.nvar;
+  const int st1i = (int)P.st[1];
+  const int goff = P.G[1] * st1i + P.G[0];
+  const double ax = slot_value(P.slots + slot_base + lev * 3 + 0), ay = slot_value(P.slots + slot_base + lev * 3 + 1);
+  const double hx = 0.5 * P.invdx[lev][0], hy = 0.5 * P.invdx[lev][1];
+  const bool same = same_i != 0;
+
+  if (tid == 0) {
+    mbar_init(bars, 1);
+    mbar_init(bars + 1, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) {
+    mbar_expect_tx(bars, 4 * C::BOX_BYTES);
+    tma_load_3d(sp, &mapP, bars, o0, o1, patch);
+    tma_load_3d(su, &mapV, bars, o0, o1, patch);
+    tma_load_3d(sv, &mapV, bars, o0, o1, P.np + patch);
+    tma_load_3d(sU, &mapU, bars, o0, o1, patch * P.nvar);
+    if (P.nvar > 1) {
+      mbar_expect_tx(bars + 1, C::BOX_BYTES);
+      tma_load_3d(sU + C::BOX, &mapU, bars + 1, o0, o1, patch * P.nvar + 1);
+    }
+  }
+
+#pragma unroll 1
+  for (int m = 0; m < P.nvar; m++) {
+    const double *sUm = sU + (m & 1) * C::BOX;
+    const double cEn = m == 3 ? 1.0 : 0.0;
+    mbar_wait(bars + (m & 1), (m >> 1) & 1);
+    {  // x pencils: lanes run over rows
+      const double cM = m == 1 ? 1.0 : 0.0;
+      const int r = tid % TY, xs = (tid / TY) * SEG;
+      const int base = (r + 3) * PIT + xs;
+      double Fh[SEG + 1];
+      if (m == 1 || m == 3)
+        weno_faces<SEG>([&](int k, double &a, double &b) { split2(sUm[base + k], su[base + k], sp[base + k], cEn, cM, ax, a, b); }, Fh);
+      else
+        weno_faces<SEG>([&](int k, double &a, double &b) { split_adv(sUm[base + k], su[base + k], ax, a, b); }, Fh);
+#pragma unroll
+      for (int i = 0; i < SEG; i++) sL[r * C::LP + xs + i] = (Fh[i] - Fh[i + 1]) * hx;
+    }
+    __syncthreads();
+    {  // y pencils: lanes run over columns; the thread applies the RK stage of its own cells
+      const double cM = m == 2 ? 1.0 : 0.0;
+      const int x = tid % TX, ys = (tid / TX) * SEG;
+      const int g0 = o0 + x, gc0 = min(g0, P.n[0] - 1);
+      const double *U0m = U0p + (long long)m * P.pc;
+      double *Uom = Uop + (long long)m * P.pc;
+      double u0v[SEG];
+      if (!same) {
+#pragma unroll
+        for (int i = 0; i < SEG; i++) u0v[i] = U0m[goff + min(o1 + ys + i, P.n[1] - 1) * st1i + gc0];
+      }
+      const int base = ys * PIT + x + 3;
+      double Fh[SEG + 1];
+      if (m == 2 || m == 3)
+        weno_faces<SEG>([&](int k, double &a, double &b) { split2(sUm[base + k * PIT], sv[base + k * PIT], sp[base + k * PIT], cEn, cM, ay, a, b); }, Fh);
+      else
+        weno_faces<SEG>([&](int k, double &a, double &b) { split_adv(sUm[base + k * PIT], sv[base + k * PIT], ay, a, b); }, Fh);
+#pragma unroll
+      for (int i = 0; i < SEG; i++) {
+        const int g1 = o1 + ys + i;
+        if (g0 < P.n[0] && g1 < P.n[1]) {
+          const double L = sL[(ys + i) * C::LP + x] + (Fh[i] - Fh[i + 1]) * hy;
+          const double uk = sUm[(ys + i + 3) * PIT + x + 3];
+          const double u0 = same ? uk : u0v[i];
+          Uom[goff + g1 * st1i + g0] = u0 + coef * ((uk - u0) + dt * L);
+        }
+      }
+    }
+    __syncthreads();   // everyone is done with sU[m & 1] and sL
+    if (tid == 0 && m + 2 < P.nvar) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy reads before the async-proxy write
+      mbar_expect_tx(bars + (m & 1), C::BOX_BYTES);
+      tma_load_3d(sU + (m & 1) * C::BOX, &mapU, bars + (m & 1), o0, o1, patch * P.nvar + m + 2);
+    }
+  }
+}

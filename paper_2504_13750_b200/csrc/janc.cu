@@ -29,6 +29,7 @@ struct Options {
   int jit_max_unknowns = JANC_JIT_MAX_N1;   // "jit_max_unknowns": largest system of the one-thread-per-cell kernel
   bool jit_big_smem = false;            // "jit_big" = "smem": the shared-memory kernel instead of the role-warp kernel
   int roles = 8;                        // "roles": 8 or 16 role-warps
+  bool tma = true;                      // "tma": 2-D tiles through cp.async.bulk.tensor (TMA) where the layout allows | cp.async
   bool halo_in_kernel = true;           // "halo" = "auto": 2-D patches <= 16 x 16 / small grids gather their halo in the
                                         //   flux kernel; "ghost": always materialise ghosts with k_ghost
 };
@@ -38,6 +39,8 @@ struct janc_ctx {
   std::set<const void *> attr_done;     // kernels whose dynamic shared-memory attribute is set on THIS context's device
   cudaError_t launch_err = cudaSuccess; // first failed kernel launch since the last check
   bool uses_cmech = false;              // table-driven kernels (c_mech in constant memory) are on this context's path
+  CUtensorMap mapU[3], mapP, mapV;      // 2-D TMA path: {Px, Py, fields} over the RK registers A, B, C, over p and over vel
+  bool have_tma = false;
   janc_grid g;
   int device;
   cudaStream_t stream;
@@ -476,6 +479,7 @@ extern "C" int janc_set_option(janc_ctx *c, const char *key, const char *value) 
   const std::string k = key, v = value;
   const bool on = !(v == "0" || v == "off" || v == "false");
   if (k == "graph") { c->opt.graph = on; c->use_graph = on; if (!on) invalidate_graphs(c); return JANC_OK; }
+  if (k == "tma") { c->opt.tma = on; invalidate_graphs(c); return JANC_OK; }
   if (k == "halo") {
     if (v != "auto" && v != "ghost") { c->err = "halo: auto | ghost"; return JANC_EINVAL; }
     c->opt.halo_in_kernel = v == "auto"; invalidate_graphs(c); return JANC_OK;
@@ -534,6 +538,57 @@ static int upload_lists(janc_ctx *c) {
   return JANC_OK;
 }
 
+// Tensor maps of the 2-D TMA path: a 3-D view {Px, Py, fields} of an array of padded fields, box = one 64 x 16 tile
+// with its 3 ghost layers.  cuTensorMapEncodeTiled is reached through the runtime (no link against libcuda).
+static bool make_map(CUtensorMap *m, void *base, int Px, int Py, long long nfields, int bx, int by) {
+  typedef CUresult (*encode_t)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                               const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_t enc = nullptr;
+  if (!enc) {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn) {
+      cudaGetLastError();
+      return false;
+    }
+    enc = (encode_t)fn;
+  }
+  const cuuint64_t dims[3] = {(cuuint64_t)Px, (cuuint64_t)Py, (cuuint64_t)nfields};
+  const cuuint64_t strides[2] = {(cuuint64_t)Px * 8, (cuuint64_t)Px * Py * 8};
+  const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// which tile the non-gathering 2-D path uses: 0 = 64 x 16 (8-cell pencils), 1 = 32 x 16, 2 = 16 x 16 (4-cell pencils)
+static int tile2d(const janc_ctx *c) { return c->P.n[0] <= 16 && c->P.n[1] <= 16 ? 2 : c->P.n[0] <= 32 ? 1 : 0; }
+
+static void setup_tma(janc_ctx *c) {
+  c->have_tma = false;
+  const Params &P = c->P;
+  if (c->g.ndim != 2 || (P.P[0] & 1) || ((long long)P.P[0] * P.P[1] & 1)) return;   // strides must be multiples of 16 bytes
+  const int t = tile2d(c), bx = (t == 0 ? 64 : t == 1 ? 32 : 16) + 6, by = 16 + 6;
+  double *regs[3] = {c->A, c->B, c->C};
+  bool ok = true;
+  for (int q = 0; q < 3; q++) ok = ok && make_map(&c->mapU[q], regs[q], P.P[0], P.P[1], (long long)c->np * c->nvar, bx, by);
+  ok = ok && make_map(&c->mapP, P.p, P.P[0], P.P[1], c->np, bx, by);
+  ok = ok && make_map(&c->mapV, P.vel, P.P[0], P.P[1], (long long)c->np * 2, bx, by);
+  c->have_tma = ok;
+}
+
+template <int TX, int TY, int SEG>
+static void launch_flux2_tma(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef) {
+  using C = Flux2TmaCfg<TX, TY, SEG>;
+  const Params &P = c->P;
+  smem_attr(c, (const void *)k_flux_rk2_tma<TX, TY, SEG>, C::SMEM);
+  const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY));
+  const int which = Uk == c->A ? 0 : Uk == c->B ? 1 : 2;
+  k_flux_rk2_tma<TX, TY, SEG><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, U0, Uout, slot_base, coef, Uk == U0 ? 1 : 0,
+                                                                                      c->mapU[which], c->mapP, c->mapV);
+}
+
 extern "C" int janc_bind_workspace(janc_ctx *c, void *dev_ptr, size_t bytes) {
   if (!c || !c->have_mech || !dev_ptr) return JANC_EINVAL;
   size_t need = janc_workspace_bytes(c);
@@ -544,6 +599,7 @@ extern "C" int janc_bind_workspace(janc_ctx *c, void *dev_ptr, size_t bytes) {
   c->ws_bytes = need;
   CK(cudaMemsetAsync(dev_ptr, 0, need, c->stream));
   c->have_ws = true; c->have_state = false; c->parity = 0;
+  setup_tma(c);
   return upload_lists(c);
 }
 
@@ -769,6 +825,12 @@ static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uou
     const bool tiny = c->P.n[0] <= 16 && c->P.n[1] <= 16;
     if (gather_mode(c) && tiny) launch_flux2<16, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // AMR patches: halo gathered in-kernel; 2 warps per patch
     else if (gather_mode(c)) launch_flux2<32, 16, 4, true>(c, Uk, U0, Uout, slot_base, coef);   // small grids: 4x the CTAs, no ghost launches
+    else if (c->opt.tma && c->have_tma) {     // materialised ghosts: one TMA box per field
+      const int t = tile2d(c);
+      if (t == 2) launch_flux2_tma<16, 16, 4>(c, Uk, U0, Uout, slot_base, coef);
+      else if (t == 1) launch_flux2_tma<32, 16, 4>(c, Uk, U0, Uout, slot_base, coef);
+      else launch_flux2_tma<64, 16, 8>(c, Uk, U0, Uout, slot_base, coef);
+    }
     else if (c->P.n[0] <= 32) launch_flux2<32, 16, 4, false>(c, Uk, U0, Uout, slot_base, coef);   // patches of <= 32 columns with materialised ghosts
     else launch_flux2<64, 16, 8>(c, Uk, U0, Uout, slot_base, coef);
   } else launch_flux<3, 16, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);   // 128 threads, 39 KB: 4 independent CTAs per SM overlap stage / walk
