@@ -19,6 +19,7 @@
  *                              :338 (rhs = flux gradient + source_terms), :351-357 (advance_one_step without
  *                              advance_source_term); the source is the mechanism's own W_k omega_k of eq 4.6
  *   average-down
+ *   crossover time advance     PAPER.md:186 (Fig 2a): level l at half the step of level l-1, deepest level first
  * No blocking, fusion or reordering beyond that.  OpenMP only splits independent cells/lines;
  * reductions are exact max, so results do not depend on the thread count.
  *
@@ -70,6 +71,7 @@ typedef struct {
 
 typedef struct jref_ctx {
   int explicit_src;            /* 1: chemical source added to the rhs of every RK stage */
+  int only;                    /* -1: every level is advanced; 0 / 1: only the patches of that level (crossover advance) */
   jref_grid g;
   int np, nvar, have_mech, have_state;
   int P[3], G[3];
@@ -289,6 +291,7 @@ int jref_create(const jref_grid *g, jref_ctx **out) {
   if (!c) return JREF_ENOMEM;
   c->g = *g;
   c->np = g->n_patches > 0 ? g->n_patches : 1;
+  c->only = -1;
   if (g->n_patches <= 0) { c->g.n_levels = 1; }
   if (c->g.n_levels < 1 || c->g.n_levels > 2 || (c->g.n_levels == 2 && g->ratio != 2)) { free(c); return JREF_EINVAL; }
   c->pc = 1;
@@ -420,6 +423,7 @@ static void prim_all(jref_ctx *c, double *U, int ghosts, double smax[2][3]) {
   int bad = 0;
   for (int p = 0; p < c->np; p++) {
     int lev = c->level[p];
+    if (c->only >= 0 && lev != c->only) continue;      /* crossover advance: one level at a time */
     double s0 = 0, s1 = 0, s2 = 0;
     int glo[3], ghi[3];
     for (int d = 0; d < 3; d++) { glo[d] = ghosts ? -c->G[d] : 0; ghi[d] = n[d] + (ghosts ? c->G[d] : 0); }
@@ -460,6 +464,7 @@ static void ghost_fill(jref_ctx *c, double *U) {
   for (int lev = 0; lev < c->g.n_levels; lev++)      /* level 0 first: level 1 injects from its padded parent */
     for (int p = 0; p < c->np; p++) {
       if (c->level[p] != lev) continue;
+      if (c->only >= 0 && lev != c->only && !(lev == 0 && c->only == 1)) continue;   /* the fine level still needs its parents' ghosts */
       for (int d = 0; d < nd; d++)
         for (int side = 0; side < 2; side++) {
           int f = 2 * d + side, kind = c->fkind[p * nf + f];
@@ -521,6 +526,7 @@ static void flux_divergence(jref_ctx *c, const double *U, double alpha[2][3], do
   memset(L, 0, sizeof(double) * (size_t)c->np * nv * c->pc);
   for (int p = 0; p < c->np; p++) {
     int lev = c->level[p];
+    if (c->only >= 0 && lev != c->only) continue;
     for (int d = 0; d < nd; d++) {
       double dx = c->g.dx[d]; for (int l = 0; l < lev; l++) dx /= c->g.ratio;
       double al = alpha[lev][d];
@@ -573,6 +579,7 @@ static void chemistry(jref_ctx *c, double dt) {
   if (n1 == 0 || c->m.nr == 0) return;
   int bad = 0;
   for (int p = 0; p < c->np; p++) {
+    if (c->only >= 0 && c->level[p] != c->only) continue;
 #pragma omp parallel
     {
       double *work = malloc(sizeof(double) * (ns + c->m.nr + c->m.nr * ns + n1 * n1 + 2 * n1));
@@ -628,6 +635,7 @@ static void source_terms(jref_ctx *c, const double *U, double *L) {
   const int *n = c->g.n; int nd = c->g.ndim, nv = c->nvar, ns = c->m.ns, n1 = ns - 1, nr = c->m.nr;
   if (n1 < 1 || nr < 1) return;
   for (int p = 0; p < c->np; p++) {
+    if (c->only >= 0 && c->level[p] != c->only) continue;
     const double *Up = U + (long)p * nv * c->pc;
 #pragma omp parallel
     {
@@ -647,13 +655,36 @@ static void source_terms(jref_ctx *c, const double *U, double *L) {
   }
 }
 
-/* advance_one_step: CFL -> advance_flux (RK3) -> advance_source_term */
-/* do_chem: 0 no chemistry, 1 point-implicit after the RK3, 2 explicit: source inside every RK stage
- * and no advance_source_term */
-int jref_step(jref_ctx *c, int nsteps, double cfl, double dt_fixed, int do_chem, double *t_adv) {
-  if (!c || !c->have_state) return JREF_ESTATE;
-  c->explicit_src = do_chem == 2;
+/* advance_flux + advance_source_term of the patches selected by c->only over one step dt */
+static void advance(jref_ctx *c, double dt, int do_chem) {
   size_t N = (size_t)c->np * c->nvar * c->pc;
+  double s[2][3];
+  memcpy(c->U0, c->U, N * sizeof(double));
+  /* Shu-Osher SSP-RK3 in increment form (readings A4); L = 0 on patches that are not selected: they keep their state */
+  rhs(c, c->U, c->L);
+  for (size_t i = 0; i < N; i++) c->U[i] = c->U0[i] + dt * c->L[i];
+  rhs(c, c->U, c->L);
+  for (size_t i = 0; i < N; i++) c->U[i] = c->U0[i] + 0.25 * ((c->U[i] - c->U0[i]) + dt * c->L[i]);
+  rhs(c, c->U, c->L);
+  for (size_t i = 0; i < N; i++) c->U[i] = c->U0[i] + (2.0 / 3.0) * ((c->U[i] - c->U0[i]) + dt * c->L[i]);
+  /* advance_source_term: update_aux -> solve_implicit_rate -> U + dU */
+  prim_all(c, c->U, 0, s);
+  if (do_chem == 1) chemistry(c, dt);
+}
+
+/* advance_one_step: CFL -> advance_flux (RK3) -> advance_source_term.
+ * mode & 3: 0 no chemistry, 1 point-implicit after the RK3, 2 explicit: source inside every RK stage
+ *           and no advance_source_term.
+ * mode & 4: crossover time advance of a two-level block list (Fig 2a; reading B9): the step of
+ *           a level is half that of the previous level and the deepest level is solved first -- two steps dt/2 of level
+ *           1, its coarse-fine ghosts injected from the level-0 state at the START of the step (level 0 has not moved
+ *           yet), then one step dt of level 0, then interpolate_fine_to_coarse.  dt = CFL * min dx(level 0) / max(|u|+c)
+ *           (twice the synchronous step: both levels run at the same CFL number); cfl <= 0: dt_fixed is the level-0 step.
+ *           Without the bit: synchronous advance, every level at the finest level's step (PAPER.md:186 Fig 2b, :460). */
+int jref_step(jref_ctx *c, int nsteps, double cfl, double dt_fixed, int mode, double *t_adv) {
+  if (!c || !c->have_state) return JREF_ESTATE;
+  const int do_chem = mode & 3, crossover = (mode & 4) && c->g.n_levels == 2;
+  c->explicit_src = do_chem == 2;
   double t = 0.0, s[2][3];
   for (int it = 0; it < nsteps; it++) {
     double dt = dt_fixed;
@@ -662,23 +693,20 @@ int jref_step(jref_ctx *c, int nsteps, double cfl, double dt_fixed, int do_chem,
       double smax = 0.0, dxmin = 1e300;
       for (int l = 0; l < 2; l++) for (int d = 0; d < c->g.ndim; d++) if (s[l][d] > smax) smax = s[l][d];
       for (int d = 0; d < c->g.ndim; d++) {
-        double dx = c->g.dx[d]; for (int l = 1; l < c->g.n_levels; l++) dx /= c->g.ratio;
+        double dx = c->g.dx[d];
+        if (!crossover) for (int l = 1; l < c->g.n_levels; l++) dx /= c->g.ratio;
         if (dx < dxmin) dxmin = dx;
       }
       dt = cfl * dxmin / smax;
     }
     c->dt_last = dt;
-    memcpy(c->U0, c->U, N * sizeof(double));
-    /* Shu-Osher SSP-RK3 in increment form (readings A4) */
-    rhs(c, c->U, c->L);
-    for (size_t i = 0; i < N; i++) c->U[i] = c->U0[i] + dt * c->L[i];
-    rhs(c, c->U, c->L);
-    for (size_t i = 0; i < N; i++) c->U[i] = c->U0[i] + 0.25 * ((c->U[i] - c->U0[i]) + dt * c->L[i]);
-    rhs(c, c->U, c->L);
-    for (size_t i = 0; i < N; i++) c->U[i] = c->U0[i] + (2.0 / 3.0) * ((c->U[i] - c->U0[i]) + dt * c->L[i]);
-    /* advance_source_term: update_aux -> solve_implicit_rate -> U + dU */
-    prim_all(c, c->U, 0, s);
-    if (do_chem == 1) chemistry(c, dt);
+    if (crossover) {
+      c->only = 1; advance(c, 0.5 * dt, do_chem); advance(c, 0.5 * dt, do_chem);
+      c->only = 0; advance(c, dt, do_chem);
+      c->only = -1;
+    } else {
+      advance(c, dt, do_chem);
+    }
     average_down(c);
     t += dt;
   }

@@ -113,10 +113,11 @@ class RefSolver:
         if rc:
             raise RuntimeError(f"jref_set_state failed: {rc}")
 
-    def step(self, nsteps, cfl=0.0, dt=0.0, chem=True):
-        """chem: True point-implicit, False none, "explicit" source inside the RK stages (:351-357)."""
+    def step(self, nsteps, cfl=0.0, dt=0.0, chem=True, crossover=False):
+        """chem: True point-implicit (PAPER.md:344-349), False none, "explicit" source inside the RK stages (:351-357);
+        crossover: sub-cycled level advance of a two-level block list (Fig 2a)."""
         t = C.c_double(0.0)
-        mode = 2 if chem == "explicit" else int(bool(chem))
+        mode = (2 if chem == "explicit" else int(bool(chem))) | (4 if crossover else 0)
         rc = lib().jref_step(self._h, int(nsteps), C.c_double(cfl), C.c_double(dt), mode, C.byref(t))
         self.status = rc
         return t.value

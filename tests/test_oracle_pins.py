@@ -787,3 +787,131 @@ def test_reflecting_wall_equals_half_of_the_mirrored_periodic_box(ref, mech9, ax
     right = np.flip(Uf[..., n:] if axis == 0 else Uf[..., n:, :], axis=4 if axis == 0 else 3).copy()
     right[:, 1 + axis] *= -1.0
     assert np.abs(right - left).max() <= 1e-13 * np.abs(left).max()
+
+
+# ----------------------------------------------------------------------------- crossover (sub-cycled) level advance
+def _run_x(ref, case, nsteps, crossover, cfl=None, dt=0.0, chem=True):
+    s = ref.RefSolver(case.grid, case.mech, case.blocks)
+    s.set_state(case.U, case.T)
+    t = s.step(nsteps, cfl=case.cfl if cfl is None else cfl, dt=dt, chem=chem, crossover=crossover)
+    U, T = s.get_state()
+    return U, T, t, s.status
+
+
+def test_crossover_on_one_level_is_the_plain_advance(ref, mech9):
+    """with a single level there is nothing to sub-cycle: bitwise the synchronous result."""
+    tiled = I.tile_uniform(_random_smooth_2d(mech9, 32, 24, 3, I.BC_REFLECT), 8, 8)
+    Ua, _, ta, _ = _run_x(ref, tiled, 3, False)
+    Ub, _, tb, _ = _run_x(ref, tiled, 3, True)
+    assert ta == tb and np.array_equal(Ua, Ub)
+
+
+def test_crossover_uniform_state_and_step_size(ref, mech9):
+    """A uniform two-level state stays uniform, and the step is CFL dx(level 0) / (|u| + c): twice the synchronous step
+    (each level at half the step of the previous one).  Not bitwise as in the synchronous advance: the
+    levels reach the same U through different sequences of Newton iterates, and T(U) is defined to 1e-11 only (reading
+    A6), so the pressures of a fine cell and of its coarse-parent ghost differ in the last bits; the momentum that
+    imbalance creates is bounded by that tolerance."""
+    c = I.config3(pcols=8, prows=4, npc=8, nsteps=3)
+    Y = I.hot_Y(9)
+    Ucell = I.prim_to_cons(mech9, 2, np.array([3e5]), np.array([900.0]), Y[None], [np.zeros(1), np.zeros(1)])[:, 0]
+    c.U[:] = Ucell[None, :, None, None, None]; c.T[:] = 900.0
+    U1, _, t, st = _run_x(ref, c, 3, True, chem=False)
+    R = (Y * RU / mech9.W).sum(); cp = (Y * RU / mech9.W * mech9.nasa[:, 0]).sum()
+    cs = math.sqrt(cp / (cp - R) * R * 900.0)
+    assert st == 0
+    for v in range(c.nvar):
+        scale = abs(Ucell[v]) if v not in (1, 2) else Ucell[0] * cs
+        assert np.abs(U1[:, v] - c.U[:, v]).max() <= 1e-11 * scale, v
+    assert np.array_equal(U1[:, 0], c.U[:, 0])                      # density: exactly (mass flux 0 x anything)
+    assert abs(t - 3 * 0.2 * 1.0e-4 / cs) <= 1e-12 * t
+
+
+def test_crossover_fully_refined_equals_two_fine_steps(ref, mech9):
+    """Every level-0 patch refined: level 1 then has only same-level neighbours and walls, so its two half steps are two
+    plain steps of the uniform fine grid with dt/2 (pinned elsewhere: tiling == uniform grid), and level 0 ends as the
+    four-to-one mean of level 1 whatever its own step did."""
+    nx, ny, tile = 32, 16, 8
+    coarse = _random_smooth_2d(mech9, nx, ny, 11, I.BC_REFLECT)
+    c2 = I.refine_uniform(coarse, (tile, tile), np.ones((ny // tile, nx // tile), bool))
+    dt = 4.0e-9
+    Ux, _, t, st = _run_x(ref, c2, 2, True, cfl=0.0, dt=dt)
+    assert st == 0 and abs(t - 2 * dt) <= 1e-15 * t
+    # the same fine data as ONE uniform grid (the injection of the coarse initial state), four steps of dt/2
+    fineU = np.repeat(np.repeat(coarse.U, 2, axis=3), 2, axis=4)
+    fineT = np.repeat(np.repeat(coarse.T, 2, axis=2), 2, axis=3)
+    g = coarse.grid
+    fine = I.Case("fine", I.Grid(2, (2 * nx, 2 * ny, 1), (g.dx[0] / 2, g.dx[1] / 2, 1), g.bc_lo, g.bc_hi), mech9, fineU, fineT, 0.2, 4)
+    Uf, _, _, st2 = run(ref, fine, nsteps=4, cfl=0.0, dt=dt / 2)
+    assert st2 == 0
+    lev, org = c2.blocks.level, c2.blocks.origin
+    for p in np.nonzero(lev == 1)[0]:
+        ox, oy = org[p]
+        want = Uf[0, :, 0, oy:oy + tile, ox:ox + tile]
+        assert np.abs(Ux[p, :, 0] - want).max() <= 1e-13 * np.abs(want).max(), p
+    for p in np.nonzero(lev == 0)[0]:
+        ox, oy = org[p]
+        f = Uf[0, :, 0, 2 * oy:2 * oy + 2 * tile, 2 * ox:2 * ox + 2 * tile]
+        mean = 0.25 * (f[:, 0::2, 0::2] + f[:, 0::2, 1::2] + f[:, 1::2, 0::2] + f[:, 1::2, 1::2])
+        assert np.abs(Ux[p, :, 0] - mean).max() <= 1e-13 * np.abs(mean).max(), p
+
+
+def test_crossover_coarse_level_takes_the_full_step_with_frozen_fine_ghosts(ref, mech9):
+    """Far from the refined patches (beyond the reach of 3 stages x 3 cells per step) level 0 must evolve exactly as a
+    level-0-only run with the same fixed dt: it takes ONE step of dt per iteration and never reads level 1."""
+    nx, ny, tile = 64, 16, 8
+    coarse = _random_smooth_2d(mech9, nx, ny, 12, I.BC_PERIODIC)
+    mask = np.zeros((ny // tile, nx // tile), bool); mask[:, 0] = True          # refine the first patch column only
+    c2 = I.refine_uniform(coarse, (tile, tile), mask)
+    dt = 3.0e-9
+    Ux, _, _, st = _run_x(ref, c2, 1, True, cfl=0.0, dt=dt)
+    U0, _, _, st0 = run(ref, coarse, nsteps=1, cfl=0.0, dt=dt)
+    assert st == 0 and st0 == 0
+    lev, org = c2.blocks.level, c2.blocks.origin
+    checked = 0
+    for p in np.nonzero(lev == 0)[0]:
+        ox, oy = org[p]
+        if 24 <= ox <= 32:                          # >= 16 cells from the refined column on either (periodic) side
+            assert np.array_equal(Ux[p, :, 0], U0[0, :, 0, oy:oy + tile, ox:ox + tile]); checked += 1
+    assert checked >= 2
+    assert np.abs(Ux[:, 0] - c2.U[:, 0]).max() > 0
+
+
+def test_crossover_converges_to_synchronous_at_first_order(ref, mech9):
+    """Both strategies integrate the same equations; they differ by the frozen coarse-fine ghost data and the splitting
+    of the steps, an O(dt) effect: at a fixed final time the difference halves with dt (Fig 2a vs 2b)."""
+    c = I.config3(pcols=8, prows=4, npc=8)
+    tend = 1.6e-8
+    errs = []
+    for n in (2, 4, 8):
+        Ux, _, _, s1 = _run_x(ref, c, n, True, cfl=0.0, dt=tend / n)               # level-0 step tend / n
+        Us, _, _, s2 = _run_x(ref, c, 2 * n, False, cfl=0.0, dt=tend / (2 * n))    # every level at the fine step
+        assert s1 == 0 and s2 == 0
+        errs.append(np.abs(Ux[:, 0] - Us[:, 0]).max() / np.abs(Us[:, 0]).max())
+    assert errs[2] < errs[1] < errs[0] and errs[2] < 0.7 * errs[1] and errs[0] < 0.05, errs
+
+
+def test_crossover_fine_level_sees_the_coarse_state_at_the_start_of_the_step(ref, mech9):
+    """"The deepest refinement level is solved first": during its two half steps the fine level's
+    coarse-fine ghosts hold level-0 data of time t^n, so the fine result of ONE step depends on the coarse initial data
+    only through the two coarse cells under its three ghost layers.  A perturbation of the coarse initial state 5..7
+    cells away from the refined patches (within reach of a coarse step: 9 cells) must therefore leave the fine patches
+    bitwise unchanged; had level 0 been advanced first, its new state next to the fine patches would differ."""
+    nx, ny, tile = 64, 16, 8
+    coarse = _random_smooth_2d(mech9, nx, ny, 13, I.BC_REFLECT)
+    mask = np.zeros((ny // tile, nx // tile), bool); mask[:, 3] = True              # refine patch column 3: cells 24..31
+    base = I.refine_uniform(coarse, (tile, tile), mask)
+    pert = I.refine_uniform(coarse, (tile, tile), mask)
+    lev, org = base.blocks.level, base.blocks.origin
+    for p in np.nonzero(lev == 0)[0]:                                               # coarse columns 37..39 (5..7 cells right of the band)
+        if org[p, 0] == 32:
+            pert.U[p, :, 0, :, 5:8] *= 0.97                                         # density, momentum, energy, species: a slower, same-T gas
+    dt = 2.0e-9
+    Ua, _, _, sa = _run_x(ref, base, 1, True, cfl=0.0, dt=dt, chem=False)
+    Ub, _, _, sb = _run_x(ref, pert, 1, True, cfl=0.0, dt=dt, chem=False)
+    assert sa == 0 and sb == 0
+    fine = np.nonzero(lev == 1)[0]
+    assert np.array_equal(Ua[fine], Ub[fine])
+    # the coarse cells next to the band did feel it (so a coarse-first order would have passed it on)
+    near = [p for p in np.nonzero(lev == 0)[0] if org[p, 0] == 32]
+    assert max(np.abs(Ua[p, 0, 0, :, 0:2] - Ub[p, 0, 0, :, 0:2]).max() for p in near) > 0
