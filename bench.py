@@ -203,7 +203,7 @@ def chem_bytes_per_cell(ndim, nvar, ns):
     return (nvar + 1 + ns) * 8
 
 
-def measure(binding, case, K, W, local, world, barrier, do_e2e=True):
+def measure(binding, case, K, W, local, world, barrier, do_e2e=True, crossover=False):
     """One workload on this rank's GPU: K timed steps with the state resident in HBM, K profiled steps (per-kernel
     device time, CUDA events on the library's stream), and (do_e2e) the end-to-end loop with pinned host buffers."""
     import torch
@@ -212,6 +212,20 @@ def measure(binding, case, K, W, local, world, barrier, do_e2e=True):
     out = {"chem_kernel": s.chem_kernel()}
     Ud = torch.from_numpy(case.U).to(dev); Td = torch.from_numpy(case.T).to(dev)
     s.set_state(Ud, Td)
+    if crossover:      # timing of the sub-cycled level advance only (Fig 2a): no per-kernel phases, no e2e
+        for _ in range(W):
+            s.step(1, cfl=case.cfl, sync=False, crossover=True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(K):
+            s.step(1, cfl=case.cfl, sync=False, crossover=True)
+        e1.record()
+        barrier()
+        assert s.status_sync() == 0
+        out["ms"] = e0.elapsed_time(e1)
+        s.close()
+        return out
     for _ in range(W):
         s.step(1, cfl=case.cfl, sync=False)
     assert s.status_sync() == 0, "device flag raised during warm-up"
@@ -388,6 +402,14 @@ def main():
                            "chem": {k: e2["chem"][k] for k in ("kernel", "frac", "avg_launch_ms", "traffic")} if "chem" in e2 else None,
                            "hbm": {"achieved": algo_bytes / (step_ms * 1e-3) / 1e9, "frac": algo_bytes / (step_ms * 1e-3) / 1e9 / hbm_peak,
                                    "unit": "GB/s", "note": "algorithmic bytes of the whole step / step time"}}
+                if c2.blocks is not None and c2.grid.n_levels == 2:
+                    # the paper's recommended strategy (PAPER.md:186 Fig 2a, :476): one crossover step advances the
+                    # solution as far as two synchronous steps
+                    mx = measure(binding, c2, K2, W, local, world, barrier, do_e2e=False, crossover=True)
+                    lev = c2.blocks.level
+                    per[wl]["crossover"] = {"ms_per_level0_step": mx["ms"] / K2, "synchronous_ms_for_the_same_time": 2 * step_ms,
+                                            "time_ratio": (mx["ms"] / K2) / (2 * step_ms),
+                                            "cell_updates_per_s": (int((lev == 0).sum()) + 2 * int((lev == 1).sum())) * c2.cells // len(lev) * K2 / (mx["ms"] * 1e-3)}
                 del c2
             line["per_config"] = per
         if not args.no_cpu_baseline and world >= 1:

@@ -117,6 +117,11 @@ int janc_set_state(janc_ctx *, const double *U, const double *T_guess, int on_de
  * source_terms); bit 1 set => explicit variant with the mechanism's own source: S_k = W_k omega_k(T, X) (eq 4.6) is added to
  * the right-hand side of every RK stage and advance_source_term is not executed; returns JANC_ESTATE if
  * the run-time specialised source kernel is not available (no NVRTC).
+ * bit 2 set => crossover time advance of a two-level block list (Fig 2a; reading B9) instead of
+ * the synchronous one (Fig 2b): per step, two steps dt/2 of level 1 -- its coarse-fine ghosts injected from the level-0
+ * state at the start of the step -- then one step dt of level 0, then the average-down; dt = cfl * min_d dx_d(level 0) /
+ * max(|u_d| + c), or dt_fixed = the level-0 step.  Needs the patches ordered by level (JANC_EINVAL otherwise); ignored
+ * on a single level.
  * t_advanced (host, nullable): receives the sum of dt; forces a stream synchronise. */
 int janc_step(janc_ctx *, int nsteps, double cfl, double dt_fixed, int flags, double *t_advanced);
 

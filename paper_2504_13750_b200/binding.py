@@ -18,6 +18,7 @@ _lib = None
 JANC_OK, JANC_EINVAL, JANC_ENOMEM, JANC_ECUDA, JANC_ESTATE, JANC_ENONFINITE = 0, -1, -2, -3, -4, -5
 FLAG_NO_CHEM = 1
 FLAG_EXPLICIT_SOURCE = 2
+FLAG_CROSSOVER = 4
 
 EXPORTS = ["janc_create", "janc_set_option", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
            "janc_set_blocks", "janc_set_state", "janc_step", "janc_get_state", "janc_status",
@@ -198,10 +199,13 @@ class Solver:
             self._check(lib().janc_set_state(self._h, _ptr(U), _ptr(Tn) if Tn is not None else None, 0),
                         "janc_set_state")
 
-    def step(self, nsteps, cfl=0.0, dt=0.0, chem=True, sync=True):
+    def step(self, nsteps, cfl=0.0, dt=0.0, chem=True, sync=True, crossover=False):
         """Returns the time advanced (sync=True) or None (asynchronous enqueue).  chem: True = point-implicit after the
-        RK3, False = none, "explicit" = source inside every RK stage."""
+        RK3, False = none, "explicit" = source inside every RK stage; crossover:
+        sub-cycled level advance of a two-level block list (Fig 2a), dt / cfl then refer to level 0."""
         flags = FLAG_EXPLICIT_SOURCE if chem == "explicit" else (0 if chem else FLAG_NO_CHEM)
+        if crossover:
+            flags |= FLAG_CROSSOVER
         if sync:
             t = C.c_double(0.0)
             rc = lib().janc_step(self._h, int(nsteps), float(cfl), float(dt), flags, C.byref(t))

@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(128) k_chem(Params P, double *__restrict__ U) 
   const int ns = NS > 0 ? NS : P.ns;
   const int n1 = ns - 1;
   const int nr = c_mech.nr;
-  const int patch = blockIdx.y;
+  const int patch = blockIdx.y + P.patch0;
   const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= ncell) return;
@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(128) k_chem(Params P, double *__restrict__ U) 
 
   if (n1 > 0 && nr > 0) {
     // ---- A = I - dt J,  J_kl = W_k (D[k][l]/W_l - D[k][Ns]/W_Ns);  rhs = dt W_k wdot_k
-    const double dt = P.scal[0];
+    const double dt = P.scal[0] * P.dt_scale;
     double rhs[N1M > 0 ? N1M : 1];
     const double iWn = c_mech.invW[n1];
     for (int a = 0; a < n1; a++) {
@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(NT) k_chem_reg(Params P, double *__restrict__ 
   double *scf = sX + NS * NT;                     // [nr]  M k_f
   double *scb = scf + nr * NT;                    // [nr]  -M k_b
   double *srn = scb + nr * NT;                    // [ntb] k_f prod X - k_b prod X of third-body reactions
-  const int patch = blockIdx.y;
+  const int patch = blockIdx.y + P.patch0;
   const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
   long long t = (long long)blockIdx.x * NT + threadIdx.x;
   const bool live = t < ncell;
@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(NT) k_chem_reg(Params P, double *__restrict__ 
       for (int k = 0; k < N1; k++) D[k][j] = col[k];
     }
     // ---- A = I - dt J,  J_kl = W_k (D[k][l]/W_l - D[k][Ns]/W_Ns);  rhs = dt W_k wdot_k
-    const double dt = P.scal[0];
+    const double dt = P.scal[0] * P.dt_scale;
     double rhs[N1 > 0 ? N1 : 1];
     const double iWn = c_mech.invW[N1];
 #pragma unroll

@@ -204,7 +204,7 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
   std::string &src = E.s;
   src += "// generated by chemgen.h for ns=" + I(ns) + " nr=" + I(nr) + " ndim=" + I(ndim) + "\n";
   src += "struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2;"
-         " long long st0, st1, st2, pc; int np; };\n";
+         " long long st0, st1, st2, pc; int np, patch0; double dts; };\n";
   emit_math(src);
   src += "extern \"C\" __global__ void __launch_bounds__(" + I(NT) + ") k_chem_jit(ChemArgs a) {\n";
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
@@ -221,8 +221,8 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
   E.line("const unsigned t32 = (unsigned)t, r_ = t32 / (unsigned)a.n0; const int ci = (int)(t32 - r_ * (unsigned)a.n0);");
   E.line("const unsigned k_ = r_ / (unsigned)a.n1; const int cj = (int)(r_ - k_ * (unsigned)a.n1), ck = (int)k_;");
   E.line("const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;");
-  E.line("double *Up = a.U + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
-  E.line("const long long pid = (long long)blockIdx.y * a.pc + id;");
+  E.line("double *Up = a.U + (long long)(blockIdx.y + a.patch0) * " + I(nvar) + " * a.pc + id;");
+  E.line("const long long pid = (long long)(blockIdx.y + a.patch0) * a.pc + id;");
   // ---- cons -> prim pieces (eq 4.2), X_k = rho Y_k / W_k
   E.line("const double rho = Up[0], irho = 1.0 / rho;");
   E.line("double ke = 0.0;");
@@ -257,7 +257,7 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
     E.line("const double g" + I(k) + " = fma(" + num(c[0]) + ", lnT, " + horner(sc, 5) + ") - (" + horner(hc, 6) + ") * iT;");
   }
   if (any_rev) E.line("const double lnC0 = " + num(std::log(JANC_PATM / JANC_RU)) + " - lnT;   // ln(p0 / (Ru T))");
-  E.line("const double dt = a.scal[0];");
+  E.line("const double dt = a.scal[0] * a.dts;");
   // ---- rates of progress (eq 4.7-4.9), wdot_k = sum_i dnu_ik q_i, D_k_j = sum_i dnu_ik dq_i/dX_j
   Acc accW(ns), accD(n1 * ns);
   for (int i = 0; i < nr; i++) {
@@ -395,7 +395,7 @@ inline std::string generate_source(const MechC &M, int ndim, bool with_math) {
   Emitter E;
   std::string &src = E.s;
   src += "struct SrcArgs { const double *Uk; double *Uout; const double *T; const double *scal; int n0, n1, n2, G0, G1, G2;"
-         " long long st0, st1, st2, pc; double coef; };\n";
+         " long long st0, st1, st2, pc; double coef; int patch0; };\n";
   if (with_math) emit_math(src);
   src += "extern \"C\" __global__ void __launch_bounds__(128) k_src_jit(SrcArgs a) {\n";
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
@@ -405,9 +405,9 @@ inline std::string generate_source(const MechC &M, int ndim, bool with_math) {
   E.line("const unsigned t32 = (unsigned)t, r_ = t32 / (unsigned)a.n0; const int ci = (int)(t32 - r_ * (unsigned)a.n0);");
   E.line("const unsigned k_ = r_ / (unsigned)a.n1; const int cj = (int)(r_ - k_ * (unsigned)a.n1), ck = (int)k_;");
   E.line("const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;");
-  E.line("const double *Up = a.Uk + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
-  E.line("double *Uo = a.Uout + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
-  E.line("const double T = a.T[(long long)blockIdx.y * a.pc + id];");
+  E.line("const double *Up = a.Uk + (long long)(blockIdx.y + a.patch0) * " + I(nvar) + " * a.pc + id;");
+  E.line("double *Uo = a.Uout + (long long)(blockIdx.y + a.patch0) * " + I(nvar) + " * a.pc + id;");
+  E.line("const double T = a.T[(long long)(blockIdx.y + a.patch0) * a.pc + id];");
   E.line("const double rho = Up[0];");
   E.line("double rsum = 0.0;");
   for (int k = 0; k < n1; k++) {
@@ -475,7 +475,7 @@ inline std::string generate_prim(const MechC &M, int ndim) {
   Emitter E;
   std::string &src = E.s;
   src += "struct PrimArgs { const double *U; double *T; double *p; double *vel; double *dbgc; unsigned long long *slots;"
-         " const int *level; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np, reduce, slot_base; };\n";
+         " const int *level; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np, reduce, slot_base, patch0; };\n";
   src += "extern \"C\" __global__ void __launch_bounds__(256) k_prim_jit(PrimArgs a) {\n";
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2;");
   E.line("const long long t = (long long)blockIdx.x * 256 + threadIdx.x;");
@@ -485,8 +485,8 @@ inline std::string generate_prim(const MechC &M, int ndim) {
   E.line("const unsigned t32 = (unsigned)t, r_ = t32 / (unsigned)a.n0; const int ci = (int)(t32 - r_ * (unsigned)a.n0);");
   E.line("const unsigned k_ = r_ / (unsigned)a.n1; const int cj = (int)(r_ - k_ * (unsigned)a.n1), ck = (int)k_;");
   E.line("const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;");
-  E.line("const double *Up = a.U + (long long)blockIdx.y * " + I(nvar) + " * a.pc + id;");
-  E.line("const long long pid = (long long)blockIdx.y * a.pc + id;");
+  E.line("const double *Up = a.U + (long long)(blockIdx.y + a.patch0) * " + I(nvar) + " * a.pc + id;");
+  E.line("const long long pid = (long long)(blockIdx.y + a.patch0) * a.pc + id;");
   E.line("const double rho = Up[0], irho = 1.0 / rho;");
   E.line("double ke = 0.0;");
   for (int d = 0; d < ndim; d++)
@@ -529,7 +529,7 @@ inline std::string generate_prim(const MechC &M, int ndim) {
   E.line("  if (threadIdx.x < " + I(ndim) + ") {");
   E.line("    double v = 0.0;");
   E.line("    for (int q = 0; q < 8; q++) v = fmax(v, sh[threadIdx.x][q]);");
-  E.line("    atomicMax(a.slots + a.slot_base + a.level[blockIdx.y] * 3 + threadIdx.x, (unsigned long long)__double_as_longlong(v));");
+  E.line("    atomicMax(a.slots + a.slot_base + a.level[blockIdx.y + a.patch0] * 3 + threadIdx.x, (unsigned long long)__double_as_longlong(v));");
   E.line("  }");
   E.line("}");
   src += "}\n";

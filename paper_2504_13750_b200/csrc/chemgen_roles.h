@@ -167,7 +167,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   // =========================================================================== tables
   src += "// generated by chemgen_roles.h for ns=" + I(ns) + " nr=" + I(nr) + " ndim=" + I(ndim) + "\n";
   src += "struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2;"
-         " long long st0, st1, st2, pc; int np; };\n";
+         " long long st0, st1, st2, pc; int np, patch0; double dts; };\n";
   // Tables: emitted as two __constant__ arrays, copied once per (persistent) CTA into shared memory, where the
   // warp-uniform, run-time indexed reads of the rate loop are plain broadcast loads.
   std::vector<std::string> td, ti;
@@ -213,13 +213,13 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   src += "__device__ __forceinline__ void prefetch_turn(const ChemArgs &a, double *sm_, long long bt, long long nbp, long long ncell) {\n"
          "  for (int q = threadIdx.x; q < " + I((nvar + 1) * 32) + "; q += " + I(NR * 32) + ") {\n"
          "    const int v = q >> 5, l = q & 31;\n"
-         "    const int patch = (int)(bt / nbp);\n"
+         "    const int patch = (int)(bt / nbp);      // relative to a.patch0\n"
          "    long long t = (bt - (long long)patch * nbp) * 32 + l;\n"
          "    if (t >= ncell) t = ncell - 1;\n"
          "    const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;\n"
          "    const int cj = (int)(r_ % a.n1), ck = (int)(r_ / a.n1);\n"
          "    const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;\n"
-         "    const double *src = v < " + I(nvar) + " ? a.U + ((long long)patch * " + I(nvar) + " + v) * a.pc + id : a.T + (long long)patch * a.pc + id;\n"
+         "    const double *src = v < " + I(nvar) + " ? a.U + ((long long)(patch + a.patch0) * " + I(nvar) + " + v) * a.pc + id : a.T + (long long)(patch + a.patch0) * a.pc + id;\n"
          "    const unsigned dst = (unsigned)__cvta_generic_to_shared(sm_ + (" + I(L.oNX) + " + v) * 32 + l);\n"
          "    asm volatile(\"cp.async.ca.shared.global [%0], [%1], 8;\" :: \"r\"(dst), \"l\"(src) : \"memory\");\n"
          "  }\n"
@@ -237,14 +237,14 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("const int *c_ri = s_ti + " + I(ori) + ", *c_fl = s_ti + " + I(ofl) + ", *c_re = s_ti + " + I(ore) + ", *c_pr = s_ti + " + I(opr) + ";");
   E.line("int *s_flag = (int *)(sm_ + " + I(L.oPIV * 32) + ");");
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2, nbp = (ncell + 31) / 32, nbt = nbp * a.np;");
-  E.line("const double dt = a.scal[0];");
+  E.line("const double dt = a.scal[0] * a.dts;");
   E.line("if ((long long)blockIdx.x < nbt) prefetch_turn(a, sm_, blockIdx.x, nbp, ncell);");
   E.line("asm volatile(\"cp.async.wait_all;\" ::: \"memory\");");
   E.line("BAR();");
   E.line("#pragma unroll 1");
   E.line("for (long long bt = blockIdx.x; bt < nbt; bt += gridDim.x) {   // persistent CTA: 32 cells per turn");
-  E.line("const int patch = (int)(bt / nbp);");
-  E.line("long long t = (bt - (long long)patch * nbp) * 32 + lane;");
+  E.line("const int patch = (int)(bt / nbp) + a.patch0;");
+  E.line("long long t = (bt - (long long)(patch - a.patch0) * nbp) * 32 + lane;");
   E.line("const bool live = t < ncell;");
   E.line("if (!live) t = ncell - 1;   // idle lanes recompute the last cell and store nothing");
   E.line("const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;");

@@ -47,6 +47,8 @@ struct MechC {
 // Geometry + device pointers handed to every kernel by value.
 struct Params {
   int ndim, nvar, ns, np, nlev, ratio;
+  int patch0;        // first patch the kernel acts on (block y + patch0); crossover advance: one level at a time
+  double dt_scale;   // the step of this launch = scal[0] * dt_scale (crossover advance: 1/2 on level 1)
   int n[3];          // interior cells per patch
   int P[3];          // padded dims
   int G[3];          // ghost width per dim (3 or 0)
@@ -58,12 +60,14 @@ struct Params {
   // device arrays
   double *T, *p, *vel;        // [np][pc], [np][pc], [ndim][np][pc]
   const int *level, *nbr, *parent, *fkind;
-  unsigned long long *slots;  // [2 parity][3 stage][2 lev][3 dir] ordered-int max(|u_d|+c)
+  unsigned long long *slots;  // [2 parity][2 sub-step][3 stage][2 lev][3 dir] ordered-int max(|u_d|+c)
   double *scal;               // [0]=dt, [1]=t accumulated
   int *flag;                  // device error flag
 };
 
-#define SLOT(par, stage, lev, d) ((((par) * 3 + (stage)) * 2 + (lev)) * 3 + (d))
+#define JANC_NSLOT 72        // per parity: 36 = 2 sub-steps (crossover advance: level 1 takes two) x 3 stages x 2 levels x 3 directions
+#define SLOTX(par, sub, stage, lev, d) (((((par) * 2 + (sub)) * 3 + (stage)) * 2 + (lev)) * 3 + (d))
+#define SLOT(par, stage, lev, d) SLOTX(par, 0, stage, lev, d)
 
 __device__ __forceinline__ long long cell_index(const Params &P, int i, int j, int k) {
   return (long long)(i + P.G[0]) * P.st[0] + (long long)(j + P.G[1]) * P.st[1] + (long long)(k + P.G[2]) * P.st[2];

@@ -133,11 +133,11 @@ k_flux_rk(Params P, const double *__restrict__ Uk, const double *U0, double *Uou
   double *sFp = flux_smem, *sFm = sFp + C::STAGE, *sL = sFm + C::STAGE;
 
   const int tid = threadIdx.x;
-  const int patch = blockIdx.y;
+  const int patch = blockIdx.y + P.patch0;
   const int lev = P.level[patch];
   const int ntx = (P.n[0] + TX - 1) / TX, nty = (P.n[1] + TY - 1) / TY;
   const int o0 = (blockIdx.x % ntx) * TX, o1 = ((blockIdx.x / ntx) % nty) * TY, o2 = (blockIdx.x / (ntx * nty)) * TZ;
-  const double dt = P.scal[0];
+  const double dt = P.scal[0] * P.dt_scale;
   const long long pbase = (long long)patch * P.pc;
   const double *Ukp = Uk + pbase * P.nvar;
   const double *U0p = U0 + pbase * P.nvar;
@@ -327,11 +327,11 @@ k_flux_rk2(Params P, const double *__restrict__ Uk, const double *U0, double *Uo
   unsigned char *sfl = (unsigned char *)(sc + C::BX * C::BY);             //         flip bits
 
   const int tid = threadIdx.x;
-  const int patch = blockIdx.y;
+  const int patch = blockIdx.y + P.patch0;
   const int lev = P.level[patch];
   const int ntx = (P.n[0] + TX - 1) / TX;
   const int o0 = (blockIdx.x % ntx) * TX, o1 = (blockIdx.x / ntx) * TY;
-  const double dt = P.scal[0];
+  const double dt = P.scal[0] * P.dt_scale;
   const long long pbase = (long long)patch * P.pc;
   const double *Ukp = Uk + pbase * P.nvar;
   const double *U0p = U0 + pbase * P.nvar;
@@ -497,11 +497,11 @@ k_flux_rk2_tma(Params P, const double *U0, double *Uout, int slot_base, double c
   unsigned long long *bars = (unsigned long long *)(sL + TY * C::LP);     // [0], [1]: U buffers (the first also p, u, v)
 
   const int tid = threadIdx.x;
-  const int patch = blockIdx.y;
+  const int patch = blockIdx.y + P.patch0;
   const int lev = P.level[patch];
   const int ntx = (P.n[0] + TX - 1) / TX;
   const int o0 = (blockIdx.x % ntx) * TX, o1 = (blockIdx.x / ntx) * TY;
-  const double dt = P.scal[0];
+  const double dt = P.scal[0] * P.dt_scale;
   const long long pbase = (long long)patch * P.pc;
   const double *U0p = U0 + pbase * P.nvar;
   double *Uop = Uout + pbase * P.nvar;

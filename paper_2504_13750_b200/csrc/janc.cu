@@ -56,6 +56,9 @@ struct janc_ctx {
   int *d_level, *d_nbr, *d_parent, *d_fkind;
   std::vector<int> level, nbr, parent, fkind;
   int parity;
+  int lvl_first[2] = {0, 0}, lvl_count[2] = {0, 0};   // patches of each level if they are contiguous (by_level)
+  bool by_level = true;
+  int act0 = 0, actn = 0;                             // patches the kernels of the current launches act on
   long long launches;
   int num_sms;
   // One step = 11..12 small launches; a step of each slot parity is captured once into a CUDA graph and replayed
@@ -151,6 +154,8 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
   Params &P = c->P;
   memset(&P, 0, sizeof P);
   P.ndim = grid->ndim; P.np = c->np; P.nlev = c->g.n_levels; P.ratio = c->g.ratio;
+  P.patch0 = 0; P.dt_scale = 1.0; c->act0 = 0; c->actn = c->np;
+  c->lvl_first[0] = 0; c->lvl_count[0] = c->np;
   P.pc = 1; c->ncell = 1;
   double dxmin = 1e300;
   for (int d = 0; d < 3; d++) {
@@ -262,7 +267,7 @@ static int fill_mech(const janc_mech *m, MechC &M, std::string &err) {
 // ------------------------------------------------------------------ run-time specialised chemistry
 // NVRTC is reached through dlopen so that libjanc.so loads (and the generic kernels run) where it is
 // absent; the cubin is loaded with the runtime's cudaLibrary API (no link against libcuda).
-struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np; };
+struct ChemArgs { double *U; double *T; const double *scal; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np, patch0; double dts; };
 
 struct NvrtcApi {
   void *h = nullptr;
@@ -317,8 +322,8 @@ static bool jit_compile(const std::string &src, std::vector<char> &cubin, std::s
 }
 
 struct PrimArgs { const double *U; double *T; double *p; double *vel; double *dbgc; unsigned long long *slots;
-                  const int *level; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np, reduce, slot_base; };
-struct SrcArgs { const double *Uk; double *Uout; const double *T; const double *scal; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; double coef; };
+                  const int *level; int *flag; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; int np, reduce, slot_base, patch0; };
+struct SrcArgs { const double *Uk; double *Uout; const double *T; const double *scal; int n0, n1, n2, G0, G1, G2; long long st0, st1, st2, pc; double coef; int patch0; };
 struct JitKernels { cudaKernel_t chem = nullptr, prim = nullptr, src = nullptr; };
 
 // 0: table-driven kernel, 1: register-resident specialised kernel (one thread per cell), 2: one thread per cell
@@ -509,7 +514,7 @@ static void carve(janc_ctx *c, char *base, size_t *total) {
   size_t oA = cv.take(cells * c->nvar * 8), oB = cv.take(cells * c->nvar * 8), oC = cv.take(cells * c->nvar * 8);
   size_t oT = cv.take(cells * 8), op = cv.take(cells * 8), ov = cv.take(cells * c->g.ndim * 8), oc = cv.take(cells * 8);
   size_t osU = cv.take((size_t)c->np * c->ncell * c->nvar * 8), osT = cv.take((size_t)c->np * c->ncell * 8);
-  size_t oslots = cv.take(36 * 8), oscal = cv.take(4 * 8), oflag = cv.take(16);
+  size_t oslots = cv.take(JANC_NSLOT * 8), oscal = cv.take(4 * 8), oflag = cv.take(16);
   size_t olev = cv.take(c->np * 4), onbr = cv.take(c->np * nf * 4), opar = cv.take(c->np * (1 + c->g.ndim) * 4), ofk = cv.take(c->np * nf * 4);
   if (total) *total = cv.off;
   if (base) {
@@ -585,7 +590,7 @@ static void launch_flux2_tma(janc_ctx *c, const double *Uk, const double *U0, do
   smem_attr(c, (const void *)k_flux_rk2_tma<TX, TY, SEG>, C::SMEM);
   const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY));
   const int which = Uk == c->A ? 0 : Uk == c->B ? 1 : 2;
-  k_flux_rk2_tma<TX, TY, SEG><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, U0, Uout, slot_base, coef, Uk == U0 ? 1 : 0,
+  k_flux_rk2_tma<TX, TY, SEG><<<dim3(tiles, (unsigned)c->actn, 1), C::NT, C::SMEM, c->stream>>>(P, U0, Uout, slot_base, coef, Uk == U0 ? 1 : 0,
                                                                                       c->mapU[which], c->mapP, c->mapV);
 }
 
@@ -643,6 +648,13 @@ extern "C" int janc_set_blocks(janc_ctx *c, const int32_t *level, const int32_t 
       }
       c->fkind[p * nf + f] = kind;
     }
+  // patches of a level contiguous (levels in non-decreasing order)?  The crossover advance launches one level at a time.
+  c->by_level = true;
+  c->lvl_first[0] = c->lvl_first[1] = 0; c->lvl_count[0] = c->lvl_count[1] = 0;
+  for (int p = 0; p < np; p++) {
+    if (p > 0 && c->level[p] < c->level[p - 1]) c->by_level = false;
+    if (c->lvl_count[c->level[p]]++ == 0) c->lvl_first[c->level[p]] = p;
+  }
   c->have_blocks = true;
   if (c->have_ws) return upload_lists(c);
   return JANC_OK;
@@ -672,7 +684,7 @@ extern "C" int janc_set_state(janc_ctx *c, const double *U, const double *Tg, in
   k_pack<<<pack_grid(c, c->np), 256, 0, c->stream>>>(c->P, dT, c->P.T, 1, 0, 1000.0);
   c->launches += 2;
   CK(cudaMemsetAsync(c->P.flag, 0, 4, c->stream));
-  CK(cudaMemsetAsync(c->P.slots, 0, 36 * 8, c->stream));
+  CK(cudaMemsetAsync(c->P.slots, 0, JANC_NSLOT * 8, c->stream));
   CK(cudaMemsetAsync(c->P.scal, 0, 4 * 8, c->stream));
   c->parity = 0;
   CK(cudaGetLastError());
@@ -752,15 +764,15 @@ static void smem_attr(janc_ctx *c, const void *fn, size_t bytes) {
 
 template <int NS>
 static void launch_prim(janc_ctx *c, const double *U, int reduce, int slot_base, double *dbgc) {
-  k_prim<NS><<<cell_grid(c, 256, c->np), 256, 0, c->stream>>>(c->P, U, reduce, slot_base, dbgc);
+  k_prim<NS><<<cell_grid(c, 256, c->actn), 256, 0, c->stream>>>(c->P, U, reduce, slot_base, dbgc);
 }
 static void do_prim(janc_ctx *c, const double *U, int reduce, int slot_base, double *dbgc, Prof *pf) {
   if (c->jit_prim) {
     const Params &P = c->P;
     PrimArgs a{U, P.T, P.p, P.vel, dbgc, P.slots, P.level, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2],
-               P.st[0], P.st[1], P.st[2], P.pc, P.np, reduce, slot_base};
+               P.st[0], P.st[1], P.st[2], P.pc, P.np, reduce, slot_base, c->act0};
     void *args[] = {&a};
-    note_launch(c, cudaLaunchKernel((const void *)c->jit_prim, cell_grid(c, 256, c->np), dim3(256, 1, 1), args, 0, c->stream));
+    note_launch(c, cudaLaunchKernel((const void *)c->jit_prim, cell_grid(c, 256, c->actn), dim3(256, 1, 1), args, 0, c->stream));
     prof_mark(c, pf, 0);
     return;
   }
@@ -782,7 +794,8 @@ static bool gather_mode(const janc_ctx *c) {
   return c->opt.halo_in_kernel && c->g.ndim == 2 && ((c->P.n[0] <= 16 && c->P.n[1] <= 16) || small_grid(c));
 }
 
-static void do_ghost(janc_ctx *c, double *U, Prof *pf) {
+// only_lev < 0: every level, coarse first (level 1 injects from its padded parent); else just that level
+static void do_ghost(janc_ctx *c, double *U, Prof *pf, int only_lev = -1) {
   if (gather_mode(c)) return;
   const int nd = c->g.ndim;
   int amax = 1;
@@ -794,6 +807,7 @@ static void do_ghost(janc_ctx *c, double *U, Prof *pf) {
   const long long total = (long long)2 * nd * JANC_NG * amax * ((c->nvar + 2 + nd + GHOST_FPT - 1) / GHOST_FPT);
   dim3 grid((unsigned)((total + 255) / 256), (unsigned)c->np, 1);
   for (int lev = 0; lev < c->g.n_levels; lev++) {
+    if (only_lev >= 0 && lev != only_lev) continue;
     k_ghost<<<grid, 256, 0, c->stream>>>(c->P, U, lev, amax);
     note_launch(c, cudaGetLastError());
   }
@@ -806,7 +820,7 @@ static void launch_flux(janc_ctx *c, const double *Uk, const double *U0, double 
   const Params &P = c->P;
   smem_attr(c, (const void *)k_flux_rk<NDIM, TX, TY, TZ, SEG>, C::SMEM);
   const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY) * ((P.n[2] + TZ - 1) / TZ));
-  k_flux_rk<NDIM, TX, TY, TZ, SEG><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
+  k_flux_rk<NDIM, TX, TY, TZ, SEG><<<dim3(tiles, (unsigned)c->actn, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
 }
 
 template <int TX, int TY, int SEG, bool GATHER = false>
@@ -815,7 +829,7 @@ static void launch_flux2(janc_ctx *c, const double *Uk, const double *U0, double
   const Params &P = c->P;
   smem_attr(c, (const void *)k_flux_rk2<TX, TY, SEG, GATHER>, C::SMEM);
   const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY));
-  k_flux_rk2<TX, TY, SEG, GATHER><<<dim3(tiles, (unsigned)c->np, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
+  k_flux_rk2<TX, TY, SEG, GATHER><<<dim3(tiles, (unsigned)c->actn, 1), C::NT, C::SMEM, c->stream>>>(P, Uk, U0, Uout, slot_base, coef);
 }
 
 static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef, Prof *pf) {
@@ -840,21 +854,21 @@ static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uou
 
 template <int NS>
 static void launch_chem(janc_ctx *c, double *U) {
-  k_chem<NS><<<cell_grid(c, 128, c->np), 128, 0, c->stream>>>(c->P, U);
+  k_chem<NS><<<cell_grid(c, 128, c->actn), 128, 0, c->stream>>>(c->P, U);
 }
 template <int NS>
 static void launch_chem_reg(janc_ctx *c, double *U) {
   constexpr int NT = 64;
   const size_t smem = (size_t)(NS + 2 * c->nr + c->mech.ntb) * NT * sizeof(double);
   smem_attr(c, (const void *)k_chem_reg<NS, NT>, 227 * 1024);
-  k_chem_reg<NS, NT><<<cell_grid(c, NT, c->np), NT, smem, c->stream>>>(c->P, U);
+  k_chem_reg<NS, NT><<<cell_grid(c, NT, c->actn), NT, smem, c->stream>>>(c->P, U);
 }
 static void do_chem(janc_ctx *c, double *U, Prof *pf) {
   if (c->jit_kernel) {
     const Params &P = c->P;
-    ChemArgs a{U, P.T, P.scal, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc, c->np};
+    ChemArgs a{U, P.T, P.scal, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc, c->actn, c->act0, P.dt_scale};
     void *args[] = {&a};
-    dim3 grid = cell_grid(c, c->jit_chem_cells, c->np);
+    dim3 grid = cell_grid(c, c->jit_chem_cells, c->actn);
     if (c->jit_chem_mode == 3) {      // persistent CTAs, one per SM, each takes 32-cell turns
       const long long turns = (long long)grid.x * grid.y;
       grid = dim3((unsigned)(turns < c->num_sms ? turns : c->num_sms), 1, 1);
@@ -876,39 +890,71 @@ static void do_chem(janc_ctx *c, double *U, Prof *pf) {
 // explicit variant: add coef dt S(Uk) to the stage result on the species rows
 static void do_src(janc_ctx *c, const double *Uk, double *Uout, double coef, Prof *pf) {
   const Params &P = c->P;
-  SrcArgs a{Uk, Uout, P.T, P.scal, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc, coef};
+  SrcArgs a{Uk, Uout, P.T, P.scal, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc, coef * P.dt_scale, c->act0};
   void *args[] = {&a};
-  note_launch(c, cudaLaunchKernel((const void *)c->jit_src, cell_grid(c, 128, c->np), dim3(128, 1, 1), args, 0, c->stream));
+  note_launch(c, cudaLaunchKernel((const void *)c->jit_src, cell_grid(c, 128, c->actn), dim3(128, 1, 1), args, 0, c->stream));
   prof_mark(c, pf, 3);
 }
 
-// advance_one_step: cfl -> advance_flux (RK3 over rhs) -> advance_source_term
-static void step_once(janc_ctx *c, double cfl, double dt_fixed, int flags, Prof *pf) {
-  const int par = c->parity;
-  prof_mark(c, pf, -1);
-  // stage 0: update_aux on U^n (also the cfl() evaluation), dt, ghost fill, fluxes
-  do_prim(c, c->A, 1, SLOT(par, 0, 0, 0), nullptr, pf);
-  k_dt<<<1, 32, 0, c->stream>>>(c->P, par, cfl, dt_fixed);
-  note_launch(c, cudaGetLastError());
-  prof_mark(c, pf, 0);
-  do_ghost(c, c->A, pf);
+static void set_active(janc_ctx *c, int first, int count, double dt_scale) {
+  c->act0 = first; c->actn = count;
+  c->P.patch0 = first; c->P.dt_scale = dt_scale;
+}
+
+// advance_flux (TVD-RK3 over rhs) + advance_source_term of the active patches, A -> A.
+// sub: which reduction-slot set the stages use; first_prim: evaluate update_aux of A (false: the caller's evaluation at
+// the start of the step is still valid for these patches); glev: ghost-fill level (-1: all levels, coarse first)
+static void advance_active(janc_ctx *c, int par, int sub, bool first_prim, int glev, int flags, Prof *pf) {
   const bool esrc = (flags & 2) && c->jit_src && c->ns > 1 && c->nr > 0;   // source inside every stage
-  do_flux(c, c->A, c->A, c->B, SLOT(par, 0, 0, 0), 1.0, pf);
+  if (first_prim) do_prim(c, c->A, 1, SLOTX(par, sub, 0, 0, 0), nullptr, pf);
+  do_ghost(c, c->A, pf, glev);
+  do_flux(c, c->A, c->A, c->B, SLOTX(par, sub, 0, 0, 0), 1.0, pf);
   if (esrc) do_src(c, c->A, c->B, 1.0, pf);
-  // stage 1
-  do_prim(c, c->B, 1, SLOT(par, 1, 0, 0), nullptr, pf);
-  do_ghost(c, c->B, pf);
-  do_flux(c, c->B, c->A, c->C, SLOT(par, 1, 0, 0), 0.25, pf);
+  do_prim(c, c->B, 1, SLOTX(par, sub, 1, 0, 0), nullptr, pf);
+  do_ghost(c, c->B, pf, glev);
+  do_flux(c, c->B, c->A, c->C, SLOTX(par, sub, 1, 0, 0), 0.25, pf);
   if (esrc) do_src(c, c->B, c->C, 0.25, pf);
-  // stage 2 (writes U* over U^n in place: each cell reads its own U^n before writing)
-  do_prim(c, c->C, 1, SLOT(par, 2, 0, 0), nullptr, pf);
-  do_ghost(c, c->C, pf);
-  do_flux(c, c->C, c->A, c->A, SLOT(par, 2, 0, 0), 2.0 / 3.0, pf);
+  // stage 3 writes U* over U^n in place: each cell reads its own U^n before writing
+  do_prim(c, c->C, 1, SLOTX(par, sub, 2, 0, 0), nullptr, pf);
+  do_ghost(c, c->C, pf, glev);
+  do_flux(c, c->C, c->A, c->A, SLOTX(par, sub, 2, 0, 0), 2.0 / 3.0, pf);
   if (esrc) do_src(c, c->C, c->A, 2.0 / 3.0, pf);
   // advance_source_term: T* inside the chemistry kernel; explicit variant: only refresh aux
   const bool chem = !(flags & 3) && c->ns > 1 && c->nr > 0;
   if (chem) do_chem(c, c->A, pf);
   else do_prim(c, c->A, 0, 0, nullptr, pf);
+}
+
+// advance_one_step: cfl -> advance_flux (RK3 over rhs) -> advance_source_term.
+// flags bit 2: crossover advance of a two-level block list (Fig 2a, reading B9): two half steps of level 1
+// with its coarse-fine ghosts taken from the level-0 state at the start of the step, then one step of level 0.
+static void step_once(janc_ctx *c, double cfl, double dt_fixed, int flags, Prof *pf) {
+  const int par = c->parity;
+  const bool crossover = (flags & 4) && c->g.n_levels == 2 && c->lvl_count[1] > 0;
+  prof_mark(c, pf, -1);
+  // update_aux on U^n of every patch (also the cfl() evaluation), then dt
+  set_active(c, 0, c->np, 1.0);
+  do_prim(c, c->A, 1, SLOTX(par, 0, 0, 0, 0), nullptr, pf);
+  k_dt<<<1, 32, 0, c->stream>>>(c->P, par, cfl, dt_fixed, crossover ? (double)c->g.ratio : 1.0);
+  note_launch(c, cudaGetLastError());
+  prof_mark(c, pf, 0);
+  if (!crossover) {
+    advance_active(c, par, 0, false, -1, flags, pf);
+  } else {
+    // level 0 keeps its state at t^n in all three RK registers while level 1 runs: stages 2 and 3 of level 1 read
+    // their coarse-fine ghosts from B and C
+    do_ghost(c, c->A, pf, 0);
+    const size_t off = (size_t)c->lvl_first[0] * c->nvar * c->P.pc, cnt = (size_t)c->lvl_count[0] * c->nvar * c->P.pc * sizeof(double);
+    cudaMemcpyAsync(c->B + off, c->A + off, cnt, cudaMemcpyDeviceToDevice, c->stream);
+    cudaMemcpyAsync(c->C + off, c->A + off, cnt, cudaMemcpyDeviceToDevice, c->stream);
+    prof_mark(c, pf, 1);
+    set_active(c, c->lvl_first[1], c->lvl_count[1], 0.5);
+    advance_active(c, par, 0, false, 1, flags, pf);
+    advance_active(c, par, 1, true, 1, flags, pf);
+    set_active(c, c->lvl_first[0], c->lvl_count[0], 1.0);
+    advance_active(c, par, 0, false, 0, flags, pf);
+    set_active(c, 0, c->np, 1.0);
+  }
   if (c->g.n_levels > 1) {
     const int r = c->g.ratio, nd = c->g.ndim;
     long long nc = c->ncell;
@@ -983,6 +1029,10 @@ extern "C" int janc_step(janc_ctx *c, int nsteps, double cfl, double dt_fixed, i
   int rc = check_ready(c);
   if (rc) return rc;
   if (nsteps < 0 || (!(cfl > 0.0) && !(dt_fixed > 0.0))) { c->err = "need cfl > 0 or dt_fixed > 0"; return JANC_EINVAL; }
+  if ((flags & 4) && c->g.n_levels == 2 && !c->by_level) {
+    c->err = "the crossover advance needs the patches ordered by level (all level-0 patches first)";
+    return JANC_EINVAL;
+  }
   if ((flags & 2) && c->ns > 1 && c->nr > 0) jit_setup_source(c);
   if ((flags & 2) && c->ns > 1 && c->nr > 0 && !c->jit_src) {
     c->err = "explicit source variant needs the run-time specialised kernel (NVRTC): " + c->jit_log;

@@ -84,7 +84,7 @@ __device__ __forceinline__ bool cons2prim(const Params &P, const double *__restr
 template <int NS>
 __global__ void __launch_bounds__(256) k_prim(Params P, const double *__restrict__ U, int reduce, int slot_base,
                                               double *dbgc) {
-  const int patch = blockIdx.y;
+  const int patch = blockIdx.y + P.patch0;
   const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   double s[3] = {0.0, 0.0, 0.0};
@@ -127,17 +127,17 @@ __global__ void __launch_bounds__(256) k_prim(Params P, const double *__restrict
 
 // One thread: dt from the step-start maxima (cfl mode) or the fixed value; accumulates t; clears the
 // other parity's reduction slots for the next step.
-__global__ void k_dt(Params P, int parity, double cfl, double dt_fixed) {
+__global__ void k_dt(Params P, int parity, double cfl, double dt_fixed, double dx_factor) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
     double dt = dt_fixed;
     if (cfl > 0.0) {
       double smax = 0.0;
       for (int l = 0; l < 2; l++)
         for (int d = 0; d < P.ndim; d++) smax = fmax(smax, slot_value(P.slots + SLOT(parity, 0, l, d)));
-      dt = cfl * P.dxmin / smax;
+      dt = cfl * (P.dxmin * dx_factor) / smax;     // dx_factor = ratio for the crossover advance (the level-0 step)
     }
     P.scal[0] = dt;
     P.scal[1] += dt;
-    for (int q = 0; q < 18; q++) P.slots[SLOT(1 - parity, 0, 0, 0) + q] = 0ull;
+    for (int q = 0; q < JANC_NSLOT / 2; q++) P.slots[SLOT(1 - parity, 0, 0, 0) + q] = 0ull;
   }
 }

@@ -56,6 +56,26 @@ def test_cfg3_full_size_50_steps(B, ref):
     march(B, ref, case, (1, 50), (TOL1, TOL100))
 
 
+def test_cfg3_full_size_crossover_advance(B, ref):
+    """configs[3] at full size with the crossover (sub-cycled) advance, Fig 2a: 1 and 12 level-0 steps
+    (the physical time of 24 synchronous steps)."""
+    case = I.config3()
+    g = B.Solver(case.grid, case.mech, case.blocks)
+    g.set_state(case.U, case.T)
+    r = ref.RefSolver(case.grid, case.mech, case.blocks)
+    r.set_state(case.U, case.T)
+    done = 0
+    for mark, tol in ((1, TOL1), (12, TOL100)):
+        tg = g.step(mark - done, cfl=case.cfl, crossover=True)
+        tr = r.step(mark - done, cfl=case.cfl, crossover=True)
+        done = mark
+        Ug, Tg = g.get_state(); Ur, Tr = r.get_state()
+        assert g.status == 0 and r.status == 0 and abs(tg - tr) <= 1e-12 * tr
+        e = field_errors(case, Ug, Ur)
+        assert e.max() <= tol, (mark, e)
+    g.close(); r.close()
+
+
 def test_cfg4_full_size_flux_path_element_by_element(B, ref):
     """configs[4] at 256^3, 20 species: ONE full RK3 step of the 3-D flux path (cons->prim, ghost fill, k_flux_rk
     <3,16,8,8,8>, three stages) compared with the oracle on all 16.7 M cells x 24 fields.  The oracle's point-implicit

@@ -40,17 +40,17 @@ def field_errors(case, Ug, Ur):
     return np.array(errs)
 
 
-def both(B, ref, case, nsteps, chem=True, cfl=None, dt=0.0, options=None):
+def both(B, ref, case, nsteps, chem=True, cfl=None, dt=0.0, options=None, crossover=False):
     cfl = case.cfl if cfl is None else cfl
     g = B.Solver(case.grid, case.mech, case.blocks, options=options)
     g.set_state(case.U, case.T)
-    tg = g.step(nsteps, cfl=cfl, dt=dt, chem=chem)
+    tg = g.step(nsteps, cfl=cfl, dt=dt, chem=chem, crossover=crossover)
     Ug, Tg = g.get_state()
     assert g.status == 0, "device flag raised"
     g.close()
     r = ref.RefSolver(case.grid, case.mech, case.blocks)
     r.set_state(case.U, case.T)
-    tr = r.step(nsteps, cfl=cfl, dt=dt, chem=chem)
+    tr = r.step(nsteps, cfl=cfl, dt=dt, chem=chem, crossover=crossover)
     Ur, Tr = r.get_state()
     assert r.status == 0
     assert abs(tg - tr) <= 1e-12 * tr, (tg, tr)
@@ -459,3 +459,42 @@ def test_degenerate_mechanisms(B, ref, mech9):
     g3 = I.Grid(2, (40, 3, 1), base.grid.dx, base.grid.bc_lo, base.grid.bc_hi)     # three rows of cells in y
     thin = I.Case("three_rows", g3, mech9, base.U[:, :, :, :3, :40].copy(), base.T[:, :, :3, :40].copy(), base.cfl, 2)
     check(B, ref, thin, 2, TOL1 * 10)
+
+
+# ------------------------------------------------------------------ crossover (sub-cycled) level advance
+def test_crossover_advance_parity(B, ref):
+    """PAPER.md:186 Fig 2a: two half steps of level 1, then one step of level 0, per janc_step iteration.  Same parity
+    bar against the oracle's crossover mode: 2-D block list with the halo gathered in the flux kernel and with k_ghost,
+    32 x 32 patches (TMA tiles), 1-D and 3-D two-level lists, the explicit-source variant, fixed dt; a single level
+    ignores the flag; patches not ordered by level are refused."""
+    c3 = I.config3(pcols=16, prows=8, npc=16)
+    check(B, ref, c3, 1, TOL1, crossover=True)
+    check(B, ref, c3, 10, TOL100, crossover=True)
+    check(B, ref, c3, 4, TOL100, crossover=True, options={"halo": "ghost"})
+    check(B, ref, c3, 3, TOL100, crossover=True, cfl=0.0, dt=4.0e-9, chem="explicit")
+    check(B, ref, I.config3(pcols=8, prows=4, npc=32), 3, TOL100, crossover=True)
+    base = I.config0(n=192)
+    base.grid.bc_lo, base.grid.bc_hi = (I.BC_REFLECT, 0, 0), (I.BC_OUTFLOW, 0, 0)
+    mask = np.zeros(12, bool); mask[4:8] = True; mask[0] = True
+    check(B, ref, I.refine_uniform(base, (16,), mask), 10, TOL100, crossover=True)
+    b3 = I.config4(n=16, nspheres=2, radius=4)
+    m3 = np.zeros((2, 2, 2), bool); m3[0, 1, 0] = m3[1, 1, 0] = m3[1, 0, 1] = True
+    check(B, ref, I.refine_uniform(b3, (8, 8, 8), m3), 2, TOL1 * 100, crossover=True)
+    # one level: the flag changes nothing
+    c1 = I.config1(nx=64, ny=32)
+    g = B.Solver(c1.grid, c1.mech); g.set_state(c1.U, c1.T); ta = g.step(3, cfl=c1.cfl); Ua, _ = g.get_state()
+    g.set_state(c1.U, c1.T); tb = g.step(3, cfl=c1.cfl, crossover=True); Ub, _ = g.get_state(); g.close()
+    assert ta == tb and np.array_equal(Ua, Ub)
+    # level order
+    perm = np.arange(c3.grid.n_patches)[::-1].copy()
+    inv = np.empty_like(perm); inv[perm] = np.arange(len(perm))
+    blk = c3.blocks
+    nbr = np.where(blk.nbr[perm] >= 0, inv[np.maximum(blk.nbr[perm], 0)], -1)
+    par = blk.parent[perm].copy(); par[:, 0] = np.where(par[:, 0] >= 0, inv[np.maximum(par[:, 0], 0)], -1)
+    rev = I.Case("rev", c3.grid, c3.mech, c3.U[perm], c3.T[perm], c3.cfl, 1, blocks=I.Blocks(blk.level[perm], nbr.astype(np.int32), par.astype(np.int32)))
+    check(B, ref, rev, 2, TOL1 * 10)                                    # the synchronous advance takes any order
+    g = B.Solver(rev.grid, rev.mech, rev.blocks); g.set_state(rev.U, rev.T)
+    with pytest.raises(B.JancError) as e:
+        g.step(1, cfl=rev.cfl, crossover=True)
+    assert e.value.code == B.JANC_EINVAL
+    g.close()
