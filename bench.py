@@ -267,6 +267,61 @@ def measure(binding, case, K, W, local, world, barrier, do_e2e=True, crossover=F
     return out
 
 
+def measure_slab(binding, case, K, W, local, rank, world, barrier):
+    """x-slab decomposition (slab.py): this rank's workload is one slab of a grid `world` times as long in x; per RK stage
+    the 3 boundary columns go to the x neighbours (NCCL send / recv) and the reduction slots are max-all-reduced."""
+    import torch
+    from paper_2504_13750_b200 import slab
+    g = case.grid
+    assert g.n_patches == 0, "--parallel slab needs a uniform-grid workload"
+    periodic = g.bc_lo[0] == I.BC_PERIODIC
+    left, right = slab.neighbours(rank, world, periodic)
+    lo, hi = list(g.bc_lo), list(g.bc_hi)
+    if left is not None:
+        lo[0] = binding.BC_EXCHANGE
+    if right is not None:
+        hi[0] = binding.BC_EXCHANGE
+    lc = I.Case(case.name, I.Grid(g.ndim, g.n, g.dx, tuple(lo), tuple(hi)), case.mech, case.U, case.T, case.cfl, case.nsteps)
+    run = slab.SlabRun(None, slab.DistComm(), device=local, local=[(lc, (rank * g.n[0], (rank + 1) * g.n[0]), (left, right))])
+    s = run.solvers[0]
+    out = {"chem_kernel": s.chem_kernel()}
+    for _ in range(W):
+        run.step(1, cfl=case.cfl)
+    assert s.status_sync() == 0
+    l0 = s.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    run.step(K, cfl=case.cfl)
+    e1.record()
+    barrier()
+    out["ms"] = e0.elapsed_time(e1)
+    out["launches"] = s.launch_count() - l0
+    assert s.status_sync() == 0
+    phases = {}
+    for _ in range(K):      # per-kernel device times of this rank's slab advanced on its own (same kernels, stale halos)
+        for k, (t, n) in s.profile_step(cfl=case.cfl).items():
+            a = phases.setdefault(k, [0.0, 0]); a[0] += t; a[1] += n
+    out["phases"] = phases
+    # end to end: host -> device, K steps with exchange, device -> host
+    Uh = torch.from_numpy(case.U).pin_memory(); Th = torch.from_numpy(case.T).pin_memory()
+    Uo = torch.empty_like(Uh).pin_memory()
+    Ke = max(1, min(K, 5))
+    barrier()
+    e0.record()
+    for _ in range(Ke):
+        s.set_state(Uh.numpy(), Th.numpy())
+        run.step(1, cfl=case.cfl)
+        rc = s.get_state_into(Uo.numpy())
+    e1.record()
+    barrier()
+    assert rc == 0
+    out["ms_e2e"] = e0.elapsed_time(e1); out["Ke"] = Ke
+    out["h2d"] = int(Uh.numel() * 8 + Th.numel() * 8); out["d2h"] = int(Uo.numel() * 8)
+    run.close()
+    return out
+
+
 def rooflines(case, m, K, dfma, hbm_peak, hbm_src):
     """Per-kernel roofline entries of one measured workload: algorithmic fp64 instructions and
     bytes per launch / the kernel's average launch duration (CUDA events, m["phases"]) against the DFMA rate measured
@@ -310,6 +365,10 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (N = 1 only)")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default; north_star keeps the path on one GPU) or the paper's x-slab "
+                         "decomposition with halo exchange and max all-reduce over NCCL (PAPER.md:359-378), weak scaling: "
+                         "every rank owns one workload-sized slab of a grid N times as long in x")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -342,7 +401,10 @@ def main():
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
         sampler.start()
-    m = measure(binding, case, K, W, local, world, barrier)
+    if args.parallel == "slab" and world > 1:
+        m = measure_slab(binding, case, K, W, local, rank, world, barrier)
+    else:
+        m = measure(binding, case, K, W, local, world, barrier)
     if sampler:           # clocks are sampled over the event-timed, the per-kernel and the end-to-end regions
         sampler.stop_flag = True
         sampler.join()
@@ -370,7 +432,9 @@ def main():
                 "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": case.name, "cells": cells, "ns": case.mech.ns, "nr": case.mech.nr,
-                           "nvar": nvar, "cfl": case.cfl, "parallelism": f"replicas x{world}",
+                           "nvar": nvar, "cfl": case.cfl,
+                           "parallelism": (f"x-slab decomposition x{world} (halo exchange + max all-reduce per RK stage, NCCL)"
+                                           if args.parallel == "slab" and world > 1 else f"replicas x{world}"),
                            "l2": "state %.0f MB per register > 126 MB L2" % (cells * nvar * 8 / 1e6)
                                  if cells * nvar * 8 > 126e6 else "state fits L2 (no flush; noted)"},
                 "clocks": sampler.summary(),

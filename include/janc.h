@@ -42,7 +42,8 @@ enum { JANC_OK = 0, JANC_EINVAL = -1, JANC_ENOMEM = -2, JANC_ECUDA = -3, JANC_ES
  * expressed through the neighbour lists), REFLECT mirrors about the face and negates the normal
  * momentum (slip wall), OUTFLOW copies the nearest interior cell (zero gradient,
  * the paper's "non-reflecting"). */
-enum { JANC_BC_PERIODIC = 0, JANC_BC_REFLECT = 1, JANC_BC_OUTFLOW = 2 };
+enum { JANC_BC_PERIODIC = 0, JANC_BC_REFLECT = 1, JANC_BC_OUTFLOW = 2,
+       JANC_BC_EXCHANGE = 3 /* x sides of a uniform grid only: the ghost columns are filled by janc_halo (x-slab decomposition) */ };
 
 typedef struct {
   int ndim;               /* 1, 2 or 3 (paper: 2; reading A18)                     */
@@ -124,6 +125,30 @@ int janc_set_state(janc_ctx *, const double *U, const double *T_guess, int on_de
  * on a single level.
  * t_advanced (host, nullable): receives the sum of dt; forces a stream synchronise. */
 int janc_step(janc_ctx *, int nsteps, double cfl, double dt_fixed, int flags, double *t_advanced);
+
+/* x-slab decomposition over several GPUs (split_grid, exchange_halo, parallel_rhs; one process per
+ * GPU).  Every rank owns a slab of the grid along x with JANC_BC_EXCHANGE on its interior x sides and advances it with
+ * janc_step_part instead of janc_step; between the parts the caller (paper_2504_13750_b200/slab.py: torch.distributed over
+ * NCCL) max-reduces the reduction slots over the ranks and swaps the halo buffers.  Per step:
+ *   PRIM(0) -> [all-reduce max of the slots] -> DT ->
+ *   for stage s = 0, 1, 2:  (s > 0: PRIM(s) -> [all-reduce]) -> GHOST(s) -> janc_halo pack lo / hi ->
+ *                           [send / receive] -> janc_halo unpack lo / hi -> FLUX(s)
+ *   -> SOURCE.
+ * The slots hold max(|u_d| + c) as the bit pattern of a non-negative double, which orders like an unsigned integer:
+ * an integer MAX all-reduce is exact, so every rank computes the same dt and the same alpha as the undecomposed grid.
+ * flags: 0, or 1 = no chemistry.  Uniform grids only; eager launches (no graph). */
+enum { JANC_PART_PRIM = 0, JANC_PART_DT = 1, JANC_PART_GHOST = 2, JANC_PART_FLUX = 3, JANC_PART_SOURCE = 4 };
+int janc_step_part(janc_ctx *, int part, int stage, double cfl, double dt_fixed, int flags);
+/* Doubles in one halo buffer: (nvar + 2 + ndim) fields (U, T, p, u_d) x 3 columns x ny x nz. */
+size_t janc_halo_doubles(const janc_ctx *);
+/* unpack = 0: copy the 3 interior columns next to x side `side` (0 lo, 1 hi) of RK register `stage` (0 = U^n, 1 = U^(1),
+ * 2 = U^(2)) and of T, p, u_d into the device buffer; unpack = 1: copy the buffer into the ghost columns of that side. */
+int janc_halo(janc_ctx *, int stage, int side, double *buf_dev, int unpack);
+/* Where the reduction slots sit inside the bound workspace (byte offset, number of 64-bit slots). */
+int janc_reduction_slots(const janc_ctx *, size_t *byte_offset, size_t *count);
+
+/* dt of the most recent step (cfl()), read from the device; synchronises. */
+int janc_last_dt(janc_ctx *, double *dt);
 
 /* Read the state back (U and/or T nullable).  Synchronises.  Returns JANC_ENONFINITE if the
  * device flag was raised since the last janc_set_state. */

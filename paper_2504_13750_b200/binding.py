@@ -19,9 +19,12 @@ JANC_OK, JANC_EINVAL, JANC_ENOMEM, JANC_ECUDA, JANC_ESTATE, JANC_ENONFINITE = 0,
 FLAG_NO_CHEM = 1
 FLAG_EXPLICIT_SOURCE = 2
 FLAG_CROSSOVER = 4
+PART_PRIM, PART_DT, PART_GHOST, PART_FLUX, PART_SOURCE = range(5)
+BC_EXCHANGE = 3
 
 EXPORTS = ["janc_create", "janc_set_option", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
-           "janc_set_blocks", "janc_set_state", "janc_step", "janc_get_state", "janc_status",
+           "janc_set_blocks", "janc_set_state", "janc_step", "janc_step_part", "janc_halo_doubles", "janc_halo",
+           "janc_reduction_slots", "janc_last_dt", "janc_get_state", "janc_status",
            "janc_launch_count", "janc_debug_cons2prim", "janc_profile_step",
            "janc_measure_dfma_peak", "janc_chem_kernel", "janc_jit_log", "janc_jit_probe",
            "janc_last_error", "janc_destroy"]
@@ -64,6 +67,12 @@ def lib():
         L.janc_set_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.janc_step.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int, C.c_void_p]
         L.janc_get_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.janc_step_part.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int]
+        L.janc_halo_doubles.argtypes = [C.c_void_p]
+        L.janc_halo_doubles.restype = C.c_size_t
+        L.janc_halo.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]
+        L.janc_reduction_slots.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.janc_last_dt.argtypes = [C.c_void_p, C.c_void_p]
         L.janc_status.argtypes = [C.c_void_p]
         L.janc_launch_count.argtypes = [C.c_void_p]
         L.janc_launch_count.restype = C.c_longlong
@@ -156,6 +165,7 @@ class Solver:
         nbytes = L.janc_workspace_bytes(self._h)
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{self.device}")
         base = (self.workspace.data_ptr() + 255) // 256 * 256
+        self._ws_off = base - self.workspace.data_ptr()
         self._check(L.janc_bind_workspace(self._h, C.c_void_p(base), nbytes), "janc_bind_workspace")
         if blocks is not None:
             self._check(L.janc_set_blocks(self._h, _ptr(_i32(blocks.level)), _ptr(_i32(blocks.nbr)),
@@ -215,6 +225,32 @@ class Solver:
             return t.value
         self._check(lib().janc_step(self._h, int(nsteps), float(cfl), float(dt), flags, None), "janc_step")
         return None
+
+    # -- x-slab decomposition (janc_step_part / janc_halo / janc_reduction_slots) -------------
+    def step_part(self, part, stage=0, cfl=0.0, dt=0.0, chem=True):
+        self._check(lib().janc_step_part(self._h, int(part), int(stage), float(cfl), float(dt), 0 if chem else FLAG_NO_CHEM),
+                    "janc_step_part")
+
+    def halo_doubles(self):
+        return lib().janc_halo_doubles(self._h)
+
+    def halo(self, stage, side, buf, unpack):
+        """buf: contiguous float64 CUDA tensor of halo_doubles() elements."""
+        assert buf.is_cuda and buf.dtype == self._torch.float64 and buf.is_contiguous() and buf.numel() >= self.halo_doubles()
+        self._check(lib().janc_halo(self._h, int(stage), int(side), C.c_void_p(buf.data_ptr()), int(bool(unpack))), "janc_halo")
+
+    def slots_tensor(self):
+        """The reduction slots as an int64 view into the workspace (non-negative doubles order like their bit patterns)."""
+        off, cnt = C.c_size_t(0), C.c_size_t(0)
+        self._check(lib().janc_reduction_slots(self._h, C.byref(off), C.byref(cnt)), "janc_reduction_slots")
+        a = self._ws_off + off.value
+        return self.workspace[a:a + 8 * cnt.value].view(self._torch.int64)
+
+    def last_dt(self):
+        """dt of the most recent step (device scalar), synchronising."""
+        t = C.c_double(0.0)
+        self._check(lib().janc_last_dt(self._h, C.byref(t)), "janc_last_dt")
+        return t.value
 
     def get_state(self, device=False):
         if device:

@@ -38,6 +38,7 @@ __global__ void __launch_bounds__(256) k_ghost(Params P, double *__restrict__ U,
   src[0] = dst[0]; src[1] = dst[1]; src[2] = dst[2];
   const int kind = P.fkind[patch * nf + f];
   const int bc = side == 0 ? P.bc_lo[d] : P.bc_hi[d];
+  if (kind == FK_PHYSICAL && bc == 3) return;      // exchange face: filled by k_halo from the neighbouring slab's buffer
   int q = patch;
   bool flip = false;
   if (kind == FK_NEIGHBOUR || (kind == FK_PHYSICAL && bc == 0 /*periodic*/)) {
@@ -99,4 +100,24 @@ __global__ void __launch_bounds__(256) k_average_down(Params P, double *__restri
     for (int jj = 0; jj < rr[1]; jj++)
       for (int ii = 0; ii < rr[0]; ii++) s += src[cell_index(P, i * rr[0] + ii, j * rr[1] + jj, k * rr[2] + kk)];
   U[((long long)q * P.nvar + v) * P.pc + cell_index(P, off[0] + i, off[1] + j, off[2] + k)] = s * (1.0 / (rr[0] * rr[1] * rr[2]));
+}
+
+
+// x-slab decomposition (split_grid / exchange_halo): the 3 interior columns next to x side `side`
+// of every field (U components, T, p, u_d) <-> a contiguous buffer [field][3][nz][ny].  pack: interior -> buffer (what
+// the neighbouring slab needs); unpack: buffer -> the ghost columns of that side.  Uniform grid (one patch) only.
+__global__ void __launch_bounds__(256) k_halo(Params P, double *__restrict__ U, double *__restrict__ buf, int side, int unpack) {
+  const int nfield = P.nvar + 2 + P.ndim;
+  const int rows = P.n[1] * P.n[2];
+  const long long total = (long long)nfield * JANC_NG * rows;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= total) return;
+  const int r = (int)(idx % rows), g = (int)((idx / rows) % JANC_NG), fld = (int)(idx / ((long long)rows * JANC_NG));
+  const int j = r % P.n[1], k = r / P.n[1];
+  // pack: lo side sends columns 0..2, hi side columns n-3..n-1; unpack: lo ghosts -3..-1, hi ghosts n..n+2
+  const int i = unpack ? (side == 0 ? -JANC_NG + g : P.n[0] + g) : (side == 0 ? g : P.n[0] - JANC_NG + g);
+  const long long ci = cell_index(P, i, j, k);
+  double *arr = fld < P.nvar ? U + (long long)fld * P.pc : fld == P.nvar ? P.T : fld == P.nvar + 1 ? P.p : P.vel + (long long)(fld - P.nvar - 2) * P.np * P.pc;
+  if (unpack) arr[ci] = buf[idx];
+  else buf[idx] = arr[ci];
 }

@@ -168,7 +168,9 @@ extern "C" int janc_create(const janc_grid *grid, int device, void *cuda_stream,
       double dxf = c->g.n_levels == 2 ? dx / c->g.ratio : dx;
       if (dxf < dxmin) dxmin = dxf;
       P.bc_lo[d] = grid->bc_lo[d]; P.bc_hi[d] = grid->bc_hi[d];
-      if (P.bc_lo[d] < 0 || P.bc_lo[d] > 2 || P.bc_hi[d] < 0 || P.bc_hi[d] > 2) { delete c; return JANC_EINVAL; }
+      if (P.bc_lo[d] < 0 || P.bc_lo[d] > 3 || P.bc_hi[d] < 0 || P.bc_hi[d] > 3) { delete c; return JANC_EINVAL; }
+      // exchange faces (x-slab decomposition): x sides of a uniform grid only
+      if ((P.bc_lo[d] == JANC_BC_EXCHANGE || P.bc_hi[d] == JANC_BC_EXCHANGE) && (d != 0 || grid->n_patches > 0)) { delete c; return JANC_EINVAL; }
       // 3 ghost layers are copied from 3 distinct interior cells by the periodic / mirror / neighbour rules;
       // only zero-gradient sides work on thinner grids (e.g. the one-cell 0-D reactor)
       const bool thin_ok = grid->n_patches <= 0 && P.bc_lo[d] == 2 && P.bc_hi[d] == 2;
@@ -791,6 +793,7 @@ static void do_prim(janc_ctx *c, const double *U, int reduce, int slot_base, dou
 // (flux.cuh, GATHER); no ghost fill
 static bool small_grid(const janc_ctx *c) { return (long long)c->np * c->ncell < 600000; }
 static bool gather_mode(const janc_ctx *c) {
+  if (c->P.bc_lo[0] == JANC_BC_EXCHANGE || c->P.bc_hi[0] == JANC_BC_EXCHANGE) return false;   // halos arrive in the ghost cells
   return c->opt.halo_in_kernel && c->g.ndim == 2 && ((c->P.n[0] <= 16 && c->P.n[1] <= 16) || small_grid(c));
 }
 
@@ -1057,6 +1060,82 @@ extern "C" int janc_step(janc_ctx *c, int nsteps, double cfl, double dt_fixed, i
     *t_advanced = t1 - t0;
     return rc;
   }
+  return JANC_OK;
+}
+
+// ------------------------------------------------------------------ x-slab decomposition
+// One step cut into the parts between which the slabs of a decomposed grid talk to each other; the caller (binding /
+// slab.py: torch.distributed plumbing) supplies the max all-reduce of the reduction slots and the halo exchange.
+static double *rk_register(janc_ctx *c, int which) { return which == 0 ? c->A : which == 1 ? c->B : c->C; }
+
+extern "C" int janc_step_part(janc_ctx *c, int part, int stage, double cfl, double dt_fixed, int flags) {
+  int rc = check_ready(c);
+  if (rc) return rc;
+  if (c->g.n_patches > 0 || stage < 0 || stage > 2 || (flags & ~1)) { c->err = "janc_step_part: uniform grid, stage 0..2, flags 0 or 1"; return JANC_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  MechLock mech_lock(c);
+  rc = upload_mech(c);
+  if (rc) return rc;
+  const int par = c->parity;
+  set_active(c, 0, c->np, 1.0);
+  double *Uk = rk_register(c, stage);
+  static const double coef[3] = {1.0, 0.25, 2.0 / 3.0};
+  switch (part) {
+    case JANC_PART_PRIM:    // update_aux of the stage state + its max(|u_d| + c) into the reduction slots
+      do_prim(c, Uk, 1, SLOTX(par, 0, stage, 0, 0), nullptr, nullptr);
+      break;
+    case JANC_PART_DT:      // cfl() from the (all-reduced) slots of stage 0
+      if (!(cfl > 0.0) && !(dt_fixed > 0.0)) { c->err = "need cfl > 0 or dt_fixed > 0"; return JANC_EINVAL; }
+      k_dt<<<1, 32, 0, c->stream>>>(c->P, par, cfl, dt_fixed, 1.0);
+      note_launch(c, cudaGetLastError());
+      break;
+    case JANC_PART_GHOST:   // physical boundaries of the stage state (exchange faces are left to janc_halo)
+      do_ghost(c, Uk, nullptr);
+      break;
+    case JANC_PART_FLUX:    // fluxes + divergence + RK stage: A -> B, B -> C, C -> A
+      do_flux(c, Uk, c->A, stage == 0 ? c->B : stage == 1 ? c->C : c->A, SLOTX(par, 0, stage, 0, 0), coef[stage], nullptr);
+      break;
+    case JANC_PART_SOURCE:  // advance_source_term (or only update_aux with flags bit 0), end of the step
+      if (!(flags & 1) && c->ns > 1 && c->nr > 0) do_chem(c, c->A, nullptr);
+      else do_prim(c, c->A, 0, 0, nullptr, nullptr);
+      c->parity = 1 - par;
+      break;
+    default: c->err = "janc_step_part: unknown part"; return JANC_EINVAL;
+  }
+  if ((rc = take_launch_error(c)) != JANC_OK) return rc;
+  CK(cudaGetLastError());
+  return JANC_OK;
+}
+
+extern "C" size_t janc_halo_doubles(const janc_ctx *c) {
+  if (!c || !c->have_mech) return 0;
+  return (size_t)(c->nvar + 2 + c->g.ndim) * JANC_NG * c->P.n[1] * c->P.n[2];
+}
+
+extern "C" int janc_halo(janc_ctx *c, int stage, int side, double *buf_dev, int unpack) {
+  int rc = check_ready(c);
+  if (rc) return rc;
+  if (c->g.n_patches > 0 || stage < 0 || stage > 2 || side < 0 || side > 1 || !buf_dev) return JANC_EINVAL;
+  CK(cudaSetDevice(c->device));
+  const size_t n = janc_halo_doubles(c);
+  set_active(c, 0, c->np, 1.0);
+  k_halo<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->P, rk_register(c, stage), buf_dev, side, unpack);
+  note_launch(c, cudaGetLastError());
+  return take_launch_error(c);
+}
+
+extern "C" int janc_reduction_slots(const janc_ctx *c, size_t *byte_offset, size_t *count) {
+  if (!c || !c->have_ws || !byte_offset || !count) return JANC_EINVAL;
+  *byte_offset = (size_t)((const char *)c->P.slots - (const char *)c->A);     // A is the first piece of the workspace
+  *count = JANC_NSLOT;
+  return JANC_OK;
+}
+
+extern "C" int janc_last_dt(janc_ctx *c, double *dt) {
+  if (!c || !dt) return JANC_EINVAL;
+  if (!c->have_ws) return JANC_ESTATE;
+  CK(cudaMemcpyAsync(dt, c->P.scal, 8, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
   return JANC_OK;
 }
 
