@@ -61,11 +61,14 @@ typedef struct {
   const int *reversible;
   const int *third_body;
   const double *eff;
+  const double *nasa_hi;   /* [ns][7] coefficients of the upper temperature range, NULL: single range (reading A7) */
+  const double *T_mid;     /* [ns] switch temperature: T >= T_mid[k] uses nasa_hi[k] (Cantera-format data) */
 } jref_mech;
 
 typedef struct {
   int ns, nr;
   double *W, *nasa, *A, *b, *Ta, *eff;
+  double *nasa_hi, *T_mid;     /* NULL: single range */
   int *nu_f, *nu_b, *reversible, *third_body;
 } mech_t;
 
@@ -85,17 +88,23 @@ typedef struct jref_ctx {
 } jref_ctx;
 
 /* ------------------------------------------------------------------ thermo (eq 4.3-4.5) */
+/* NASA-7 coefficients of species k at temperature T: the two-range form of the Cantera / Chemkin data the paper reads
+ * (PAPER.md:258, :279): the upper set from T_mid upwards */
+static const double *nasa_at(const mech_t *m, int k, double T) {
+  return (m->nasa_hi && T >= m->T_mid[k]) ? m->nasa_hi + 7 * k : m->nasa + 7 * k;
+}
+
 static double cp_R(const mech_t *m, int k, double T) {
-  const double *a = m->nasa + 7 * k;
+  const double *a = nasa_at(m, k, T);
   return a[0] + a[1] * T + a[2] * T * T + a[3] * T * T * T + a[4] * T * T * T * T;
 }
 static double h_R(const mech_t *m, int k, double T) { /* h_k/(Ru/W_k), eq 4.4 */
-  const double *a = m->nasa + 7 * k;
+  const double *a = nasa_at(m, k, T);
   return a[0] * T + a[1] / 2 * T * T + a[2] / 3 * T * T * T + a[3] / 4 * T * T * T * T +
          a[4] / 5 * T * T * T * T * T + a[5];
 }
 static double s_R(const mech_t *m, int k, double T) { /* s_k/(Ru/W_k), eq 4.5 */
-  const double *a = m->nasa + 7 * k;
+  const double *a = nasa_at(m, k, T);
   return a[0] * log(T) + a[1] * T + a[2] / 2 * T * T + a[3] / 3 * T * T * T +
          a[4] / 4 * T * T * T * T + a[6];
 }
@@ -257,7 +266,7 @@ static int chem_cell(const mech_t *m, double T, double rho, const double *rhoY, 
 
 /* ------------------------------------------------------------------ context */
 static void mech_free(mech_t *m) {
-  free(m->W); free(m->nasa); free(m->A); free(m->b); free(m->Ta); free(m->eff);
+  free(m->W); free(m->nasa); free(m->A); free(m->b); free(m->Ta); free(m->eff); free(m->nasa_hi); free(m->T_mid);
   free(m->nu_f); free(m->nu_b); free(m->reversible); free(m->third_body);
   memset(m, 0, sizeof *m);
 }
@@ -280,6 +289,8 @@ static int mech_copy(mech_t *m, const jref_mech *in) {
   m->Ta = dup_mem(in->Ta, sizeof(double) * nr);
   m->reversible = dup_mem(in->reversible, sizeof(int) * nr);
   m->third_body = dup_mem(in->third_body, sizeof(int) * nr);
+  m->nasa_hi = (in->nasa_hi && in->T_mid) ? dup_mem(in->nasa_hi, sizeof(double) * 7 * ns) : NULL;
+  m->T_mid = (in->nasa_hi && in->T_mid) ? dup_mem(in->T_mid, sizeof(double) * ns) : NULL;
   m->eff = malloc(sizeof(double) * (nr * ns + 1));
   for (int i = 0; i < nr * ns; i++) m->eff[i] = in->eff ? in->eff[i] : 1.0;
   return JREF_OK;

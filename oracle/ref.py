@@ -36,7 +36,8 @@ class _Mech(C.Structure):
                 ("W", C.c_void_p), ("nasa", C.c_void_p),
                 ("nu_f", C.c_void_p), ("nu_b", C.c_void_p),
                 ("A", C.c_void_p), ("b", C.c_void_p), ("Ta", C.c_void_p),
-                ("reversible", C.c_void_p), ("third_body", C.c_void_p), ("eff", C.c_void_p)]
+                ("reversible", C.c_void_p), ("third_body", C.c_void_p), ("eff", C.c_void_p),
+                ("nasa_hi", C.c_void_p), ("T_mid", C.c_void_p)]
 
 
 def lib():
@@ -73,9 +74,13 @@ class _MechHolder:
                          A=_f64(mech.A), b=_f64(mech.b), Ta=_f64(mech.Ta),
                          reversible=_i32(mech.reversible), third_body=_i32(mech.third_body),
                          eff=_f64(mech.eff))
+        two = getattr(mech, "nasa_hi", None) is not None
+        if two:
+            self.arrs["nasa_hi"] = _f64(mech.nasa_hi); self.arrs["T_mid"] = _f64(mech.T_mid)
         self.c = _Mech(mech.ns, mech.nr, *[_ptr(self.arrs[k]) for k in
                                            ("W", "nasa", "nu_f", "nu_b", "A", "b", "Ta",
-                                            "reversible", "third_body", "eff")])
+                                            "reversible", "third_body", "eff")],
+                       _ptr(self.arrs["nasa_hi"]) if two else None, _ptr(self.arrs["T_mid"]) if two else None)
 
 
 class RefSolver:

@@ -45,6 +45,8 @@ class Mechanism:
     eff: np.ndarray          # [nr,ns] third-body efficiencies a_ij
     elements: np.ndarray = None   # [ns,ne] atoms of element e in species k (tests only)
     names: list = field(default_factory=list)
+    nasa_hi: np.ndarray = None    # [ns,7] upper-range coefficients (two-range NASA-7, as in Cantera / Chemkin data); None: single range
+    T_mid: np.ndarray = None      # [ns] switch temperature: T >= T_mid[k] uses nasa_hi[k]
 
 
 @dataclass
@@ -91,12 +93,16 @@ class Case:
 # --------------------------------------------------------------------------
 # ideal-gas mixture bookkeeping for initial conditions (eq. 4.2-4.4)
 # --------------------------------------------------------------------------
-def _h_over_R(nasa, T):
-    """h_k/(Ru/W_k) of eq. 4.4 for every species; T array broadcast on the right."""
-    a = nasa
+def _h_over_R(nasa, T, nasa_hi=None, T_mid=None):
+    """h_k/(Ru/W_k) of eq. 4.4 for every species; T array broadcast on the right.  Two-range data: the upper set from
+    T_mid[k] upwards."""
     T = np.asarray(T, dtype=np.float64)[..., None]
-    return (a[:, 0] * T + a[:, 1] / 2 * T**2 + a[:, 2] / 3 * T**3
-            + a[:, 3] / 4 * T**4 + a[:, 4] / 5 * T**5 + a[:, 5])
+    def poly(a):
+        return (a[:, 0] * T + a[:, 1] / 2 * T**2 + a[:, 2] / 3 * T**3
+                + a[:, 3] / 4 * T**4 + a[:, 4] / 5 * T**5 + a[:, 5])
+    if nasa_hi is None:
+        return poly(nasa)
+    return np.where(T >= np.asarray(T_mid), poly(np.asarray(nasa_hi)), poly(nasa))
 
 
 def prim_to_cons(mech: Mechanism, ndim, p, T, Y, vel):
@@ -107,7 +113,7 @@ def prim_to_cons(mech: Mechanism, ndim, p, T, Y, vel):
     Rk = RU / mech.W
     R = (Y * Rk).sum(-1)
     rho = p / (R * T)
-    h = (Y * Rk * _h_over_R(mech.nasa, T)).sum(-1)
+    h = (Y * Rk * _h_over_R(mech.nasa, T, getattr(mech, "nasa_hi", None), getattr(mech, "T_mid", None))).sum(-1)
     ke = np.zeros_like(rho)
     for d in range(ndim):
         ke = ke + 0.5 * vel[d] ** 2
@@ -559,3 +565,23 @@ def refine_uniform(case: Case, tile, refine):
     g2 = Grid(nd, tuple(t), g.dx, g.bc_lo, g.bc_hi, n_patches=npatch, n_levels=2, ratio=2)
     return Case(case.name + "_2lev", g2, case.mech, U, T, case.cfl, case.nsteps,
                 blocks=Blocks(level, nbr, parent, origin))
+
+
+def two_range(mech: Mechanism, T_mid, dcp, seed=0):
+    """A two-range version of a single-range mechanism: above T_mid[k] species k has c_p/R = a0 + dcp[k] + a1' T with
+    a seeded small slope, and a5', a6' chosen so that h_k and s_k are continuous at T_mid[k] (what fitted NASA data
+    satisfy to their fitting accuracy).  Stands in for Cantera-format thermo data."""
+    rng = np.random.default_rng(seed)
+    T_mid = np.broadcast_to(np.asarray(T_mid, dtype=np.float64), (mech.ns,)).copy()
+    lo = mech.nasa
+    hi = lo.copy()
+    hi[:, 0] = lo[:, 0] + np.broadcast_to(dcp, (mech.ns,))
+    hi[:, 1] = lo[:, 1] + rng.uniform(1e-5, 2e-4, size=mech.ns)
+    Tm = T_mid
+    def h(a): return a[:, 0] * Tm + a[:, 1] / 2 * Tm**2 + a[:, 2] / 3 * Tm**3 + a[:, 3] / 4 * Tm**4 + a[:, 4] / 5 * Tm**5
+    def s(a): return a[:, 0] * np.log(Tm) + a[:, 1] * Tm + a[:, 2] / 2 * Tm**2 + a[:, 3] / 3 * Tm**3 + a[:, 4] / 4 * Tm**4
+    hi[:, 5] = lo[:, 5] + h(lo) - h(hi)
+    hi[:, 6] = lo[:, 6] + s(lo) - s(hi)
+    out = Mechanism(**{**mech.__dict__})
+    out.nasa_hi, out.T_mid = hi, T_mid
+    return out

@@ -915,3 +915,97 @@ def test_crossover_fine_level_sees_the_coarse_state_at_the_start_of_the_step(ref
     # the coarse cells next to the band did feel it (so a coarse-first order would have passed it on)
     near = [p for p in np.nonzero(lev == 0)[0] if org[p, 0] == 32]
     assert max(np.abs(Ua[p, 0, 0, :, 0:2] - Ub[p, 0, 0, :, 0:2]).max() for p in near) > 0
+
+
+# ----------------------------------------------------------------------------- two-range NASA-7
+def test_two_range_identical_sets_equal_single_range(ref, mech9):
+    """PAPER.md:247-258 with Cantera-format data: two coefficient sets per species, switched at T_mid.  Both sets equal
+    => bitwise the single-range answer (full steps with chemistry)."""
+    m2 = I.Mechanism(**{**mech9.__dict__}); m2.nasa_hi = mech9.nasa.copy(); m2.T_mid = np.full(9, 1000.0)
+    c1 = I.config1(nx=24, ny=12, mech=mech9); c2 = I.config1(nx=24, ny=12, mech=m2)
+    U1, T1, t1, s1 = run(ref, c1, nsteps=3); U2, T2, t2, s2 = run(ref, c2, nsteps=3)
+    assert s1 == 0 and s2 == 0 and t1 == t2 and np.array_equal(U1, U2) and np.array_equal(T1, T2)
+
+
+def test_two_range_temperature_closed_form_per_species_switch(ref):
+    """Piecewise-constant c_p with different switch temperatures per species and h continuous at each T_mid:
+    e(T) = sum_k Y_k R_k (h_k/R_k - T) is piecewise linear, so T(e) is known in closed form on every piece; the pressure,
+    gamma and sound speed must use the coefficient set of the recovered T."""
+    W = np.array([0.010, 0.030, 0.020]); Rk = RU / W
+    lo = np.zeros((3, 7)); lo[:, 0] = [3.5, 4.0, 2.5]; lo[:, 5] = [-500.0, 2000.0, 100.0]
+    hi = lo.copy(); hi[:, 0] = [4.5, 4.75, 2.5]
+    Tm = np.array([800.0, 1500.0, 1000.0])
+    hi[:, 5] = lo[:, 5] + (lo[:, 0] - hi[:, 0]) * Tm                      # h continuous at T_mid
+    z = np.zeros((0, 3), dtype=np.int32)
+    m = I.Mechanism(3, 0, W, lo, z, z.copy(), np.zeros(0), np.zeros(0), np.zeros(0), np.zeros(0, dtype=np.int32),
+                    np.zeros(0, dtype=np.int32), np.zeros((0, 3)), nasa_hi=hi, T_mid=Tm)
+    Y = np.array([0.2, 0.5, 0.3]); rho = 1.7; u = 140.0
+    def e_of(T):
+        a0 = np.where(T >= Tm, hi[:, 0], lo[:, 0]); a5 = np.where(T >= Tm, hi[:, 5], lo[:, 5])
+        return (Y * Rk * ((a0 - 1.0) * T + a5)).sum(), a0
+    for T in (500.0, 799.0, 801.0, 1200.0, 1499.9, 1500.1, 2600.0):
+        e, a0 = e_of(T)
+        Uc = np.array([rho, rho * u, rho * e + 0.5 * rho * u * u, rho * Y[0], rho * Y[1]])
+        for guess in (300.0, T, 3000.0):                                  # Newton crosses the kinks from either side
+            rc, out = ref.cons2prim(m, 1, Uc, guess)
+            assert rc == 0 and abs(out[0] - T) <= 1e-10 * T, (T, guess, out[0])
+        cv = (Y * Rk * (a0 - 1.0)).sum(); R = (Y * Rk).sum()
+        assert abs(out[2] - (cv + R) / cv) <= 1e-12 and abs(out[1] - rho * R * T) <= 1e-9 * rho * R * T
+
+
+def test_two_range_equilibrium_constant_uses_the_upper_set_and_is_continuous(ref, mech9):
+    """eq 4.9 with two-range data: above T_mid a reversible reaction is in detailed balance at the composition built
+    from the UPPER coefficients' Gibbs energies (re-derived here), and K_eq is continuous across T_mid when h and s are
+    (inputs.two_range builds such data)."""
+    m2 = I.two_range(mech9, 1000.0, 0.6, seed=3)
+    T = 1850.0
+    a = m2.nasa_hi
+    h = a[:, 0] + a[:, 1] / 2 * T + a[:, 5] / T
+    s = a[:, 0] * math.log(T) + a[:, 1] * T + a[:, 6]
+    g = h - s
+    for i in (0, 5, 11, 20):
+        dn = (m2.nu_b[i] - m2.nu_f[i]).astype(float)
+        lnK = -(dn * g).sum() + dn.sum() * math.log(101325.0 / (RU * T))
+        lx = np.log(np.full(9, 2.0) + np.arange(9) * 0.3)
+        lx = lx + dn * (lnK - dn @ lx) / (dn @ dn)
+        m1 = I.Mechanism(9, 1, m2.W, m2.nasa, m2.nu_f[i:i + 1], m2.nu_b[i:i + 1], m2.A[i:i + 1], m2.b[i:i + 1], m2.Ta[i:i + 1],
+                         m2.reversible[i:i + 1], m2.third_body[i:i + 1], m2.eff[i:i + 1], nasa_hi=m2.nasa_hi, T_mid=m2.T_mid)
+        X = np.exp(lx)
+        q = ref.rates(m1, T, X)[0]
+        kf = m2.A[i] * T ** m2.b[i] * math.exp(-m2.Ta[i] / T)
+        M = (m2.eff[i] * X).sum() if m2.third_body[i] else 1.0
+        fwd = M * kf * np.prod(X ** m2.nu_f[i])
+        assert abs(q) <= 1e-10 * fwd, (i, q, fwd)
+        # with the LOWER set the same composition is far from balance: the switch matters
+        m_lo = I.Mechanism(9, 1, m2.W, m2.nasa, m2.nu_f[i:i + 1], m2.nu_b[i:i + 1], m2.A[i:i + 1], m2.b[i:i + 1], m2.Ta[i:i + 1],
+                           m2.reversible[i:i + 1], m2.third_body[i:i + 1], m2.eff[i:i + 1])
+        assert abs(ref.rates(m_lo, T, X)[0]) > 1e-4 * fwd
+        # continuity of the net rate across T_mid
+        X1 = np.full(9, 1.3) + 0.1 * np.arange(9)
+        qa, qb = ref.rates(m1, 1000.0 * (1 - 1e-12), X1)[0], ref.rates(m1, 1000.0, X1)[0]
+        assert abs(qa - qb) <= 1e-8 * max(abs(qa), abs(qb), 1e-300), (i, qa, qb)
+
+
+def test_two_range_roundtrip_and_energy_conservation_in_a_step(ref, mech9):
+    """prim -> cons (inputs, forward formula) -> prim (oracle, Newton) on two-range data across the switch, and a 0-D
+    point-implicit run heating through T_mid keeps rho, E fixed and elements conserved."""
+    m2 = I.two_range(mech9, np.linspace(900.0, 1300.0, 9), 0.4, seed=4)
+    rng = np.random.default_rng(8)
+    for T in (600.0, 950.0, 1100.0, 1299.0, 1301.0, 2400.0):
+        Y = rng.dirichlet(np.ones(9)); p = 3.0e5
+        U = I.prim_to_cons(m2, 2, np.array([p]), np.array([T]), Y[None], [np.array([50.0]), np.array([-20.0])])[:, 0]
+        rc, out = ref.cons2prim(m2, 2, U, 1000.0)
+        assert rc == 0 and abs(out[0] - T) <= 1e-10 * T and abs(out[1] - p) <= 1e-9 * p
+    m3 = I.two_range(mech9, np.linspace(2002.0, 2012.0, 9), 0.4, seed=5)     # the 0-D case of the pins above: 2000 K -> ~2018 K
+    U = I.prim_to_cons(m3, 1, np.array([2.0e6]), np.array([2000.0]), I.hot_Y(9)[None], [np.zeros(1)])
+    g = I.Grid(1, (1, 1, 1), (1e-3, 1, 1), (2, 0, 0), (2, 0, 0))
+    s = ref.RefSolver(g, m3); s.set_state(U.reshape(1, -1, 1, 1, 1), np.full((1, 1, 1, 1), 2000.0))
+    s.step(100, cfl=0.0, dt=2e-9)
+    U1, T1 = s.get_state()
+    assert s.status == 0 and T1[0, 0, 0, 0] > 2012.5, T1                   # heated through every species' T_mid
+    assert np.array_equal(U1[0, :3], U.reshape(1, -1, 1, 1, 1)[0, :3])
+    el = np.asarray(m3.elements, dtype=float)
+    def moles(Us):
+        ry = np.concatenate([Us[0, 3:, 0, 0, 0], [Us[0, 0, 0, 0, 0] - Us[0, 3:, 0, 0, 0].sum()]])
+        return (ry / m3.W) @ el
+    assert np.abs(moles(U1) - moles(U.reshape(1, -1, 1, 1, 1))).max() <= 1e-12 * np.abs(moles(U1)).max()
