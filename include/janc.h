@@ -64,6 +64,10 @@ typedef struct {
   const int32_t *reversible; /* [nr] 0 => k_b = 0 (reading A10)                                   */
   const int32_t *third_body; /* [nr] 1 => rate multiplied by sum_j a_ij X_j (eq 4.7, reading A9)  */
   const double *eff;         /* [nr][ns] a_ij; NULL => all 1                                      */
+  const double *nasa_hi;     /* [ns][7] two-range NASA-7 data (Cantera / Chemkin thermo):   */
+  const double *T_mid;       /* [ns]    species k uses nasa_hi[k] for T >= T_mid[k], nasa[k] below; both NULL => */
+                             /*         single range.  (The role-warp chemistry kernel is single-range only:    */
+                             /*         two-range mechanisms of more than 13 species run the "jit-smem" kernel.) */
 } janc_mech;
 
 /* Create a context for one grid on CUDA device `device`; kernels go to `cuda_stream`.  JANC_EINVAL for a malformed

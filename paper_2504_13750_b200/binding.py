@@ -46,7 +46,8 @@ class _Mech(C.Structure):
     _fields_ = [("ns", C.c_int), ("nr", C.c_int),
                 ("W", C.c_void_p), ("nasa", C.c_void_p), ("nu_f", C.c_void_p), ("nu_b", C.c_void_p),
                 ("A", C.c_void_p), ("b", C.c_void_p), ("Ta", C.c_void_p),
-                ("reversible", C.c_void_p), ("third_body", C.c_void_p), ("eff", C.c_void_p)]
+                ("reversible", C.c_void_p), ("third_body", C.c_void_p), ("eff", C.c_void_p),
+                ("nasa_hi", C.c_void_p), ("T_mid", C.c_void_p)]
 
 
 def lib():
@@ -108,8 +109,12 @@ def _mech_struct(mech):
     keep = dict(W=_f64(mech.W), nasa=_f64(mech.nasa), nu_f=_i32(mech.nu_f), nu_b=_i32(mech.nu_b),
                 A=_f64(mech.A), b=_f64(mech.b), Ta=_f64(mech.Ta), reversible=_i32(mech.reversible),
                 third_body=_i32(mech.third_body), eff=_f64(mech.eff))
+    two = getattr(mech, "nasa_hi", None) is not None
+    if two:
+        keep["nasa_hi"] = _f64(mech.nasa_hi); keep["T_mid"] = _f64(mech.T_mid)
     m = _Mech(mech.ns, mech.nr, *[_ptr(keep[k]) for k in
-                                  ("W", "nasa", "nu_f", "nu_b", "A", "b", "Ta", "reversible", "third_body", "eff")])
+                                  ("W", "nasa", "nu_f", "nu_b", "A", "b", "Ta", "reversible", "third_body", "eff")],
+              _ptr(keep["nasa_hi"]) if two else None, _ptr(keep["T_mid"]) if two else None)
     return m, keep
 
 

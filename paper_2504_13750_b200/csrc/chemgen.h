@@ -45,6 +45,26 @@ inline std::string horner(const double *c, int n) {
   return s;
 }
 
+// The same polynomial for two-range NASA-7 data: every coefficient is a select on hi<k> (T >= T_mid of species k,
+// declared by emit_range_flags next to each temperature the polynomials are evaluated at)
+inline std::string horner2(const double *lo, const double *hi, int n, int k) {
+  int deg = n - 1;
+  while (deg > 0 && lo[deg] == 0.0 && hi[deg] == 0.0) deg--;
+  auto co = [&](int q) { return lo[q] == hi[q] ? num(lo[q]) : "(hi" + std::to_string(k) + " ? " + num(hi[q]) + " : " + num(lo[q]) + ")"; };
+  std::string s = co(deg);
+  for (int q = deg - 1; q >= 0; q--) s = "fma(T, " + s + ", " + co(q) + ")";
+  return s;
+}
+// polynomial in T of species k built from its 7 NASA coefficients by `build` (fills out[n])
+template <class F>
+inline std::string nasa_poly(const MechC &M, int k, int n, F build) {
+  double lo[8], hi[8];
+  build(M.nasa[k], lo);
+  if (!M.two_range) return horner(lo, n);
+  build(M.nasa_hi[k], hi);
+  return horner2(lo, hi, n, k);
+}
+
 struct Emitter {
   std::string s;
   void line(const std::string &l) { s += "  " + l + "\n"; }
@@ -126,19 +146,26 @@ inline void emit_math(std::string &src, bool estrin = false) {
 }
 
 // Newton on e(T) = sum_k Y_k R_k (h_k/R_k - T) (eq 4.3-4.4; reading A6): expects yr<k>, e, T; sets ok
+// two-range data: which coefficient set every species uses at the current T (reading A7 -> SURVEY NEXT-3)
+inline void emit_range_flags(Emitter &E, const MechC &M, const std::string &ind, const std::vector<char> *need = nullptr) {
+  if (!M.two_range) return;
+  for (int k = 0; k < M.ns; k++)
+    if (!need || (*need)[k]) E.line(ind + "const bool hi" + I(k) + " = T >= " + num(M.Tmid[k]) + ";");
+}
+
 inline void emit_newton(Emitter &E, const MechC &M) {
   const int ns = M.ns;
   E.line("bool ok = false;");
   E.line("#pragma unroll 1");
   E.line("for (int it = 0; it < 50; it++) {");
   E.line("  double f = -e, cv = 0.0;");
+  emit_range_flags(E, M, "  ");
   for (int k = 0; k < ns; k++) {
-    const double *c = M.nasa[k];
     // h_k/R_k - T = a5 + (a0-1) T + a1/2 T^2 + ... ;  cp_k/R_k - 1 = (a0-1) + a1 T + ...
-    double hc[6] = {c[5], c[0] - 1.0, 0.5 * c[1], c[2] / 3.0, 0.25 * c[3], 0.2 * c[4]};
-    double cc[5] = {c[0] - 1.0, c[1], c[2], c[3], c[4]};
-    E.line("  f = fma(yr" + I(k) + ", " + horner(hc, 6) + ", f);");
-    E.line("  cv = fma(yr" + I(k) + ", " + horner(cc, 5) + ", cv);");
+    const std::string h = nasa_poly(M, k, 6, [](const double *c, double *o) { o[0] = c[5]; o[1] = c[0] - 1.0; o[2] = 0.5 * c[1]; o[3] = c[2] / 3.0; o[4] = 0.25 * c[3]; o[5] = 0.2 * c[4]; });
+    const std::string cv = nasa_poly(M, k, 5, [](const double *c, double *o) { o[0] = c[0] - 1.0; o[1] = c[1]; o[2] = c[2]; o[3] = c[3]; o[4] = c[4]; });
+    E.line("  f = fma(yr" + I(k) + ", " + h + ", f);");
+    E.line("  cv = fma(yr" + I(k) + ", " + cv + ", cv);");
   }
   E.line("  const double dT = -f / cv;");
   E.line("  T += dT;");
@@ -249,12 +276,13 @@ inline std::string generate(const MechC &M, int ndim, bool big = false) {
       for (int k = 0; k < ns; k++) if (M.dnu[i][k] != 0.0) need_g[k] = 1;
     }
   E.line("const double lnT = log(T), iT = 1.0 / T;");
+  emit_range_flags(E, M, "", &need_g);
   for (int k = 0; k < ns; k++) {
     if (!need_g[k]) continue;
-    const double *c = M.nasa[k];
-    double sc[5] = {c[6], c[1], 0.5 * c[2], c[3] / 3.0, 0.25 * c[4]};        // + a0 ln T
-    double hc[6] = {c[5], c[0], 0.5 * c[1], c[2] / 3.0, 0.25 * c[3], 0.2 * c[4]};
-    E.line("const double g" + I(k) + " = fma(" + num(c[0]) + ", lnT, " + horner(sc, 5) + ") - (" + horner(hc, 6) + ") * iT;");
+    const std::string sp = nasa_poly(M, k, 5, [](const double *c, double *o) { o[0] = c[6]; o[1] = c[1]; o[2] = 0.5 * c[2]; o[3] = c[3] / 3.0; o[4] = 0.25 * c[4]; });   // + a0 ln T
+    const std::string hp = nasa_poly(M, k, 6, [](const double *c, double *o) { o[0] = c[5]; o[1] = c[0]; o[2] = 0.5 * c[1]; o[3] = c[2] / 3.0; o[4] = 0.25 * c[3]; o[5] = 0.2 * c[4]; });
+    const std::string a0 = nasa_poly(M, k, 1, [](const double *c, double *o) { o[0] = c[0]; });
+    E.line("const double g" + I(k) + " = fma(" + a0 + ", lnT, " + sp + ") - (" + hp + ") * iT;");
   }
   if (any_rev) E.line("const double lnC0 = " + num(std::log(JANC_PATM / JANC_RU)) + " - lnT;   // ln(p0 / (Ru T))");
   E.line("const double dt = a.scal[0] * a.dts;");
@@ -423,12 +451,13 @@ inline std::string generate_source(const MechC &M, int ndim, bool with_math) {
       for (int k = 0; k < ns; k++) if (M.dnu[i][k] != 0.0) need_g[k] = 1;
     }
   E.line("const double lnT = log(T), iT = 1.0 / T;");
+  emit_range_flags(E, M, "", &need_g);
   for (int k = 0; k < ns; k++) {
     if (!need_g[k]) continue;
-    const double *c = M.nasa[k];
-    double sc[5] = {c[6], c[1], 0.5 * c[2], c[3] / 3.0, 0.25 * c[4]};
-    double hc[6] = {c[5], c[0], 0.5 * c[1], c[2] / 3.0, 0.25 * c[3], 0.2 * c[4]};
-    E.line("const double g" + I(k) + " = fma(" + num(c[0]) + ", lnT, " + horner(sc, 5) + ") - (" + horner(hc, 6) + ") * iT;");
+    const std::string sp = nasa_poly(M, k, 5, [](const double *c, double *o) { o[0] = c[6]; o[1] = c[1]; o[2] = 0.5 * c[2]; o[3] = c[3] / 3.0; o[4] = 0.25 * c[4]; });   // + a0 ln T
+    const std::string hp = nasa_poly(M, k, 6, [](const double *c, double *o) { o[0] = c[5]; o[1] = c[0]; o[2] = 0.5 * c[1]; o[3] = c[2] / 3.0; o[4] = 0.25 * c[3]; o[5] = 0.2 * c[4]; });
+    const std::string a0 = nasa_poly(M, k, 1, [](const double *c, double *o) { o[0] = c[0]; });
+    E.line("const double g" + I(k) + " = fma(" + a0 + ", lnT, " + sp + ") - (" + hp + ") * iT;");
   }
   if (any_rev) E.line("const double lnC0 = " + num(std::log(JANC_PATM / JANC_RU)) + " - lnT;   // ln(p0 / (Ru T))");
   Acc accW(ns);
@@ -502,10 +531,10 @@ inline std::string generate_prim(const MechC &M, int ndim) {
   E.line("double T = a.T[pid];");
   emit_newton(E, M);
   E.line("double R = 0.0, cp = 0.0;");
+  emit_range_flags(E, M, "");
   for (int k = 0; k < ns; k++) {
-    const double *c = M.nasa[k];
-    double cc[5] = {c[0], c[1], c[2], c[3], c[4]};
-    E.line("R += yr" + I(k) + "; cp = fma(yr" + I(k) + ", " + horner(cc, 5) + ", cp);");
+    const std::string cc = nasa_poly(M, k, 5, [](const double *c, double *o) { o[0] = c[0]; o[1] = c[1]; o[2] = c[2]; o[3] = c[3]; o[4] = c[4]; });
+    E.line("R += yr" + I(k) + "; cp = fma(yr" + I(k) + ", " + cc + ", cp);");
   }
   E.line("const double p = rho * R * T;");
   E.line("const double c = sqrt(cp / (cp - R) * R * T);");

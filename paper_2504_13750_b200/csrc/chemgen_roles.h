@@ -76,6 +76,7 @@ inline size_t roles_table_ints(const MechC &M) {
 }
 
 inline bool roles_applicable(const MechC &M) {
+  if (M.two_range) return false;     // the reverse-rate polynomial collected per reaction on the host assumes one coefficient set
   return M.ns >= 3 && M.ns <= JANC_ROLES_MAXCOLS && M.nr >= 1;
 }
 

@@ -29,6 +29,9 @@ struct MechC {
   int ns, nr;
   double W[JANC_MAX_NS], invW[JANC_MAX_NS], Rk[JANC_MAX_NS];
   double nasa[JANC_MAX_NS][7];
+  double nasa_hi[JANC_MAX_NS][7];            // two-range data: upper set, used from Tmid[k] upwards (two_range != 0)
+  double Tmid[JANC_MAX_NS];
+  int two_range;
   double lnA[JANC_MAX_NR], b[JANC_MAX_NR], Ta[JANC_MAX_NR];
   double Asign[JANC_MAX_NR];                 // sign(A) (A may not be <= 0; kept for safety: +1)
   signed char rev[JANC_MAX_NR], tb[JANC_MAX_NR], dn[JANC_MAX_NR];

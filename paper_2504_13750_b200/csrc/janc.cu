@@ -220,6 +220,11 @@ static int fill_mech(const janc_mech *m, MechC &M, std::string &err) {
     if (!(m->W[k] > 0.0)) return JANC_EINVAL;
     M.W[k] = m->W[k]; M.invW[k] = 1.0 / m->W[k]; M.Rk[k] = JANC_RU / m->W[k];
     for (int q = 0; q < 7; q++) M.nasa[k][q] = m->nasa[k * 7 + q];
+    if (m->nasa_hi && m->T_mid) {
+      for (int q = 0; q < 7; q++) M.nasa_hi[k][q] = m->nasa_hi[k * 7 + q];
+      M.Tmid[k] = m->T_mid[k];
+      M.two_range = 1;
+    }
   }
   for (int i = 0; i < m->nr; i++) {
     if (!(m->A[i] > 0.0)) { err = "A must be > 0"; return JANC_EINVAL; }

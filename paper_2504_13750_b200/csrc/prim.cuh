@@ -8,16 +8,20 @@ __constant__ MechC c_mech;
 static_assert(sizeof(MechC) <= 65536, "MechC must fit constant memory");
 
 // cp_k/R_k and h_k/R_k (eq 4.3, 4.4), Horner form
+// coefficient set of species k at T (two-range NASA-7: the upper set from Tmid[k] upwards)
+__device__ __forceinline__ const double *nasa_at(int k, double T) {
+  return (c_mech.two_range && T >= c_mech.Tmid[k]) ? c_mech.nasa_hi[k] : c_mech.nasa[k];
+}
 __device__ __forceinline__ double cp_R(int k, double T) {
-  const double *a = c_mech.nasa[k];
+  const double *a = nasa_at(k, T);
   return a[0] + T * (a[1] + T * (a[2] + T * (a[3] + T * a[4])));
 }
 __device__ __forceinline__ double h_R(int k, double T) {
-  const double *a = c_mech.nasa[k];
+  const double *a = nasa_at(k, T);
   return a[5] + T * (a[0] + T * (0.5 * a[1] + T * (a[2] * (1.0 / 3.0) + T * (0.25 * a[3] + T * (0.2 * a[4])))));
 }
 __device__ __forceinline__ double s_R(int k, double T, double lnT) {
-  const double *a = c_mech.nasa[k];
+  const double *a = nasa_at(k, T);
   return a[0] * lnT + a[6] + T * (a[1] + T * (0.5 * a[2] + T * (a[3] * (1.0 / 3.0) + T * (0.25 * a[4]))));
 }
 
