@@ -70,6 +70,21 @@ typedef struct {
                              /*         two-range mechanisms of more than 13 species run the "jit-smem" kernel.) */
 } janc_mech;
 
+/* Chemkin-format mechanism reader (PAPER.md:279 "a chemkin-format reader", :400; two-range NASA-7 thermo, :258): host
+ * only, needs no device.  mech_text: ELEMENTS / SPECIES / [THERMO] / REACTIONS sections; thermo_text (nullable): a
+ * separate thermo file.  Supported subset = what eq 4.6-4.9 can express: Arrhenius reactions, reversible ("=", "<=>")
+ * or not ("=>"), third bodies "+ M" with efficiency lines; units CAL/MOLE (default), KCAL/MOLE, JOULES/MOLE,
+ * KJOULES/MOLE, KELVINS; element weights from a small built-in table or "X /w/".  Anything else (fall-off, PLOG, REV,
+ * ...) is refused: JANC_EINVAL with a message in err (NUL-terminated, at most errcap bytes).  The result is in SI
+ * (W kg/mol; A in mol, m^3, s; Ta = E / R_u in K), species in file order -- the LAST species is the one carried by
+ * difference.  janc_mech_file_view fills a janc_mech whose pointers stay valid until janc_mech_file_free.
+ * No mechanism data ships with the library. */
+typedef struct janc_mech_file janc_mech_file;
+int janc_mech_parse(const char *mech_text, const char *thermo_text, janc_mech_file **out, char *err, size_t errcap);
+int janc_mech_file_view(const janc_mech_file *, janc_mech *view);
+const char *janc_mech_file_species(const janc_mech_file *, int k);
+void janc_mech_file_free(janc_mech_file *);
+
 /* Create a context for one grid on CUDA device `device`; kernels go to `cuda_stream`.  JANC_EINVAL for a malformed
  * grid, including fewer than 3 cells along a direction whose sides are not both zero-gradient (the 3 ghost layers of
  * PAPER.md:295 are copies of 3 distinct interior cells under the periodic, mirror and neighbour-patch rules), or a

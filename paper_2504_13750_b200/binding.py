@@ -22,7 +22,8 @@ FLAG_CROSSOVER = 4
 PART_PRIM, PART_DT, PART_GHOST, PART_FLUX, PART_SOURCE = range(5)
 BC_EXCHANGE = 3
 
-EXPORTS = ["janc_create", "janc_set_option", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
+EXPORTS = ["janc_mech_parse", "janc_mech_file_view", "janc_mech_file_species", "janc_mech_file_free",
+           "janc_create", "janc_set_option", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
            "janc_set_blocks", "janc_set_state", "janc_step", "janc_step_part", "janc_halo_doubles", "janc_halo",
            "janc_reduction_slots", "janc_last_dt", "janc_get_state", "janc_status",
            "janc_launch_count", "janc_debug_cons2prim", "janc_profile_step",
@@ -87,6 +88,12 @@ def lib():
         L.janc_jit_log.argtypes = [C.c_void_p]
         L.janc_jit_log.restype = C.c_char_p
         L.janc_jit_probe.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p]
+        L.janc_mech_parse.argtypes = [C.c_char_p, C.c_char_p, C.c_void_p, C.c_char_p, C.c_size_t]
+        L.janc_mech_file_view.argtypes = [C.c_void_p, C.c_void_p]
+        L.janc_mech_file_species.argtypes = [C.c_void_p, C.c_int]
+        L.janc_mech_file_species.restype = C.c_char_p
+        L.janc_mech_file_free.argtypes = [C.c_void_p]
+        L.janc_mech_file_free.restype = None
         L.janc_destroy.argtypes = [C.c_void_p]
         L.janc_destroy.restype = None
         _lib = L
@@ -131,6 +138,32 @@ def jit_probe(mech, ndim, compile=True):
     if rc:
         raise JancError(rc, "janc_jit_probe (NVRTC)")
     return buf.value.decode(), (nb.value if compile else None)
+
+
+def load_chemkin(mech_text, thermo_text=None):
+    """janc_mech_parse: Chemkin-format text(s) -> inputs.Mechanism (SI units, two-range NASA-7).  Needs no GPU."""
+    from . import inputs
+    h = C.c_void_p()
+    err = C.create_string_buffer(512)
+    rc = lib().janc_mech_parse(mech_text.encode(), thermo_text.encode() if thermo_text else None, C.byref(h), err, 512)
+    if rc:
+        raise JancError(rc, "janc_mech_parse: " + err.value.decode())
+    try:
+        v = _Mech()
+        lib().janc_mech_file_view(h, C.byref(v))
+        ns, nr = v.ns, v.nr
+        def arr(ptr, n, ct, dt):
+            return np.ctypeslib.as_array(C.cast(ptr, C.POINTER(ct)), shape=(n,)).astype(dt).copy() if n else np.zeros(0, dt)
+        f = lambda ptr, n: arr(ptr, n, C.c_double, np.float64)
+        i = lambda ptr, n: arr(ptr, n, C.c_int32, np.int32)
+        names = [lib().janc_mech_file_species(h, k).decode() for k in range(ns)]
+        return inputs.Mechanism(ns=ns, nr=nr, W=f(v.W, ns), nasa=f(v.nasa, ns * 7).reshape(ns, 7),
+                                nu_f=i(v.nu_f, nr * ns).reshape(nr, ns), nu_b=i(v.nu_b, nr * ns).reshape(nr, ns),
+                                A=f(v.A, nr), b=f(v.b, nr), Ta=f(v.Ta, nr), reversible=i(v.reversible, nr),
+                                third_body=i(v.third_body, nr), eff=f(v.eff, nr * ns).reshape(nr, ns), names=names,
+                                nasa_hi=f(v.nasa_hi, ns * 7).reshape(ns, 7), T_mid=f(v.T_mid, ns))
+    finally:
+        lib().janc_mech_file_free(h)
 
 
 def measure_dfma_peak(device=0, stream=None):

@@ -20,6 +20,7 @@
 #include "chemgen_roles.h"
 #include "flux.cuh"
 #include "ghost.cuh"
+#include "mechfile.h"
 #include "prim.cuh"
 
 // janc_set_option keys (include/janc.h); defaults are what the product runs
@@ -447,6 +448,37 @@ extern "C" int janc_jit_probe(const janc_mech *m, int ndim, char *src_out, size_
   }
   return JANC_OK;
 }
+
+// ------------------------------------------------------------------ Chemkin-format reader (mechfile.h; host only)
+extern "C" int janc_mech_parse(const char *mech_text, const char *thermo_text, janc_mech_file **out, char *err, size_t errcap) {
+  if (!mech_text || !out) return JANC_EINVAL;
+  janc_mech_file *F = new (std::nothrow) janc_mech_file();
+  if (!F) return JANC_ENOMEM;
+  bool ok = false;
+  try { ok = mechfile::parse(mech_text, thermo_text, *F); } catch (...) { F->err = "internal error while parsing"; }
+  if (!ok) {
+    if (err && errcap) { strncpy(err, F->err.c_str(), errcap - 1); err[errcap - 1] = 0; }
+    delete F;
+    return JANC_EINVAL;
+  }
+  *out = F;
+  return JANC_OK;
+}
+
+extern "C" int janc_mech_file_view(const janc_mech_file *F, janc_mech *v) {
+  if (!F || !v) return JANC_EINVAL;
+  v->ns = (int)F->species.size(); v->nr = (int)F->A.size();
+  v->W = F->W.data(); v->nasa = F->nasa.data(); v->nu_f = F->nu_f.data(); v->nu_b = F->nu_b.data();
+  v->A = F->A.data(); v->b = F->b.data(); v->Ta = F->Ta.data(); v->reversible = F->reversible.data();
+  v->third_body = F->third_body.data(); v->eff = F->eff.data(); v->nasa_hi = F->nasa_hi.data(); v->T_mid = F->T_mid.data();
+  return JANC_OK;
+}
+
+extern "C" const char *janc_mech_file_species(const janc_mech_file *F, int k) {
+  return (F && k >= 0 && k < (int)F->species.size()) ? F->species[k].c_str() : "";
+}
+
+extern "C" void janc_mech_file_free(janc_mech_file *F) { delete F; }
 
 extern "C" int janc_set_mechanism(janc_ctx *c, const janc_mech *m) {
   if (!c || !m) return JANC_EINVAL;

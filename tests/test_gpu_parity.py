@@ -525,3 +525,13 @@ def test_two_range_thermo_parity(B, ref, mech9, mech20):
     for c in (ca, cb):
         g = B.Solver(c.grid, c.mech); g.set_state(c.U, c.T); g.step(3, cfl=c.cfl); out.append(g.get_state()[0]); g.close()
     assert np.array_equal(out[0], out[1])
+
+
+def test_mechanism_read_from_chemkin_text_runs_on_the_gpu(B, ref, mech9):
+    """janc_mech_parse -> janc_set_mechanism: a mechanism that came in as Chemkin-format text (written here from the
+    seeded synthetic one, two-range thermo) drives the specialised kernels; parity with the oracle on the same arrays."""
+    from tests import chemkin_writer as CW
+    m = B.load_chemkin(CW.write(I.two_range(mech9, 1000.0, 0.5, seed=2))[0])
+    case = I.config1(nx=96, ny=40, mech=m)
+    check(B, ref, case, 1, TOL1)
+    check(B, ref, case, 20, TOL100)
