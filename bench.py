@@ -63,8 +63,12 @@ def chem_ops_per_cell(mech):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (flux: stages 2 and 3; the first stage reads U^n only
 # once) from the committed `ncu --set full` captures named in profiles/*_summary.md; None where no capture exists.
-NCU_TRAFFIC_BYTES = {
-    ("cfg2_2d_channel_4096x512", "flux"): 6.26e8,       # profiles/r1f_summary.md
+NCU_TRAFFIC_BYTES = {                                   # profiles/r2_summary.md (captures prof_r2_cfg4 / cfg2 / cfg3)
+    ("cfg4_3d_256cubed", "chem"): 6.12e9,
+    ("cfg4_3d_256cubed", "flux"): 13.33e9,
+    ("cfg2_2d_channel_4096x512", "flux"): 6.31e8,
+    ("cfg2_2d_channel_4096x512", "chem"): 3.15e8,
+    ("cfg3_amr_8192x16x16", "flux"): 9.65e8,
 }
 NCU_TRAFFIC_SOURCE = "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch (profiles/*_summary.md)"
 

@@ -23,8 +23,9 @@
  * No blocking, fusion or reordering beyond that.  OpenMP only splits independent cells/lines;
  * reductions are exact max, so results do not depend on the thread count.
  *
- * Pins: tests/test_oracle_*.py (closed forms, exact Riemann solution, conservation,
- * finite differences, LAPACK, brute force).  Parity unpinned: absolute accuracy of the
+ * Pins: tests/test_oracle_*.py (closed forms, exact Riemann solution, conservation, finite differences, LAPACK,
+ * brute force, ghost cells from global coordinates, mirrored periodic boxes; for the crossover advance and the
+ * two-range thermo data see DESIGN.md section 3).  Parity unpinned: absolute accuracy of the
  * synthetic multi-step detonations (configs 1-4) -- only invariants apply there.
  */
 #include <math.h>
