@@ -815,3 +815,138 @@ int jref_set_threads(int n) {
   (void)n; return 1;
 #endif
 }
+
+/* ------------------------------------------------------------------ regridding (JAX-AMR "update refinement layer")
+ * PAPER.md:73-75 (refinement criterion mask + buffer cells -> blocks to refine), :123 (update of the refinement layer
+ * keeps the data of blocks with the same global index), :175-184 (get_refinement_grid_mask, get_refinement_block_mask,
+ * get_refinement_block_info, get_refinement_block_data, find_and_update_unaltered_block), :115 (one-to-four).
+ * Two levels, ratio 2; the level-0 patches are the first n0 entries of the list and tile the domain.  DESIGN.md reading
+ * B12:
+ *   1. mask (level-0 cells): max_d |rho(i + e_d) - rho(i - e_d)| / (2 rho(i)) > thr, on the level-0 state (covered cells
+ *      hold the average of their fine cells) with its ghost layers filled;
+ *   2. buffer: every cell within nbuf cells (in every direction: a box) of a masked cell is marked too, across patch
+ *      boundaries and periodic sides, not across walls / outflow sides;
+ *   3. a sub-region (level-0 patch k, sub-index s in {0,1}^ndim) is refined if it contains a marked cell;
+ *   4. the new level-1 list follows the level-0 patches, ordered by parent, sub-index x fastest; same-level neighbours
+ *      through the parents' neighbour lists;
+ *   5. data: a block that existed before (same parent and sub-index) keeps its data, a new one is the one-to-four
+ *      injection of its parent's sub-region (T likewise).
+ * Outputs (caller-allocated for the worst case n0 (1 + 2^ndim) patches): level, nbr [2 ndim], parent [1 + ndim] per
+ * patch; Unew [np_new][nvar][cells], Tnew [np_new][cells] in the interior layout of jref_set_state. */
+int jref_regrid(jref_ctx *c, double thr, int nbuf, int *np_new, int32_t *level, int32_t *nbr, int32_t *parent,
+                double *Unew, double *Tnew) {
+  if (!c || !c->have_state || c->g.n_patches <= 0 || c->g.n_levels != 2 || nbuf < 0 || nbuf > 64) return JREF_EINVAL;
+  const int nd = c->g.ndim, nf = 2 * nd, nv = c->nvar, nsub = 1 << nd;
+  const int *n = c->g.n;
+  int n0 = 0;
+  while (n0 < c->np && c->level[n0] == 0) n0++;
+  for (int p = n0; p < c->np; p++) if (c->level[p] != 1) return JREF_EINVAL;       /* level-0 patches first */
+  const long ic = (long)n[0] * n[1] * n[2];
+  /* 1. mask on the padded level-0 arrays (ghosts filled from neighbours / physical sides) */
+  ghost_fill(c, c->U);
+  unsigned char *mark = calloc((size_t)n0 * c->pc, 1), *tmp = calloc((size_t)n0 * c->pc, 1);
+  if (!mark || !tmp) { free(mark); free(tmp); return JREF_ENOMEM; }
+  for (int p = 0; p < n0; p++)
+    for (int k = 0; k < n[2]; k++) for (int j = 0; j < n[1]; j++) for (int i = 0; i < n[0]; i++) {
+      const double *rho = c->U + (long)p * nv * c->pc;
+      long id = cidx(c, i, j, k);
+      double g = 0.0;
+      for (int d = 0; d < nd; d++) {
+        double a = fabs(rho[id + c->st[d]] - rho[id - c->st[d]]) / (2.0 * rho[id]);
+        if (a > g) g = a;
+      }
+      mark[(long)p * c->pc + id] = g > thr;
+    }
+  /* 2. buffer: nbuf passes of a one-cell box dilation; a pass reads the marks of neighbouring patches through a
+   *    ghost layer of marks filled by the same neighbour rule (periodic sides wrap, other physical sides contribute 0) */
+  for (int pass = 0; pass < nbuf; pass++) {
+    /* ghost marks, one layer, direction by direction so that edge / corner cells arrive after nd sweeps */
+    for (int d = 0; d < nd; d++)
+      for (int p = 0; p < n0; p++)
+        for (int side = 0; side < 2; side++) {
+          int f = 2 * d + side, q = c->nbr[p * nf + f];
+          int bc = side == 0 ? c->g.bc_lo[d] : c->g.bc_hi[d];
+          if (q < 0 && bc == BC_PERIODIC) q = p;                     /* single patch across a periodic direction */
+          int lo[3] = {0, 0, 0}, hi[3] = {n[0], n[1], n[2]};
+          for (int e = 0; e < d; e++) { lo[e] = -1; hi[e] = n[e] + 1; }   /* include the ghost marks of earlier sweeps */
+          lo[d] = side == 0 ? -1 : n[d]; hi[d] = lo[d] + 1;
+          for (int k = lo[2]; k < hi[2]; k++) for (int j = lo[1]; j < hi[1]; j++) for (int i = lo[0]; i < hi[0]; i++) {
+            int src[3] = {i, j, k};
+            src[d] = side == 0 ? n[d] - 1 : 0;
+            unsigned char v = 0;
+            if (q >= 0 && (c->nbr[p * nf + f] >= 0 || bc == BC_PERIODIC)) v = mark[(long)q * c->pc + cidx(c, src[0], src[1], src[2])];
+            mark[(long)p * c->pc + cidx(c, i, j, k)] = v;
+          }
+        }
+    memcpy(tmp, mark, (size_t)n0 * c->pc);
+    for (int p = 0; p < n0; p++)
+      for (int k = 0; k < n[2]; k++) for (int j = 0; j < n[1]; j++) for (int i = 0; i < n[0]; i++) {
+        unsigned char v = 0;
+        for (int dk = (nd > 2 ? -1 : 0); dk <= (nd > 2 ? 1 : 0); dk++)
+          for (int dj = (nd > 1 ? -1 : 0); dj <= (nd > 1 ? 1 : 0); dj++)
+            for (int di = -1; di <= 1; di++) v |= tmp[(long)p * c->pc + cidx(c, i + di, j + dj, k + dk)];
+        mark[(long)p * c->pc + cidx(c, i, j, k)] = v;
+      }
+  }
+  free(tmp);
+  /* 3. sub-regions that hold a marked cell */
+  unsigned char *flag = calloc((size_t)n0 * nsub, 1);
+  int *newid = malloc(sizeof(int) * (size_t)n0 * nsub), *oldid = malloc(sizeof(int) * (size_t)n0 * nsub);
+  for (int p = 0; p < n0; p++)
+    for (int k = 0; k < n[2]; k++) for (int j = 0; j < n[1]; j++) for (int i = 0; i < n[0]; i++)
+      if (mark[(long)p * c->pc + cidx(c, i, j, k)]) {
+        int s = (i >= n[0] / 2 ? 1 : 0) + (nd > 1 && j >= n[1] / 2 ? 2 : 0) + (nd > 2 && k >= n[2] / 2 ? 4 : 0);
+        flag[p * nsub + s] = 1;
+      }
+  free(mark);
+  /* 4. the new list */
+  for (int q = 0; q < n0 * nsub; q++) { newid[q] = -1; oldid[q] = -1; }
+  for (int p = n0; p < c->np; p++) {
+    const int *par = c->parent + p * (1 + nd);
+    int s = par[1] + (nd > 1 ? 2 * par[2] : 0) + (nd > 2 ? 4 * par[3] : 0);
+    oldid[par[0] * nsub + s] = p;
+  }
+  int np2 = n0;
+  for (int p = 0; p < n0; p++) for (int s = 0; s < nsub; s++) if (flag[p * nsub + s]) newid[p * nsub + s] = np2++;
+  for (int p = 0; p < n0; p++) {
+    level[p] = 0;
+    for (int f = 0; f < nf; f++) nbr[p * nf + f] = c->nbr[p * nf + f];
+    for (int e = 0; e <= nd; e++) parent[p * (1 + nd) + e] = -1;
+  }
+  for (int p = 0; p < n0; p++) for (int s = 0; s < nsub; s++) {
+    int id = newid[p * nsub + s];
+    if (id < 0) continue;
+    level[id] = 1;
+    parent[id * (1 + nd)] = p;
+    for (int e = 0; e < nd; e++) parent[id * (1 + nd) + 1 + e] = (s >> e) & 1;
+    for (int d = 0; d < nd; d++) for (int side = 0; side < 2; side++) {
+      int sd = (s >> d) & 1, k2 = p, s2;
+      if ((side == 0 && sd == 1) || (side == 1 && sd == 0)) s2 = s ^ (1 << d);            /* the sibling inside the parent */
+      else { k2 = c->nbr[p * nf + 2 * d + side]; s2 = s ^ (1 << d); }                    /* across the parent's face */
+      nbr[id * nf + 2 * d + side] = k2 >= 0 ? newid[k2 * nsub + s2] : -1;
+    }
+  }
+  /* 5. data: level 0 as it is; level 1 carried over or injected */
+  for (int p = 0; p < np2; p++) {
+    int src = -1, par = -1, sub[3] = {0, 0, 0};
+    if (p < n0) src = p;
+    else {
+      par = parent[p * (1 + nd)];
+      for (int e = 0; e < nd; e++) sub[e] = parent[p * (1 + nd) + 1 + e];
+      src = oldid[par * nsub + sub[0] + 2 * sub[1] + 4 * sub[2]];
+    }
+    for (int k = 0; k < n[2]; k++) for (int j = 0; j < n[1]; j++) for (int i = 0; i < n[0]; i++) {
+      long o = ((long)k * n[1] + j) * n[0] + i, sid; int q;
+      if (src >= 0) { q = src; sid = cidx(c, i, j, k); }
+      else {                                            /* one-to-four: the coarse cell that contains this fine cell */
+        q = par;
+        sid = cidx(c, (sub[0] * n[0] + i) / 2, nd > 1 ? (sub[1] * n[1] + j) / 2 : 0, nd > 2 ? (sub[2] * n[2] + k) / 2 : 0);
+      }
+      for (int v = 0; v < nv; v++) Unew[((long)p * nv + v) * ic + o] = c->U[((long)q * nv + v) * c->pc + sid];
+      Tnew[(long)p * ic + o] = c->T[(long)q * c->pc + sid];
+    }
+  }
+  free(flag); free(newid); free(oldid);
+  *np_new = np2;
+  return JREF_OK;
+}

@@ -147,6 +147,19 @@ class RefSolver:
         assert rc == 0, rc
         return U, T
 
+    def regrid(self, thr, nbuf):
+        """jref_regrid: (level, nbr, parent, U, T) of the regridded two-level list (level-0 patches first)."""
+        n0cap = self.np_ * (1 + (1 << self.ndim))
+        nf = 2 * self.ndim
+        level = np.zeros(n0cap, np.int32); nbr = np.zeros((n0cap, nf), np.int32); parent = np.zeros((n0cap, 1 + self.ndim), np.int32)
+        U = np.zeros((n0cap,) + self.shape[1:]); T = np.zeros((n0cap,) + self.shape[2:])
+        n = C.c_int(0)
+        rc = lib().jref_regrid(self._h, C.c_double(thr), int(nbuf), C.byref(n), _ptr(level), _ptr(nbr), _ptr(parent), _ptr(U), _ptr(T))
+        if rc:
+            raise RuntimeError(f"jref_regrid failed: {rc}")
+        k = n.value
+        return level[:k].copy(), nbr[:k].copy(), parent[:k].copy(), U[:k].copy(), T[:k].copy()
+
     def close(self):
         if self._h:
             lib().jref_destroy(self._h)

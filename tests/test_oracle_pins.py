@@ -1009,3 +1009,110 @@ def test_two_range_roundtrip_and_energy_conservation_in_a_step(ref, mech9):
         ry = np.concatenate([Us[0, 3:, 0, 0, 0], [Us[0, 0, 0, 0, 0] - Us[0, 3:, 0, 0, 0].sum()]])
         return (ry / m3.W) @ el
     assert np.abs(moles(U1) - moles(U.reshape(1, -1, 1, 1, 1))).max() <= 1e-12 * np.abs(moles(U1)).max()
+
+
+# ----------------------------------------------------------------------------- regridding (rest of SURVEY NEXT-1)
+def _assemble_level0(case, U, n0, NX, NY):
+    """level-0 density as one global array, from the generator's patch origins"""
+    npc = case.grid.n[0]
+    rho = np.zeros((NY, NX))
+    for p in range(n0):
+        ox, oy = case.blocks.origin[p]
+        rho[oy:oy + npc, ox:ox + npc] = U[p, 0, 0]
+    return rho
+
+
+def _brute_force_flags(rho, thr, nbuf, npc, wall=True):
+    """criterion, box dilation and sub-region flags recomputed on the global array (reflecting walls: mirror ghosts)"""
+    NY, NX = rho.shape
+    pad = np.pad(rho, 1, mode="symmetric" if wall else "wrap")                 # mirror about the wall face / periodic
+    gx = np.abs(pad[1:-1, 2:] - pad[1:-1, :-2]) / (2 * rho)
+    gy = np.abs(pad[2:, 1:-1] - pad[:-2, 1:-1]) / (2 * rho)
+    m = np.maximum(gx, gy) > thr
+    for _ in range(nbuf):
+        pm = np.pad(m, 1, mode="constant" if wall else "wrap")
+        m = np.zeros_like(m)
+        for dj in (0, 1, 2):
+            for di in (0, 1, 2):
+                m |= pm[dj:dj + NY, di:di + NX]
+    h = npc // 2
+    return m.reshape(NY // h, h, NX // h, h).any(axis=(1, 3))                 # [sub-region row, sub-region column]
+
+
+def test_regrid_marks_buffers_and_rebuilds_the_block_list(ref, mech9):
+    """PAPER.md:73-75, :123, :175-184 (reading B12): the refined sub-regions are exactly those that hold a cell whose
+    relative density jump exceeds the threshold or that lies within nbuf cells of one -- recomputed here by brute force
+    on the assembled global array --; blocks that existed keep their data bitwise, new ones are the one-to-four
+    injection of their parent; neighbour lists follow the geometry; regridding the result changes nothing."""
+    pcols, prows, npc = 16, 8, 8
+    base = I.config2(nx=pcols * npc, ny=prows * npc)                          # hot driver in the first 8 columns, walls / outflow
+    base.grid.bc_hi = (I.BC_REFLECT, I.BC_REFLECT, 0)
+    m0 = np.zeros((prows, pcols), bool); m0[:, 0] = True; m0[:, 5] = True      # refined so far: patch columns 0 and 5
+    c = I.refine_uniform(base, (npc, npc), m0)
+    n0, NX, NY = pcols * prows, pcols * npc, prows * npc
+    s = ref.RefSolver(c.grid, c.mech, c.blocks); s.set_state(c.U, c.T)
+    s.step(3, cfl=c.cfl)                                                     # a state with fine data that differs from its parents
+    U, T = s.get_state()
+    for thr, nbuf in ((0.05, 0), (0.05, 2), (0.2, 3), (1e9, 1)):
+        lev, nbr, par, Un, Tn = s.regrid(thr, nbuf)
+        want = _brute_force_flags(_assemble_level0(c, U, n0, NX, NY), thr, nbuf, npc)
+        got = np.zeros_like(want)
+        assert (lev[:n0] == 0).all() and (lev[n0:] == 1).all()
+        for p in range(n0, len(lev)):
+            k, sx, sy = par[p]
+            ox, oy = c.blocks.origin[k]
+            got[2 * (oy // npc) + sy, 2 * (ox // npc) + sx] = True
+        assert np.array_equal(got, want), (thr, nbuf, got.sum(), want.sum())
+        assert len(lev) - n0 == want.sum()
+        if thr > 1e8:
+            assert len(lev) == n0
+        # data: level 0 untouched; carried-over blocks bitwise, new blocks injected
+        assert np.array_equal(Un[:n0], U[:n0]) and np.array_equal(Tn[:n0], T[:n0])
+        old = {tuple(c.blocks.parent[p]): p for p in range(n0, c.grid.n_patches)}
+        carried = fresh = 0
+        for p in range(n0, len(lev)):
+            key = tuple(par[p])
+            if key in old:
+                assert np.array_equal(Un[p], U[old[key]]) and np.array_equal(Tn[p], T[old[key]]); carried += 1
+            else:
+                k, sx, sy = par[p]; h = npc // 2
+                blk = U[k, :, 0, sy * h:(sy + 1) * h, sx * h:(sx + 1) * h]
+                assert np.array_equal(Un[p, :, 0], np.repeat(np.repeat(blk, 2, axis=1), 2, axis=2)); fresh += 1
+        if nbuf == 2:
+            assert carried > 0 and fresh > 0 and carried < c.grid.n_patches - n0      # some kept, some new, some dropped
+        # neighbours from geometry: fine-patch coordinates (fx, fy) -> id
+        pos = {}
+        for p in range(n0, len(lev)):
+            k, sx, sy = par[p]; ox, oy = c.blocks.origin[k]
+            pos[(2 * (ox // npc) + sx, 2 * (oy // npc) + sy)] = p
+        for (fx, fy), p in pos.items():
+            assert nbr[p].tolist() == [pos.get((fx - 1, fy), -1), pos.get((fx + 1, fy), -1), pos.get((fx, fy - 1), -1), pos.get((fx, fy + 1), -1)]
+        assert np.array_equal(nbr[:n0], c.blocks.nbr[:n0])
+        # idempotent: the regridded list, regridded again with the same parameters, is itself
+        if len(lev) > n0:
+            g2 = I.Grid(2, c.grid.n, c.grid.dx, c.grid.bc_lo, c.grid.bc_hi, n_patches=len(lev), n_levels=2, ratio=2)
+            s2 = ref.RefSolver(g2, c.mech, I.Blocks(lev, nbr, par)); s2.set_state(Un, Tn)
+            lev2, nbr2, par2, Un2, Tn2 = s2.regrid(thr, nbuf)
+            assert np.array_equal(lev2, lev) and np.array_equal(nbr2, nbr) and np.array_equal(par2, par) and np.array_equal(Un2, Un)
+
+
+def test_regrid_periodic_buffer_wraps_and_the_new_list_runs(ref, mech9):
+    """Buffer cells cross periodic sides (through the neighbour lists of a tiled periodic grid) and stop at nothing else;
+    the regridded list is a valid input of the solver."""
+    base = _random_smooth_2d(mech9, 64, 32, 17, I.BC_PERIODIC)
+    base.U[0, :, 0, :, 60:64] *= 1.6                                         # a density jump next to the periodic seam
+    c = I.refine_uniform(base, (8, 8), np.zeros((4, 8), bool))               # no level-1 patches yet
+    c.grid.n_levels = 2
+    s = ref.RefSolver(c.grid, c.mech, c.blocks); s.set_state(c.U, c.T)
+    lev, nbr, par, Un, Tn = s.regrid(0.1, 3)
+    want = _brute_force_flags(base.U[0, 0, 0], 0.1, 3, 8, wall=False)
+    got = np.zeros_like(want)
+    for p in range(32, len(lev)):
+        k, sx, sy = par[p]; ox, oy = c.blocks.origin[k]
+        got[2 * (oy // 8) + sy, 2 * (ox // 8) + sx] = True
+    assert np.array_equal(got, want) and got[:, 0].any() and got[:, -1].any()          # both sides of the seam
+    g2 = I.Grid(2, c.grid.n, c.grid.dx, c.grid.bc_lo, c.grid.bc_hi, n_patches=len(lev), n_levels=2, ratio=2)
+    s2 = ref.RefSolver(g2, c.mech, I.Blocks(lev, nbr, par)); s2.set_state(Un, Tn)
+    s2.step(3, cfl=0.2)
+    U3, _ = s2.get_state()
+    assert s2.status == 0 and np.isfinite(U3).all()
