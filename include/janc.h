@@ -166,6 +166,21 @@ int janc_halo(janc_ctx *, int stage, int side, double *buf_dev, int unpack);
 /* Where the reduction slots sit inside the bound workspace (byte offset, number of 64-bit slots). */
 int janc_reduction_slots(const janc_ctx *, size_t *byte_offset, size_t *count);
 
+/* Regridding of a two-level block list (JAX-AMR "update refinement layer": PAPER.md:73-75 refinement criterion mask +
+ * buffer cells, :123 / :184 unaltered blocks keep their data, :175-184 get_refinement_grid_mask / _block_mask / _block_info
+ * / _block_data; reading B12).  The level-0 patches must be the first entries of the list and tile the domain.
+ * janc_regrid_plan: marks the level-0 cells with max_d |rho(i+e_d) - rho(i-e_d)| / (2 rho(i)) > thr, adds nbuf buffer
+ * cells in every direction (across patch boundaries and periodic sides), refines every fixed sub-region (parent, s in
+ * {0,1}^ndim) that holds a marked cell, and returns the new list in host arrays sized for the worst case
+ * n0 (1 + 2^ndim) patches: np_new, level[np], nbr[np][2 ndim], parent[np][1 + ndim] -- level 0 unchanged, then the
+ * level-1 blocks ordered by parent and sub-index (x fastest).  janc_regrid_fill: the state of that list in the interior
+ * layout of janc_set_state, U_new[np_new][nvar][cells], T_new[np_new][cells] (device or host): blocks that existed keep
+ * their data, new ones are the one-to-four injection of their parent.  The caller then creates a context
+ * for the new list (janc_create with n_patches = np_new, janc_set_blocks, janc_set_state).  Both calls synchronise and
+ * use the RK scratch registers: call them between steps. */
+int janc_regrid_plan(janc_ctx *, double thr, int nbuf, int32_t *np_new, int32_t *level, int32_t *nbr, int32_t *parent);
+int janc_regrid_fill(janc_ctx *, double *U_new, double *T_new, int on_device);
+
 /* dt of the most recent step (cfl()), read from the device; synchronises. */
 int janc_last_dt(janc_ctx *, double *dt);
 

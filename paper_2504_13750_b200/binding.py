@@ -25,7 +25,7 @@ BC_EXCHANGE = 3
 EXPORTS = ["janc_mech_parse", "janc_mech_file_view", "janc_mech_file_species", "janc_mech_file_free",
            "janc_create", "janc_set_option", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
            "janc_set_blocks", "janc_set_state", "janc_step", "janc_step_part", "janc_halo_doubles", "janc_halo",
-           "janc_reduction_slots", "janc_last_dt", "janc_get_state", "janc_status",
+           "janc_reduction_slots", "janc_last_dt", "janc_regrid_plan", "janc_regrid_fill", "janc_get_state", "janc_status",
            "janc_launch_count", "janc_debug_cons2prim", "janc_profile_step",
            "janc_measure_dfma_peak", "janc_chem_kernel", "janc_jit_log", "janc_jit_probe",
            "janc_last_error", "janc_destroy"]
@@ -75,6 +75,8 @@ def lib():
         L.janc_halo.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]
         L.janc_reduction_slots.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.janc_last_dt.argtypes = [C.c_void_p, C.c_void_p]
+        L.janc_regrid_plan.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.janc_regrid_fill.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.janc_status.argtypes = [C.c_void_p]
         L.janc_launch_count.argtypes = [C.c_void_p]
         L.janc_launch_count.restype = C.c_longlong
@@ -283,6 +285,21 @@ class Solver:
         self._check(lib().janc_reduction_slots(self._h, C.byref(off), C.byref(cnt)), "janc_reduction_slots")
         a = self._ws_off + off.value
         return self.workspace[a:a + 8 * cnt.value].view(self._torch.int64)
+
+    def regrid(self, thr, nbuf):
+        """janc_regrid_plan + janc_regrid_fill: (level, nbr, parent, U, T) of the regridded two-level list (host arrays)."""
+        nd = 1 + (self.shape[3] > 1) + (self.shape[2] > 1)
+        cap = self.np_ * (1 + (1 << nd))
+        level = np.zeros(cap, np.int32); nbr = np.zeros((cap, 2 * nd), np.int32); parent = np.zeros((cap, 1 + nd), np.int32)
+        n = C.c_int32(0)
+        self._check(lib().janc_regrid_plan(self._h, float(thr), int(nbuf), C.byref(n), _ptr(level), _ptr(nbr), _ptr(parent)),
+                    "janc_regrid_plan")
+        k = n.value
+        torch = self._torch
+        U = torch.empty((k,) + self.shape[1:], dtype=torch.float64, device=f"cuda:{self.device}")
+        T = torch.empty((k,) + self.shape[2:], dtype=torch.float64, device=f"cuda:{self.device}")
+        self._check(lib().janc_regrid_fill(self._h, C.c_void_p(U.data_ptr()), C.c_void_p(T.data_ptr()), 1), "janc_regrid_fill")
+        return level[:k].copy(), nbr[:k].copy(), parent[:k].copy(), U.cpu().numpy(), T.cpu().numpy()
 
     def last_dt(self):
         """dt of the most recent step (device scalar), synchronising."""

@@ -121,3 +121,93 @@ __global__ void __launch_bounds__(256) k_halo(Params P, double *__restrict__ U, 
   if (unpack) arr[ci] = buf[idx];
   else buf[idx] = arr[ci];
 }
+
+// ------------------------------------------------------------------------------------------------ regridding kernels
+// PAPER.md:73-75 (criterion mask + buffer cells -> blocks to refine), :175-184; reading B12.
+// mark[p][padded cell] (bytes) for the n0 level-0 patches; the ghost layers of rho must be filled (k_ghost, level 0).
+__global__ void __launch_bounds__(256) k_regrid_mark(Params P, const double *__restrict__ U, unsigned char *mark, double thr) {
+  const int patch = blockIdx.y;
+  const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ncell) return;
+  const int i = (int)(t % P.n[0]);
+  const long long r = t / P.n[0];
+  const int j = (int)(r % P.n[1]), k = (int)(r / P.n[1]);
+  const long long id = cell_index(P, i, j, k);
+  const double *rho = U + (long long)patch * P.nvar * P.pc;
+  double g = 0.0;
+  for (int d = 0; d < P.ndim; d++) g = fmax(g, fabs(rho[id + P.st[d]] - rho[id - P.st[d]]) / (2.0 * rho[id]));
+  mark[(long long)patch * P.pc + id] = g > thr;
+}
+
+// the mark of cell (c[0], c[1], c[2]) of level-0 patch p, where each coordinate may lie one cell outside the patch: hop
+// through the same-level neighbour lists, highest direction first (periodic sides of a single patch wrap onto itself;
+// beyond a wall / outflow side there is nothing to refine)
+__device__ __forceinline__ int regrid_mark_at(const Params &P, const unsigned char *mark, int p, int c0, int c1, int c2) {
+  int c[3] = {c0, c1, c2};
+  for (int d = P.ndim - 1; d >= 0; d--) {
+    if (c[d] >= 0 && c[d] < P.n[d]) continue;
+    const int side = c[d] < 0 ? 0 : 1;
+    int q = P.nbr[p * 2 * P.ndim + 2 * d + side];
+    if (q < 0 && (side == 0 ? P.bc_lo[d] : P.bc_hi[d]) == 0) q = p;
+    if (q < 0) return 0;
+    p = q;
+    c[d] = side == 0 ? P.n[d] - 1 : 0;
+  }
+  return mark[(long long)p * P.pc + cell_index(P, c[0], c[1], c[2])];
+}
+
+// one pass of the one-cell box dilation: out = OR of the 3^ndim neighbourhood of in
+__global__ void __launch_bounds__(256) k_regrid_dilate(Params P, const unsigned char *in, unsigned char *out) {
+  const int patch = blockIdx.y;
+  const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ncell) return;
+  const int i = (int)(t % P.n[0]);
+  const long long r = t / P.n[0];
+  const int j = (int)(r % P.n[1]), k = (int)(r / P.n[1]);
+  int v = 0;
+  for (int dk = (P.ndim > 2 ? -1 : 0); dk <= (P.ndim > 2 ? 1 : 0); dk++)
+    for (int dj = (P.ndim > 1 ? -1 : 0); dj <= (P.ndim > 1 ? 1 : 0); dj++)
+      for (int di = -1; di <= 1; di++) v |= regrid_mark_at(P, in, patch, i + di, j + dj, k + dk);
+  out[(long long)patch * P.pc + cell_index(P, i, j, k)] = (unsigned char)v;
+}
+
+// flags[p][sub-region] = 1 if the sub-region holds a marked cell (sub index: x bit 0, y bit 1, z bit 2)
+__global__ void __launch_bounds__(256) k_regrid_flags(Params P, const unsigned char *mark, int *flags) {
+  const int patch = blockIdx.y;
+  const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ncell) return;
+  const int i = (int)(t % P.n[0]);
+  const long long r = t / P.n[0];
+  const int j = (int)(r % P.n[1]), k = (int)(r / P.n[1]);
+  if (mark[(long long)patch * P.pc + cell_index(P, i, j, k)]) {
+    const int s = (i >= P.n[0] / 2 ? 1 : 0) + (P.ndim > 1 && j >= P.n[1] / 2 ? 2 : 0) + (P.ndim > 2 && k >= P.n[2] / 2 ? 4 : 0);
+    flags[patch * (1 << P.ndim) + s] = 1;
+  }
+}
+
+// data of the regridded list in the interior layout: src[p] >= 0: copy of old patch src[p]; else one-to-four injection
+// of sub-region sub[p] of parent par[p]; T likewise.  grid: (cells, new patches)
+__global__ void __launch_bounds__(256) k_regrid_fill(Params P, const double *__restrict__ U, const int *src, const int *par, const int *sub,
+                                                     double *Unew, double *Tnew) {
+  const int p = blockIdx.y;
+  const long long ncell = (long long)P.n[0] * P.n[1] * P.n[2];
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ncell) return;
+  const int i = (int)(t % P.n[0]);
+  const long long r = t / P.n[0];
+  const int j = (int)(r % P.n[1]), k = (int)(r / P.n[1]);
+  int q = src[p];
+  long long sid;
+  if (q >= 0) sid = cell_index(P, i, j, k);
+  else {
+    q = par[p];
+    const int s = sub[p];
+    sid = cell_index(P, ((s & 1) * P.n[0] + i) / 2, P.ndim > 1 ? (((s >> 1) & 1) * P.n[1] + j) / 2 : 0,
+                     P.ndim > 2 ? (((s >> 2) & 1) * P.n[2] + k) / 2 : 0);
+  }
+  for (int v = 0; v < P.nvar; v++) Unew[((long long)p * P.nvar + v) * ncell + t] = U[((long long)q * P.nvar + v) * P.pc + sid];
+  Tnew[(long long)p * ncell + t] = P.T[(long long)q * P.pc + sid];
+}

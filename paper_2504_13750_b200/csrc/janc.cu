@@ -60,6 +60,7 @@ struct janc_ctx {
   int lvl_first[2] = {0, 0}, lvl_count[2] = {0, 0};   // patches of each level if they are contiguous (by_level)
   bool by_level = true;
   int act0 = 0, actn = 0;                             // patches the kernels of the current launches act on
+  std::vector<int> rg_src, rg_par, rg_sub;            // regrid plan: where the data of every new patch comes from
   long long launches;
   int num_sms;
   // One step = 11..12 small launches; a step of each slot parity is captured once into a CUDA graph and replayed
@@ -1166,6 +1167,113 @@ extern "C" int janc_reduction_slots(const janc_ctx *c, size_t *byte_offset, size
   *byte_offset = (size_t)((const char *)c->P.slots - (const char *)c->A);     // A is the first piece of the workspace
   *count = JANC_NSLOT;
   return JANC_OK;
+}
+
+// ------------------------------------------------------------------ regridding (B12)
+extern "C" int janc_regrid_plan(janc_ctx *c, double thr, int nbuf, int32_t *np_new, int32_t *level, int32_t *nbr, int32_t *parent) {
+  int rc = check_ready(c);
+  if (rc) return rc;
+  if (!np_new || !level || !nbr || !parent || nbuf < 0 || nbuf > 64) return JANC_EINVAL;
+  const int nd = c->g.ndim, nf = 2 * nd, nsub = 1 << nd, np = c->np;
+  int n0 = 0;
+  while (n0 < np && c->level[n0] == 0) n0++;
+  if (c->g.n_patches <= 0 || c->g.n_levels != 2 || !c->by_level || n0 == 0) {
+    c->err = "janc_regrid_plan: a two-level block list with the level-0 patches first";
+    return JANC_EINVAL;
+  }
+  CK(cudaSetDevice(c->device));
+  // 1. criterion on the level-0 state with its ghosts filled; 2. nbuf box dilations (B holds the marks: free between steps)
+  set_active(c, 0, np, 1.0);
+  {
+    int amax = 1;
+    for (int d = 0; d < nd; d++) { int a = 1; for (int e = 0; e < nd; e++) if (e != d) a *= c->P.n[e]; if (a > amax) amax = a; }
+    const long long total = (long long)2 * nd * JANC_NG * amax * ((c->nvar + 2 + nd + GHOST_FPT - 1) / GHOST_FPT);
+    k_ghost<<<dim3((unsigned)((total + 255) / 256), (unsigned)np, 1), 256, 0, c->stream>>>(c->P, c->A, 0, amax);
+    note_launch(c, cudaGetLastError());
+  }
+  unsigned char *m0 = (unsigned char *)c->B, *m1 = m0 + align_up((size_t)n0 * c->P.pc, 256);
+  int *d_flags = (int *)(m1 + align_up((size_t)n0 * c->P.pc, 256));
+  const dim3 grid = cell_grid(c, 256, n0);
+  CK(cudaMemsetAsync(m0, 0, 2 * align_up((size_t)n0 * c->P.pc, 256) + (size_t)n0 * nsub * 4, c->stream));
+  k_regrid_mark<<<grid, 256, 0, c->stream>>>(c->P, c->A, m0, thr);
+  note_launch(c, cudaGetLastError());
+  for (int pass = 0; pass < nbuf; pass++) {
+    k_regrid_dilate<<<grid, 256, 0, c->stream>>>(c->P, m0, m1);
+    note_launch(c, cudaGetLastError());
+    unsigned char *t_ = m0; m0 = m1; m1 = t_;
+  }
+  k_regrid_flags<<<grid, 256, 0, c->stream>>>(c->P, m0, d_flags);
+  note_launch(c, cudaGetLastError());
+  std::vector<int> flags((size_t)n0 * nsub);
+  CK(cudaMemcpyAsync(flags.data(), d_flags, flags.size() * 4, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  if ((rc = take_launch_error(c)) != JANC_OK) return rc;
+  // 3. - 5. the new list (host): refined sub-regions in the order (parent, sub-index), neighbours through the parents
+  std::vector<int> newid((size_t)n0 * nsub, -1), oldid((size_t)n0 * nsub, -1);
+  for (int p = n0; p < np; p++) {
+    const int *par = &c->parent[(size_t)p * (1 + nd)];
+    int sidx = 0;
+    for (int e = 0; e < nd; e++) sidx |= par[1 + e] << e;
+    oldid[(size_t)par[0] * nsub + sidx] = p;
+  }
+  int np2 = n0;
+  for (int q = 0; q < n0 * nsub; q++) if (flags[q]) newid[q] = np2++;
+  c->rg_src.assign(np2, -1); c->rg_par.assign(np2, -1); c->rg_sub.assign(np2, 0);
+  for (int p = 0; p < n0; p++) {
+    level[p] = 0; c->rg_src[p] = p;
+    for (int f = 0; f < nf; f++) nbr[p * nf + f] = c->nbr[(size_t)p * nf + f];
+    for (int e = 0; e <= nd; e++) parent[p * (1 + nd) + e] = -1;
+  }
+  for (int p = 0; p < n0; p++)
+    for (int sidx = 0; sidx < nsub; sidx++) {
+      const int id = newid[(size_t)p * nsub + sidx];
+      if (id < 0) continue;
+      level[id] = 1;
+      parent[id * (1 + nd)] = p;
+      for (int e = 0; e < nd; e++) parent[id * (1 + nd) + 1 + e] = (sidx >> e) & 1;
+      for (int d = 0; d < nd; d++)
+        for (int side = 0; side < 2; side++) {
+          const int bit = (sidx >> d) & 1;
+          const bool inside = (side == 0) == (bit == 1);                 // the sibling across this face lies in the same parent
+          const int k2 = inside ? p : c->nbr[(size_t)p * nf + 2 * d + side];
+          nbr[id * nf + 2 * d + side] = k2 >= 0 ? newid[(size_t)k2 * nsub + (sidx ^ (1 << d))] : -1;
+        }
+      c->rg_src[id] = oldid[(size_t)p * nsub + sidx];
+      c->rg_par[id] = p; c->rg_sub[id] = sidx;
+    }
+  *np_new = np2;
+  return JANC_OK;
+}
+
+extern "C" int janc_regrid_fill(janc_ctx *c, double *U_new, double *T_new, int on_device) {
+  int rc = check_ready(c);
+  if (rc) return rc;
+  if (!U_new || !T_new) return JANC_EINVAL;
+  if (c->rg_src.empty()) { c->err = "janc_regrid_fill: no plan (call janc_regrid_plan first)"; return JANC_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  const int np2 = (int)c->rg_src.size();
+  const size_t nU = (size_t)np2 * c->nvar * c->ncell, nT = (size_t)np2 * c->ncell;
+  // device scratch in B: the three int lists, then (host output only) the new arrays
+  int *d_src = (int *)c->B, *d_par = d_src + np2, *d_sub = d_par + np2;
+  double *dU = U_new, *dT = T_new;
+  if (!on_device) {
+    dU = (double *)((char *)c->B + align_up((size_t)3 * np2 * 4, 256));
+    dT = dU + nU;
+    const size_t need = align_up((size_t)3 * np2 * 4, 256) + (nU + nT) * 8, have = (size_t)c->np * c->nvar * c->P.pc * 8 * 2;   // B and C are contiguous
+    if (need > have) { c->err = "janc_regrid_fill: the new list does not fit the scratch registers; pass device buffers"; return JANC_ENOMEM; }
+  }
+  CK(cudaMemcpyAsync(d_src, c->rg_src.data(), (size_t)np2 * 4, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(d_par, c->rg_par.data(), (size_t)np2 * 4, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(d_sub, c->rg_sub.data(), (size_t)np2 * 4, cudaMemcpyHostToDevice, c->stream));
+  set_active(c, 0, c->np, 1.0);
+  k_regrid_fill<<<cell_grid(c, 256, np2), 256, 0, c->stream>>>(c->P, c->A, d_src, d_par, d_sub, dU, dT);
+  note_launch(c, cudaGetLastError());
+  if (!on_device) {
+    CK(cudaMemcpyAsync(U_new, dU, nU * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaMemcpyAsync(T_new, dT, nT * 8, cudaMemcpyDeviceToHost, c->stream));
+  }
+  CK(cudaStreamSynchronize(c->stream));
+  return take_launch_error(c);
 }
 
 extern "C" int janc_last_dt(janc_ctx *c, double *dt) {

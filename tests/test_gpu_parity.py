@@ -535,3 +535,43 @@ def test_mechanism_read_from_chemkin_text_runs_on_the_gpu(B, ref, mech9):
     case = I.config1(nx=96, ny=40, mech=m)
     check(B, ref, case, 1, TOL1)
     check(B, ref, case, 20, TOL100)
+
+
+# ------------------------------------------------------------------ regridding (rest of SURVEY NEXT-1)
+def test_regrid_matches_the_oracle(B, ref, mech9):
+    """janc_regrid_plan / janc_regrid_fill (reading B12) against jref_regrid: identical
+    block lists (integer work: exact), identical data (copies and injections: bitwise) -- after both sides advanced the
+    same list; 2-D with walls (carried / new / dropped blocks), periodic 2-D, 1-D and 3-D; then the regridded list runs
+    on the GPU and stays in parity."""
+    base = I.config2(nx=128, ny=64)
+    base.grid.bc_hi = (I.BC_REFLECT, I.BC_REFLECT, 0)
+    m0 = np.zeros((8, 16), bool); m0[:, 0] = True; m0[:, 5] = True
+    c2 = I.refine_uniform(base, (8, 8), m0)
+    from tests.test_oracle_pins import _random_smooth_2d
+    per = _random_smooth_2d(mech9, 64, 32, 17, I.BC_PERIODIC)
+    per.U[0, :, 0, :, 60:64] *= 1.6
+    cp = I.refine_uniform(per, (8, 8), np.zeros((4, 8), bool)); cp.grid.n_levels = 2
+    b1 = I.config0(n=192)
+    b1.grid.bc_lo, b1.grid.bc_hi = (I.BC_REFLECT, 0, 0), (I.BC_OUTFLOW, 0, 0)
+    m1 = np.zeros(12, bool); m1[2] = True
+    c1 = I.refine_uniform(b1, (16,), m1)
+    b3 = I.config4(n=16, nspheres=2, radius=4)
+    m3 = np.zeros((2, 2, 2), bool); m3[0, 1, 0] = True
+    c3 = I.refine_uniform(b3, (8, 8, 8), m3)
+    for case, nsteps, thr, nbuf in ((c2, 3, 0.05, 2), (c2, 0, 0.2, 0), (cp, 0, 0.1, 3), (c1, 4, 0.02, 2), (c3, 1, 0.05, 1)):
+        g = B.Solver(case.grid, case.mech, case.blocks); g.set_state(case.U, case.T)
+        r = ref.RefSolver(case.grid, case.mech, case.blocks); r.set_state(case.U, case.T)
+        if nsteps:
+            g.step(nsteps, cfl=case.cfl); r.step(nsteps, cfl=case.cfl)
+            # the criterion is a threshold on data that agree to round-off only: give both sides the same state
+            Ur, Tr = r.get_state(); g.set_state(Ur, Tr)
+        lg, ng, pg, Ug, Tg = g.regrid(thr, nbuf)
+        lr, nr_, pr, Ur2, Tr2 = r.regrid(thr, nbuf)
+        assert np.array_equal(lg, lr) and np.array_equal(ng, nr_) and np.array_equal(pg, pr), case.name
+        assert np.array_equal(Ug, Ur2) and np.array_equal(Tg, Tr2), case.name
+        assert (lg == 1).sum() > 0
+        g.close(); r.close()
+        new = I.Case(case.name + "_regridded", I.Grid(case.grid.ndim, case.grid.n, case.grid.dx, case.grid.bc_lo, case.grid.bc_hi,
+                                                       n_patches=len(lg), n_levels=2, ratio=2),
+                     case.mech, Ug, Tg, case.cfl, 2, blocks=I.Blocks(lg, ng, pg))
+        check(B, ref, new, 2, TOL1 * 100)
