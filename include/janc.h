@@ -184,6 +184,28 @@ int janc_regrid_fill(janc_ctx *, double *U_new, double *T_new, int on_device);
 /* dt of the most recent step (cfl()), read from the device; synchronises. */
 int janc_last_dt(janc_ctx *, double *dt);
 
+/* The stable time step of a state WITHOUT a workspace and without any allocation (cfl(): dt = cfl *
+ * dx_min / max_d max_cells(|u_d| + c), with T, c from the cons->prim Newton iteration of PAPER.md:237-258, :306) -- for
+ * callers that cannot call cudaMalloc (CUDA graph capture, serving loops).  A variant of the cons->prim + max-reduction
+ * kernel whose per-CTA partial maxima and error flag live in a file-scope `static __device__` array of the library
+ * (csrc/static_scratch.cuh; 256 B + JANC_STATIC_MAX_CELLS / 256 x 3 doubles = 1.5 MiB that every GPU which loads the
+ * library holds until exit).  The context needs a mechanism only (janc_create + janc_set_mechanism; no workspace, blocks
+ * or state): it supplies grid, dx_min, species data and the stream.
+ *   U_dev   device, the interior layout of janc_set_state: [n_patches][nvar][nz][ny][nx]             (input, not modified)
+ *   T_dev   device, [n_patches][nz][ny][nx] Newton starting temperatures, or NULL = 1000 K           (input, not modified)
+ *   out_dev device, double[4]: dt, max(|u_x| + c), max(|u_y| + c), max(|u_z| + c) (0 for unused directions); dt is NaN
+ *           if the Newton iteration failed in some cell (the maxima then exclude such cells)        (output)
+ * Asynchronous on the context's stream; the caller owns all three buffers.  Returns JANC_EINVAL with a text in
+ * janc_last_error if n_patches * cells per patch exceeds JANC_STATIC_MAX_CELLS, or cfl <= 0; JANC_ESTATE without a
+ * mechanism.  Calls no cudaMalloc / cudaFree / allocating routine.  The first call of a context on a device resolves the
+ * array's device address (cudaGetSymbolAddress, once per device) and, if another context's species tables sit in that
+ * device's constant memory, drains the device and uploads its own: make that first call outside graph capture.
+ * ALL calls of the process on one device share the array (it keeps the last call's contents; the flag word is cleared at
+ * the start of every call): calls that overlap on the GPU -- different streams, or graphs replayed concurrently -- race;
+ * calls on one stream are ordered and safe. */
+#define JANC_STATIC_MAX_CELLS (1LL << 24)
+int janc_cfl_dt_static(janc_ctx *, const double *U_dev, const double *T_dev, double cfl, double *out_dev);
+
 /* Read the state back (U and/or T nullable).  Synchronises.  Returns JANC_ENONFINITE if the
  * device flag was raised since the last janc_set_state. */
 int janc_get_state(janc_ctx *, double *U, double *T, int on_device);

@@ -25,7 +25,8 @@ BC_EXCHANGE = 3
 EXPORTS = ["janc_mech_parse", "janc_mech_file_view", "janc_mech_file_species", "janc_mech_file_free",
            "janc_create", "janc_set_option", "janc_set_mechanism", "janc_workspace_bytes", "janc_bind_workspace",
            "janc_set_blocks", "janc_set_state", "janc_step", "janc_step_part", "janc_halo_doubles", "janc_halo",
-           "janc_reduction_slots", "janc_last_dt", "janc_regrid_plan", "janc_regrid_fill", "janc_get_state", "janc_status",
+           "janc_reduction_slots", "janc_last_dt", "janc_regrid_plan", "janc_regrid_fill", "janc_cfl_dt_static", "janc_get_state",
+           "janc_status",
            "janc_launch_count", "janc_debug_cons2prim", "janc_profile_step",
            "janc_measure_dfma_peak", "janc_chem_kernel", "janc_jit_log", "janc_jit_probe",
            "janc_last_error", "janc_destroy"]
@@ -77,6 +78,7 @@ def lib():
         L.janc_last_dt.argtypes = [C.c_void_p, C.c_void_p]
         L.janc_regrid_plan.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.janc_regrid_fill.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.janc_cfl_dt_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.janc_status.argtypes = [C.c_void_p]
         L.janc_launch_count.argtypes = [C.c_void_p]
         L.janc_launch_count.restype = C.c_longlong
@@ -306,6 +308,15 @@ class Solver:
         t = C.c_double(0.0)
         self._check(lib().janc_last_dt(self._h, C.byref(t)), "janc_last_dt")
         return t.value
+
+    def cfl_dt_static(self, U, T, cfl, out):
+        """janc_cfl_dt_static: dt and the max(|u_d| + c) of the state U (T = Newton start or None), all CUDA tensors of the
+        caller (U, T in the interior layout of set_state; out: 4 doubles), enqueued on the solver's stream; allocates nothing."""
+        torch = self._torch
+        for t, n in ((U, int(np.prod(self.shape))), (T, int(np.prod(self.tshape))), (out, 4)):
+            assert t is None or (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n)
+        self._check(lib().janc_cfl_dt_static(self._h, C.c_void_p(U.data_ptr()), C.c_void_p(T.data_ptr()) if T is not None else None,
+                                             float(cfl), C.c_void_p(out.data_ptr())), "janc_cfl_dt_static")
 
     def get_state(self, device=False):
         if device:

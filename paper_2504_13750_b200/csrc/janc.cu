@@ -1362,3 +1362,5 @@ extern "C" int janc_measure_dfma_peak(int device, void *cuda_stream, double *dfm
   *dfma_per_s = best;
   return JANC_OK;
 }
+
+#include "static_scratch.cuh"   // janc_cfl_dt_static: the entry point that allocates nothing
