@@ -583,3 +583,163 @@ k_flux_rk2_tma(Params P, const double *U0, double *Uout, int slot_base, double c
     }
   }
 }
+
+// ------------------------------------------------------------------------------------------------
+// TMA variant of the 3-D kernel (materialised ghosts, even padded width).  The work of a tile is cut into units
+// (component m, direction d); a unit needs the tile extended by 3 cells along d only -- one dense box
+// {TX (+6), TY (+6), TZ (+6)} of U_m, one of u_d and, for the normal momentum and the energy, one of p -- which arrive
+// as cp.async.bulk.tensor boxes of a 4-D tensor map {Px, Py, Pz, fields} (one map per box shape), two units ahead of
+// the walk: while the pencils of unit u are walked, the boxes of unit u + 1 are in flight or landed.  No thread
+// executes a staging loop: the split fluxes 2f+- = F +- alpha U are formed by the walk from the raw boxes (as in the
+// 2-D kernel), the x and y contributions wait in the per-cell accumulator, and the thread that walks a z pencil
+// (lanes along x: coalesced) adds its own and applies the RK stage of its cells.  Same arithmetic, in the same order,
+// as k_flux_rk<3, ...>: results are bit-identical.
+__device__ __forceinline__ void tma_load_4d(double *dst, const CUtensorMap *map, unsigned long long *bar, int x, int y, int z, int f) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(dst)),
+               "l"(map), "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(x), "r"(y), "r"(z), "r"(f)
+               : "memory");
+}
+
+struct Flux3Maps { CUtensorMap U[3], V[3], P[3]; };       // [d]: the box shape of direction d over the stage state, vel, p
+
+template <int TX, int TY, int TZ, int SEG>
+struct Flux3TmaCfg {
+  static constexpr int NT = TX * TY * TZ / SEG;
+  static constexpr int TXB = TX + 2;                                      // x extent of the y / z boxes: a TMA box starts at a 16-byte aligned
+                                                                         // address, i.e. at an even padded x; interior cell 0 sits at x = 3
+  static constexpr int NB0 = (TX + 6) * TY * TZ, NB1 = TXB * (TY + 6) * TZ, NB2 = TXB * TY * (TZ + 6);   // doubles per box
+  static constexpr int NBMAX = NB0 > NB1 ? (NB0 > NB2 ? NB0 : NB2) : (NB1 > NB2 ? NB1 : NB2);
+  static constexpr int BOX = (NBMAX + 15) / 16 * 16;                      // 128-byte aligned slots
+  static constexpr int LP = TX | 1;
+  static constexpr int ROWS = TY * TZ;
+  static constexpr size_t SMEM = (size_t)(6 * BOX + ROWS * LP) * sizeof(double) + 64;
+  static_assert(TX % SEG == 0 && TY % SEG == 0 && TZ % SEG == 0 && (TX * 8) % 16 == 0, "tile");
+  static_assert(NT % TX == 0 && NT % ROWS == 0, "thread maps");
+};
+
+template <int TX, int TY, int TZ, int SEG>
+__global__ void __launch_bounds__(TX * TY * TZ / SEG, 2)
+k_flux_rk3_tma(Params P, const double *U0, double *Uout, int slot_base, double coef, int same_i,
+               const __grid_constant__ Flux3Maps M) {
+  using C = Flux3TmaCfg<TX, TY, TZ, SEG>;
+  constexpr int NT = C::NT;
+  extern __shared__ __align__(128) double flux_smem[];
+  double *sL = flux_smem + 6 * C::BOX;
+  unsigned long long *bars = (unsigned long long *)(sL + C::ROWS * C::LP);
+
+  const int tid = threadIdx.x;
+  const int patch = blockIdx.y + P.patch0;
+  const int lev = P.level[patch];
+  const int ntx = (P.n[0] + TX - 1) / TX, nty = (P.n[1] + TY - 1) / TY;
+  const int o0 = (blockIdx.x % ntx) * TX, o1 = ((blockIdx.x / ntx) % nty) * TY, o2 = (blockIdx.x / (ntx * nty)) * TZ;
+  const double dt = P.scal[0] * P.dt_scale;
+  const long long pbase = (long long)patch * P.pc;
+  const double *U0p = U0 + pbase * P.nvar;
+  double *Uop = Uout + pbase * P.nvar;
+  const int s1 = (int)P.st[1], s2 = (int)P.st[2];
+  const int goff = P.G[0] + P.G[1] * s1 + P.G[2] * s2;
+  double alpha[3], hidx[3];
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    alpha[d] = slot_value(P.slots + slot_base + lev * 3 + d);
+    hidx[d] = 0.5 * P.invdx[lev][d];
+  }
+  const bool same = same_i != 0;
+  const int nunits = 3 * P.nvar;
+
+  // unit u = 3 m + d goes to slot u & 1: boxes U, u_d, p at (3 slot + 0 / 1 / 2) * BOX.  d is a compile-time constant
+  // (the tensor maps are addressed statically in the kernel's parameter space).
+  auto issue = [&](int m, auto dc) {
+    constexpr int d = decltype(dc)::value;
+    const int s = (3 * m + d) & 1;
+    const bool needp = m == 1 + d || m == 4;
+    constexpr unsigned nb = (d == 0 ? C::NB0 : d == 1 ? C::NB1 : C::NB2) * 8u;
+    double *b = flux_smem + 3 * s * C::BOX;
+    const int cx = o0 + (d == 0 ? 0 : 2), cy = o1 + (d == 1 ? 0 : 3), cz = o2 + (d == 2 ? 0 : 3);     // padded coordinates (x even)
+    mbar_expect_tx(bars + s, needp ? 3 * nb : 2 * nb);
+    tma_load_4d(b, &M.U[d], bars + s, cx, cy, cz, patch * P.nvar + m);
+    tma_load_4d(b + C::BOX, &M.V[d], bars + s, cx, cy, cz, d * P.np + patch);
+    if (needp) tma_load_4d(b + 2 * C::BOX, &M.P[d], bars + s, cx, cy, cz, patch);
+  };
+  if (tid == 0) {
+    mbar_init(bars, 1);
+    mbar_init(bars + 1, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) { issue(0, std::integral_constant<int, 0>{}); issue(0, std::integral_constant<int, 1>{}); }
+
+  // one unit: wait for its boxes, walk, hand the slot to unit u + 2
+  auto unit = [&](int m, auto dc) {
+    constexpr int d = decltype(dc)::value;
+    const double cEn = m == 4 ? 1.0 : 0.0;
+    const bool en = m == 4;
+    {
+      const int u = 3 * m + d, s = u & 1;
+      const double *sU = flux_smem + 3 * s * C::BOX, *sV = sU + C::BOX, *sP = sV + C::BOX;
+      const double cM = m == 1 + d ? 1.0 : 0.0;
+      const bool withp = en || m == 1 + d;
+      const double al = alpha[d];
+      double Fh[SEG + 1];
+      if (d == 0) {           // x pencils: lanes run over the rows (y, z) of the box [z][y][TX + 6]
+        const int r = tid % C::ROWS, xs = (tid / C::ROWS) * SEG;
+        const int base = r * (TX + 6) + xs;
+        mbar_wait(bars + s, (u >> 1) & 1);
+        if (withp) weno_faces<SEG>([&](int k, double &a, double &b) { split2(sU[base + k], sV[base + k], sP[base + k], cEn, cM, al, a, b); }, Fh);
+        else weno_faces<SEG>([&](int k, double &a, double &b) { split_adv(sU[base + k], sV[base + k], al, a, b); }, Fh);
+#pragma unroll
+        for (int i = 0; i < SEG; i++) sL[r * C::LP + xs + i] = (Fh[i] - Fh[i + 1]) * hidx[0];
+      } else if (d == 1) {    // y pencils: lanes along x, box [z][TY + 6][TX + 2], cell x at column x + 1
+        constexpr int TXB = C::TXB;
+        const int x = tid % TX, rest = tid / TX;
+        const int lz = rest % TZ, seg = (rest / TZ) * SEG;
+        const int base = (lz * (TY + 6) + seg) * TXB + x + 1;
+        mbar_wait(bars + s, (u >> 1) & 1);
+        if (withp) weno_faces<SEG>([&](int k, double &a, double &b) { split2(sU[base + k * TXB], sV[base + k * TXB], sP[base + k * TXB], cEn, cM, al, a, b); }, Fh);
+        else weno_faces<SEG>([&](int k, double &a, double &b) { split_adv(sU[base + k * TXB], sV[base + k * TXB], al, a, b); }, Fh);
+        double *acc = sL + (lz * TY + seg) * C::LP + x;
+#pragma unroll
+        for (int i = 0; i < SEG; i++) acc[i * C::LP] += (Fh[i] - Fh[i + 1]) * hidx[1];
+      } else {                // z pencils: lanes along x, box [TZ + 6][y][TX + 2]; RK stage of the pencil's own cells
+        const int x = tid % TX, rest = tid / TX;
+        const int ly = rest % TY, seg = (rest / TY) * SEG;
+        const int base = (seg * TY + ly) * C::TXB + x + 1;
+        constexpr int SK = TY * C::TXB;
+        const int g0 = o0 + x, g1 = o1 + ly;
+        const int idc = goff + min(g0, P.n[0] - 1) + min(g1, P.n[1] - 1) * s1;
+        const double *U0m = U0p + (long long)m * P.pc;
+        double *Uom = Uop + (long long)m * P.pc;
+        double u0v[SEG];
+        if (!same) {
+#pragma unroll
+          for (int i = 0; i < SEG; i++) u0v[i] = U0m[idc + min(o2 + seg + i, P.n[2] - 1) * s2];
+        }
+        mbar_wait(bars + s, (u >> 1) & 1);
+        if (withp) weno_faces<SEG>([&](int k, double &a, double &b) { split2(sU[base + k * SK], sV[base + k * SK], sP[base + k * SK], cEn, cM, al, a, b); }, Fh);
+        else weno_faces<SEG>([&](int k, double &a, double &b) { split_adv(sU[base + k * SK], sV[base + k * SK], al, a, b); }, Fh);
+#pragma unroll
+        for (int i = 0; i < SEG; i++) {
+          const int g2 = o2 + seg + i;
+          if (g0 < P.n[0] && g1 < P.n[1] && g2 < P.n[2]) {
+            const double L = sL[((seg + i) * TY + ly) * C::LP + x] + (Fh[i] - Fh[i + 1]) * hidx[2];
+            const double uk = sU[base + (i + 3) * SK];
+            const double u0 = same ? uk : u0v[i];
+            Uom[goff + g0 + g1 * s1 + g2 * s2] = u0 + coef * ((uk - u0) + dt * L);
+          }
+        }
+      }
+      __syncthreads();   // everyone is done with slot s; sL is ordered between the directions
+      if (tid == 0 && u + 2 < nunits) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy reads before the async-proxy write
+        issue(d == 0 ? m : m + 1, std::integral_constant<int, (d + 2) % 3>{});
+      }
+    }
+  };
+#pragma unroll 1
+  for (int m = 0; m < P.nvar; m++) {
+    unit(m, std::integral_constant<int, 0>{});
+    unit(m, std::integral_constant<int, 1>{});
+    unit(m, std::integral_constant<int, 2>{});
+  }
+}

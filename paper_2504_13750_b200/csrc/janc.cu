@@ -42,6 +42,8 @@ struct janc_ctx {
   bool uses_cmech = false;              // table-driven kernels (c_mech in constant memory) are on this context's path
   CUtensorMap mapU[3], mapP, mapV;      // 2-D TMA path: {Px, Py, fields} over the RK registers A, B, C, over p and over vel
   bool have_tma = false;
+  Flux3Maps map3[3];                    // 3-D TMA path: per RK register, the three box shapes over the register, vel and p
+  bool have_tma3 = false;
   janc_grid g;
   int device;
   cudaStream_t stream;
@@ -607,11 +609,62 @@ static bool make_map(CUtensorMap *m, void *base, int Px, int Py, long long nfiel
              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// 4-D view {Px, Py, Pz, fields} for the 3-D TMA path: one map per box shape
+static bool make_map4(CUtensorMap *m, void *base, const int *Pd, long long nfields, int bx, int by, int bz) {
+  typedef CUresult (*encode_t)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                               const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn) {
+    cudaGetLastError();
+    return false;
+  }
+  const cuuint64_t dims[4] = {(cuuint64_t)Pd[0], (cuuint64_t)Pd[1], (cuuint64_t)Pd[2], (cuuint64_t)nfields};
+  const cuuint64_t strides[3] = {(cuuint64_t)Pd[0] * 8, (cuuint64_t)Pd[0] * Pd[1] * 8, (cuuint64_t)Pd[0] * Pd[1] * Pd[2] * 8};
+  const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz, 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  return ((encode_t)fn)(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // which tile the non-gathering 2-D path uses: 0 = 64 x 16 (8-cell pencils), 1 = 32 x 16, 2 = 16 x 16 (4-cell pencils)
 static int tile2d(const janc_ctx *c) { return c->P.n[0] <= 16 && c->P.n[1] <= 16 ? 2 : c->P.n[0] <= 32 ? 1 : 0; }
 
+#define JANC_F3T 16, 8, 8, 8      // tile and pencil length of the 3-D TMA flux kernel
+
+static void setup_tma3(janc_ctx *c) {
+  c->have_tma3 = false;
+  const Params &P = c->P;
+  if (c->g.ndim != 3 || (P.P[0] & 1)) return;      // global strides must be multiples of 16 bytes
+  constexpr int T[4] = {JANC_F3T};
+  double *regs[3] = {c->A, c->B, c->C};
+  bool ok = true;
+  for (int d = 0; d < 3; d++) {
+    const int bx = T[0] + (d == 0 ? 6 : 2), by = T[1] + (d == 1 ? 6 : 0), bz = T[2] + (d == 2 ? 6 : 0);   // y / z boxes start at an even x
+    for (int q = 0; q < 3; q++) {
+      ok = ok && make_map4(&c->map3[q].U[d], regs[q], P.P, (long long)c->np * c->nvar, bx, by, bz);
+      ok = ok && make_map4(&c->map3[q].V[d], P.vel, P.P, (long long)c->np * 3, bx, by, bz);
+      ok = ok && make_map4(&c->map3[q].P[d], P.p, P.P, c->np, bx, by, bz);
+    }
+  }
+  c->have_tma3 = ok;
+}
+
+template <int TX, int TY, int TZ, int SEG>
+static void launch_flux3_tma(janc_ctx *c, const double *Uk, const double *U0, double *Uout, int slot_base, double coef) {
+  using C = Flux3TmaCfg<TX, TY, TZ, SEG>;
+  const Params &P = c->P;
+  smem_attr(c, (const void *)k_flux_rk3_tma<TX, TY, TZ, SEG>, C::SMEM);
+  const unsigned tiles = (unsigned)(((P.n[0] + TX - 1) / TX) * ((P.n[1] + TY - 1) / TY) * ((P.n[2] + TZ - 1) / TZ));
+  const int which = Uk == c->A ? 0 : Uk == c->B ? 1 : 2;
+  k_flux_rk3_tma<TX, TY, TZ, SEG><<<dim3(tiles, (unsigned)c->actn, 1), C::NT, C::SMEM, c->stream>>>(P, U0, Uout, slot_base, coef, Uk == U0 ? 1 : 0,
+                                                                                          c->map3[which]);
+}
+
 static void setup_tma(janc_ctx *c) {
   c->have_tma = false;
+  setup_tma3(c);
   const Params &P = c->P;
   if (c->g.ndim != 2 || (P.P[0] & 1) || ((long long)P.P[0] * P.P[1] & 1)) return;   // strides must be multiples of 16 bytes
   const int t = tile2d(c), bx = (t == 0 ? 64 : t == 1 ? 32 : 16) + 6, by = 16 + 6;
@@ -888,7 +941,8 @@ static void do_flux(janc_ctx *c, const double *Uk, const double *U0, double *Uou
     }
     else if (c->P.n[0] <= 32) launch_flux2<32, 16, 4, false>(c, Uk, U0, Uout, slot_base, coef);   // patches of <= 32 columns with materialised ghosts
     else launch_flux2<64, 16, 8>(c, Uk, U0, Uout, slot_base, coef);
-  } else launch_flux<3, 16, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);   // 128 threads, 39 KB: 4 independent CTAs per SM overlap stage / walk
+  } else if (c->opt.tma && c->have_tma3) launch_flux3_tma<JANC_F3T>(c, Uk, U0, Uout, slot_base, coef);   // boxes by TMA, two units ahead
+  else launch_flux<3, 16, 8, 8, 8>(c, Uk, U0, Uout, slot_base, coef);   // 128 threads, 39 KB: 4 independent CTAs per SM overlap stage / walk
   note_launch(c, cudaGetLastError());
   prof_mark(c, pf, 2);
 }

@@ -160,7 +160,31 @@ def test_3d_ragged_nonperiodic(B, ref):
     g = c1.grid
     U = c1.U[:, :, :18, :13, :].copy(); T = c1.T[:, :18, :13, :].copy()
     g2 = I.Grid(3, (20, 13, 18), g.dx, (I.BC_REFLECT, I.BC_OUTFLOW, I.BC_PERIODIC), (I.BC_OUTFLOW, I.BC_REFLECT, I.BC_PERIODIC))
-    check(B, ref, I.Case("3d_ragged", g2, c1.mech, U, T, 0.2, 2), 2, TOL1 * 10)
+    case = I.Case("3d_ragged", g2, c1.mech, U, T, 0.2, 2)
+    check(B, ref, case, 2, TOL1 * 10)                           # even padded width: the TMA flux kernel
+    check(B, ref, case, 2, TOL1 * 10, options={"tma": 0})       # the staged kernel it replaces (still the odd-width path)
+    odd = I.Case("3d_ragged_odd", I.Grid(3, (19, 13, 18), g.dx, g2.bc_lo, g2.bc_hi), c1.mech,
+                 np.ascontiguousarray(U[..., :19]), np.ascontiguousarray(T[..., :19]), 0.2, 2)
+    check(B, ref, odd, 2, TOL1 * 10)                            # odd padded width: TMA not applicable
+
+
+def test_3d_tma_flux_kernel_is_bitwise_the_staged_one(B):
+    """k_flux_rk3_tma does the arithmetic of k_flux_rk<3> in the same order: identical states on ragged grids (tiles that
+    stick out in x, y, z; a grid smaller than one tile), with chemistry and over several steps."""
+    def run(case, opts):
+        s = B.Solver(case.grid, case.mech, case.blocks, options=opts)
+        s.set_state(case.U, case.T)
+        s.step(3, cfl=case.cfl)
+        U, _ = s.get_state()
+        assert s.status == 0
+        s.close()
+        return U
+    c = I.config4(n=40, nspheres=3, radius=5)
+    for n in ((40, 20, 12), (34, 10, 18), (16, 8, 8), (6, 4, 4)):
+        g = I.Grid(3, n, c.grid.dx, c.grid.bc_lo, c.grid.bc_hi)
+        sub = I.Case("crop", g, c.mech, np.ascontiguousarray(c.U[:, :, 8:8 + n[2], 8:8 + n[1], :n[0]]),
+                     np.ascontiguousarray(c.T[:, 8:8 + n[2], 8:8 + n[1], :n[0]]), c.cfl, 3)
+        assert np.array_equal(run(sub, {"tma": 1}), run(sub, {"tma": 0})), n
 
 
 # ------------------------------------------------------------------ generic species count (run-time ns path)
