@@ -44,6 +44,11 @@ inline int roles_nr() { return roles_nr_ref(); }
 // factorised with one ROW per lane inside a warp (no inter-warp synchronisation), false = the column-distributed
 // Gauss-Jordan across the role warps
 inline bool &roles_lu_rows_ref() { static thread_local bool v = true; return v; }
+// where T* = T(U*) comes from (janc_set_option "roles_newton"): false = the cons->prim kernel is run on U* just before this
+// kernel and T* is read from the T array (default: in this kernel the Newton iteration is a chain of barriers and
+// dependent operations on 8 warps per SM, 2.1 k cycles per turn; the bandwidth-bound cons->prim kernel does it for the
+// whole grid in 0.6 ms at full occupancy), true = the Newton iteration runs inside this kernel
+inline bool &roles_newton_ref() { static thread_local bool v = false; return v; }
 
 struct RolesLayout {
   int oX, oP, oN, oRN, oDL, oRHS, oF, oPIV, oIP, oXS, oNX, oR, oPB, rows;   // offsets in rows of 32 doubles
@@ -54,8 +59,23 @@ struct RolesLayout {
 
 // sizes that depend on the mechanism only: polynomial degrees, reaction orders, table lengths
 struct RolesDims { int degh, degc, nkb, maxof, maxob, nslot; };
+// Reactions are dealt to the roles round-robin, third-body reactions first; a role's list is its third-body reactions
+// followed by the others padded to a multiple of four with the dummy reaction `nr` (k_f = 1, no species, results
+// stored to rows of their own), so that the rate loop only has a four-reactions-per-trip body.
+inline int roles_slots(const MechC &M) {
+  const int NR = roles_nr();
+  int ntb = 0;
+  for (int i = 0; i < M.nr; i++) ntb += M.tb[i] ? 1 : 0;
+  int best = 1;
+  for (int w = 0; w < NR; w++) {
+    int tb = 0, other = 0;
+    for (int q = w; q < M.nr; q += NR) (q < ntb ? tb : other)++;
+    best = std::max(best, tb + (other + 3) / 4 * 4);
+  }
+  return best;
+}
 inline RolesDims roles_dims(const MechC &M) {
-  RolesDims D{1, 0, 3, 1, 1, (M.nr + roles_nr() - 1) / roles_nr()};
+  RolesDims D{1, 0, 3, 1, 1, roles_slots(M)};
   for (int k = 0; k < M.ns; k++)
     for (int q = 1; q <= 4; q++)
       if (M.nasa[k][q] != 0.0) { D.degh = std::max(D.degh, q + 1); D.degc = std::max(D.degc, q); }
@@ -68,11 +88,11 @@ inline RolesDims roles_dims(const MechC &M) {
 }
 inline size_t roles_table_doubles(const MechC &M) {
   const RolesDims D = roles_dims(M);
-  return (size_t)2 * M.ns + (size_t)M.ns * (D.degh + 1) + (size_t)M.ns * (D.degc + 1) + (size_t)M.nr * 3 + (size_t)M.nr * D.nkb + (size_t)M.ntb * M.ns;
+  return (size_t)2 * M.ns + (size_t)M.ns * (D.degh + 1) + (size_t)M.ns * (D.degc + 1) + (size_t)(M.nr + 1) * 3 + (size_t)(M.nr + 1) * D.nkb + (size_t)M.ntb * M.ns;
 }
 inline size_t roles_table_ints(const MechC &M) {
   const RolesDims D = roles_dims(M);
-  return (size_t)roles_nr() * D.nslot + M.nr + (size_t)M.nr * D.maxof + (size_t)M.nr * D.maxob;
+  return (size_t)roles_nr() * D.nslot + (M.nr + 1) + (size_t)(M.nr + 1) * D.maxof + (size_t)(M.nr + 1) * D.maxob;
 }
 
 inline bool roles_applicable(const MechC &M) {
@@ -96,13 +116,13 @@ inline RolesLayout roles_layout(const MechC &M, int ndim) {
   L.oNX = o; o += ndim + 2 + n1 + 1;         // U (nvar rows) and T of the NEXT turn's cells, prefetched with cp.async
   // one region, three lives: M k_f, M k_b, q per reaction (until the assembly barrier); the multipliers of every
   // column (elimination: nothing is reused, so the roles may run several columns apart); the whole system (slow path)
-  // row-LU: the system transposed to [row][column][cell] with the row stride padded so that the lanes of a half-warp
-  // (16 / NR cells x NR rows) read 16 distinct 8-byte banks
-  L.rstr = (n1 + 1) * 32 + 16 / roles_nr();
+  // row-LU: the system transposed to [row][column][cell] with the row stride padded by the cells per warp, so that the
+  // lanes of a warp (lane = row group x cells per warp + cell) read 32 consecutive doubles
+  L.rstr = (n1 + 1) * 32 + 32 / roles_nr();
   { int usz = 0; for (int c = 0; c < n1; c++) usz += (n1 + 1 - c + 1) / 2 * 2;   // triangular U store per cell, even row lengths,
     L.pbs = usz + (n1 + 2) / 2 * 2 + 4; }                                          // + the overrun of fixed-length row writes
 
-  L.oR = o; o += std::max(std::max(3 * nr, n1 * (n1 + 1)), roles_lu_rows_ref() ? (n1 * L.rstr + 31) / 32 : 0);
+  L.oR = o; o += std::max(std::max(3 * (nr + 1), n1 * (n1 + 1)), roles_lu_rows_ref() ? (n1 * L.rstr + 31) / 32 : 0);
   L.oF = L.oR;
   L.oPB = o; if (roles_lu_rows_ref()) o += L.pbs;                        // U store: pbs doubles per cell x 32 cells
   L.rows = o;
@@ -163,7 +183,12 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   for (int i = 0; i < nr; i++) if (!M.tb[i]) order.push_back(i);
   const int NSLOT = DM.nslot;
   std::vector<int> ri((size_t)NR * NSLOT, -1);
-  for (int q = 0; q < nr; q++) ri[(size_t)(q % NR) * NSLOT + q / NR] = order[q];
+  const int nrs = nr + 1;                              // row stride of the k_f / k_b / q rows: the dummy reaction has rows too
+  for (int w = 0; w < NR; w++) {
+    int n = 0, other = 0;
+    for (int q = w; q < nr; q += NR) { ri[(size_t)w * NSLOT + n++] = order[q]; if (!M.tb[order[q]]) other++; }
+    for (; other % 4; other++) ri[(size_t)w * NSLOT + n++] = nr;
+  }
 
   // =========================================================================== tables
   src += "// generated by chemgen_roles.h for ns=" + I(ns) + " nr=" + I(nr) + " ndim=" + I(ndim) + "\n";
@@ -189,12 +214,15 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     for (int q = 0; q <= degc; q++) td.push_back(num(cc[q]));
   }
   addd("kf", okf); for (int i = 0; i < nr; i++) { td.push_back(num(M.lnA[i])); td.push_back(num(M.b[i])); td.push_back(num(-M.Ta[i])); }
+  for (int q = 0; q < 3; q++) td.push_back(num(0.0));
   addd("kb", okb); for (int i = 0; i < nr; i++) for (int q = 0; q < NKB; q++) td.push_back(num(kbc[(size_t)i * 7 + q]));
+  for (int q = 0; q < NKB; q++) td.push_back(num(0.0));
   addd("eff", oeff); for (int q = 0; q < M.ntb; q++) for (int k = 0; k < ns; k++) td.push_back(num(M.eff[q][k]));
   ori = (int)ti.size(); for (int v : ri) ti.push_back(I(v));
   ofl = (int)ti.size(); for (int i = 0; i < nr; i++) ti.push_back(I((M.rev[i] ? 1 : 0) | ((M.tb[i] ? M.tbi[i] + 1 : 0) << 1)));
-  ore = (int)ti.size(); for (int i = 0; i < nr; i++) for (int q = 0; q < maxof; q++) ti.push_back(I(q < M.nreac[i] ? M.reac[i][q] : ns));
-  opr = (int)ti.size(); for (int i = 0; i < nr; i++) for (int q = 0; q < maxob; q++) ti.push_back(I(q < M.nprod[i] ? M.prod[i][q] : ns));
+  ti.push_back(I(0));
+  ore = (int)ti.size(); for (int i = 0; i <= nr; i++) for (int q = 0; q < maxof; q++) ti.push_back(I(i < nr && q < M.nreac[i] ? M.reac[i][q] : ns));
+  opr = (int)ti.size(); for (int i = 0; i <= nr; i++) for (int q = 0; q < maxob; q++) ti.push_back(I(i < nr && q < M.nprod[i] ? M.prod[i][q] : ns));
   const int NTD = (int)td.size(), NTI = (int)ti.size();
   if ((size_t)NTD != roles_table_doubles(M) || (size_t)NTI != roles_table_ints(M)) return std::string("#error roles table size\n");
   src += "__constant__ double g_td[" + I(NTD) + "] = {";
@@ -280,6 +308,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   for (int s = 0; s < NSL; s++)
     E.line("const double yr" + I(s) + " = k" + I(s) + " < " + I(ns) + " ? Y" + I(s) + " * c_Rk[k" + I(s) + " < " + I(ns) + " ? k" + I(s) + " : 0] : 0.0;");
   // ---- Newton on e(T) (eq 4.3-4.4, reading A6): partial sums per role, summed in the same order by everyone
+  if (roles_newton_ref()) {
   E.line("bool conv = false;");
   E.line("#pragma unroll 1");
   E.line("for (int it = 0; it < 50; it++) {");
@@ -303,69 +332,82 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("}");
   E.line("bool ok = conv && (T > 0.0) && isfinite(T);");
   E.line("if (live && w == 0) a.T[pid] = T;");
+  } else {
+  E.line("bool ok = (T > 0.0) && isfinite(T);     // T* was computed by the cons->prim kernel launched before this one");
+  }
   // ---- rates of progress (eq 4.7-4.9): shared code, tables indexed by the warp-uniform role.  Third-body
   //      reactions come first in every role's list; the others are taken two at a time (branch-free body,
   //      so the two exponential chains interleave).
-  auto rate_body = [&](const std::string &S, const std::string &idx, bool tb) {
+  // One reaction in three parts, so that a trip through the loop can be emitted as  loads of all its reactions / arithmetic
+  // / stores: everything lives in one shared-memory array, so the compiler may not move the loads of the next reaction
+  // above the stores of the previous one, and a body written reaction by reaction executes them one after the other
+  // (two exponential chains in flight instead of eight).
+  auto rate_loads = [&](const std::string &S, const std::string &idx) {
     E.line("    const int i" + S + " = " + idx + ";");
     E.line("    const double *f" + S + " = c_kf + 3 * i" + S + ";");
-    E.line("    const double kf" + S + " = exp_nb(fma(f" + S + "[2], iT, fma(f" + S + "[1], lnT, f" + S + "[0])));");
+    E.line("    const double f0" + S + " = f" + S + "[0], f1" + S + " = f" + S + "[1], f2" + S + " = f" + S + "[2];");
     if (any_rev) {
       E.line("    const double *d" + S + " = c_kb + " + I(NKB) + " * i" + S + ";");
-      std::string lk = "fma(d" + S + "[2], iT, fma(d" + S + "[1], lnT, d" + S + "[0]))";
+      std::string l = "    const double ";
+      for (int q = 0; q < NKB; q++) l += "d" + I(q) + S + " = d" + S + "[" + I(q) + "]" + (q + 1 < NKB ? ", " : ";");
+      E.line(l);
+      if (!all_rev) E.line("    const double rv" + S + " = (double)(c_fl[i" + S + "] & 1);");
+    }
+    for (int q = 0; q < maxof; q++) E.line("    const double xf" + I(q) + S + " = SM(" + I(L.oX) + " + c_re[i" + S + " * " + I(maxof) + " + " + I(q) + "]);");
+    if (any_rev) for (int q = 0; q < maxob; q++) E.line("    const double xb" + I(q) + S + " = SM(" + I(L.oX) + " + c_pr[i" + S + " * " + I(maxob) + " + " + I(q) + "]);");
+  };
+  auto rate_math = [&](const std::string &S) {
+    E.line("    const double kf" + S + " = exp_nb(fma(f2" + S + ", iT, fma(f1" + S + ", lnT, f0" + S + ")));");
+    if (any_rev) {
+      std::string lk = "fma(d2" + S + ", iT, fma(d1" + S + ", lnT, d0" + S + "))";
       if (degc > 0) {
-        std::string pol = "d" + S + "[" + I(NKB - 1) + "]";
-        for (int q = NKB - 2; q >= 3; q--) pol = "fma(T, " + pol + ", d" + S + "[" + I(q) + "])";
+        std::string pol = "d" + I(NKB - 1) + S;
+        for (int q = NKB - 2; q >= 3; q--) pol = "fma(T, " + pol + ", d" + I(q) + S + ")";
         lk = "fma(T, " + pol + ", " + lk + ")";
       }
-      // branch-free (a branch per reaction keeps the compiler from interleaving the exponential chains of the
-      // reactions of one trip): irreversible reactions multiply a finite exponential by zero
+      // branch-free: irreversible reactions multiply a finite exponential by zero
       if (all_rev) E.line("    const double kb" + S + " = exp_nb(" + lk + ");");
-      else E.line("    const double kb" + S + " = exp_nb(" + lk + ") * (double)(c_fl[i" + S + "] & 1);");
+      else E.line("    const double kb" + S + " = exp_nb(" + lk + ") * rv" + S + ";");
     } else {
       E.line("    const double kb" + S + " = 0.0;");
     }
     E.line("    double pf" + S + " = kf" + S + ", pb" + S + " = kb" + S + ";");
-    for (int q = 0; q < maxof; q++) E.line("    pf" + S + " *= SM(" + I(L.oX) + " + c_re[i" + S + " * " + I(maxof) + " + " + I(q) + "]);");
-    if (any_rev) for (int q = 0; q < maxob; q++) E.line("    pb" + S + " *= SM(" + I(L.oX) + " + c_pr[i" + S + " * " + I(maxob) + " + " + I(q) + "]);");
+    for (int q = 0; q < maxof; q++) E.line("    pf" + S + " *= xf" + I(q) + S + ";");
+    if (any_rev) for (int q = 0; q < maxob; q++) E.line("    pb" + S + " *= xb" + I(q) + S + ";");
     E.line("    const double rn" + S + " = pf" + S + " - pb" + S + ";");
-    if (tb) {
-      E.line("    const int tb_ = (c_fl[i" + S + "] >> 1) - 1;");
-      E.line("    const double *ef = c_eff + tb_ * " + I(ns) + ";");
-      // four partial sums: the ns-term chain of dependent FMAs would be the longest path of the trip
-      E.line("    double Mi, Mi1 = 0.0, Mi2 = 0.0, Mi3 = 0.0;");
-      E.line("    Mi = ef[0] * SM(" + I(L.oX) + ");");
-      for (int j = 1; j < ns; j++) {
-        const std::string acc = (j % 4 == 0) ? "Mi" : "Mi" + I(j % 4);
-        E.line("    " + acc + " = fma(ef[" + I(j) + "], SM(" + I(L.oX + j) + "), " + acc + ");");
-      }
-      E.line("    Mi = (Mi + Mi1) + (Mi2 + Mi3);");
-      E.line("    SM(" + I(L.oRN) + " + tb_) = rn" + S + ";");
-      E.line("    SM(" + I(L.oR) + " + i" + S + ") = Mi * kf" + S + "; SM(" + I(L.oR + nr) + " + i" + S + ") = Mi * kb" + S + "; SM(" + I(L.oR + 2 * nr) + " + i" + S + ") = Mi * rn" + S + ";");
-    } else {
-      E.line("    SM(" + I(L.oR) + " + i" + S + ") = kf" + S + "; SM(" + I(L.oR + nr) + " + i" + S + ") = kb" + S + "; SM(" + I(L.oR + 2 * nr) + " + i" + S + ") = rn" + S + ";");
-    }
   };
-  const std::string RI = "c_ri[w * " + I(NSLOT) + " + r]", RI1 = "c_ri[w * " + I(NSLOT) + " + r + 1]";
+  auto rate_stores = [&](const std::string &S) {
+    E.line("    SM(" + I(L.oR) + " + i" + S + ") = kf" + S + "; SM(" + I(L.oR + nrs) + " + i" + S + ") = kb" + S + "; SM(" + I(L.oR + 2 * nrs) + " + i" + S + ") = rn" + S + ";");
+  };
+  const std::string RI = "c_ri[w * " + I(NSLOT) + " + r]";
   E.line("{ const double lnT = log(T), iT = 1.0 / T;");
   E.line("  int r = 0;");
   if (M.ntb > 0) {
     E.line("  #pragma unroll 1");
     E.line("  for (; r < " + I(NSLOT) + "; r++) {");
     E.line("    if (" + RI + " < 0 || (c_fl[" + RI + "] >> 1) == 0) break;");
-    rate_body("", RI, true);
+    rate_loads("", RI);
+    E.line("    const int tb_ = (c_fl[i] >> 1) - 1;");
+    E.line("    const double *ef = c_eff + tb_ * " + I(ns) + ";");
+    // four partial sums: the ns-term chain of dependent FMAs would be the longest path of the trip
+    E.line("    double Mi, Mi1 = 0.0, Mi2 = 0.0, Mi3 = 0.0;");
+    E.line("    Mi = ef[0] * SM(" + I(L.oX) + ");");
+    for (int j = 1; j < ns; j++) {
+      const std::string acc = (j % 4 == 0) ? "Mi" : "Mi" + I(j % 4);
+      E.line("    " + acc + " = fma(ef[" + I(j) + "], SM(" + I(L.oX + j) + "), " + acc + ");");
+    }
+    E.line("    Mi = (Mi + Mi1) + (Mi2 + Mi3);");
+    rate_math("");
+    E.line("    SM(" + I(L.oRN) + " + tb_) = rn;");
+    E.line("    SM(" + I(L.oR) + " + i) = Mi * kf; SM(" + I(L.oR + nrs) + " + i) = Mi * kb; SM(" + I(L.oR + 2 * nrs) + " + i) = Mi * rn;");
     E.line("  }");
   }
-  const std::string RIq[4] = {RI, RI1, "c_ri[w * " + I(NSLOT) + " + r + 2]", "c_ri[w * " + I(NSLOT) + " + r + 3]"};
   E.line("  #pragma unroll 1");
   E.line("  for (; r + 3 < " + I(NSLOT) + "; r += 4) {");
-  E.line("    if (" + RIq[3] + " < 0) break;");
-  for (int q = 0; q < 4; q++) rate_body(std::string(1, (char)('a' + q)), RIq[q], false);
-  E.line("  }");
-  E.line("  #pragma unroll 1");
-  E.line("  for (; r < " + I(NSLOT) + "; r++) {");
   E.line("    if (" + RI + " < 0) break;");
-  rate_body("", RI, false);
+  for (int q = 0; q < 4; q++) rate_loads(std::string(1, (char)('a' + q)), "c_ri[w * " + I(NSLOT) + " + r + " + I(q) + "]");
+  for (int q = 0; q < 4; q++) rate_math(std::string(1, (char)('a' + q)));
+  for (int q = 0; q < 4; q++) rate_stores(std::string(1, (char)('a' + q)));
   E.line("  }");
   E.line("}");
   E.line("BAR();");
@@ -386,7 +428,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
       std::string sum;
       for (int i = 0; i < nr; i++) {
         if (dnu[i][k] == 0) continue;
-        const std::string q = row(L.oR + 2 * nr + i);
+        const std::string q = row(L.oR + 2 * nrs + i);
         if (sum.empty()) sum = dnu[i][k] == 1 ? q : dnu[i][k] == -1 ? "-" + q : num((double)dnu[i][k]) + " * " + q;
         else if (dnu[i][k] == 1) sum = "(" + sum + " + " + q + ")";
         else if (dnu[i][k] == -1) sum = "(" + sum + " - " + q + ")";
@@ -414,7 +456,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
         const bool rev = M.rev[i] != 0, tb = M.tb[i] != 0;
         const std::string si = I(i);
         std::string dq;
-        const std::string cfs = row(L.oR + i), cbs = row(L.oR + nr + i);
+        const std::string cfs = row(L.oR + i), cbs = row(L.oR + nrs + i);
         if (cf[i][j] > 0) dq = (cf[i][j] > 1 ? num((double)cf[i][j]) + " * " : std::string("")) + xprod(cfs, cf[i].data(), ns, j);
         if (rev && cb[i][j] > 0) dq += (dq.empty() ? "-" : " - ") + (cb[i][j] > 1 ? num((double)cb[i][j]) + " * " : std::string("")) + xprod(cbs, cb[i].data(), ns, j);
         (void)tb;     // the efficiency term a_ij r_i of a third-body reaction touches every column: shared code below
@@ -512,7 +554,10 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   // physical columns and fewer live row slots.
   E.line("int bad = 0;");
   E.line("{");
-  E.line("  const int g_ = threadIdx.x % " + I(NR) + ", cell_ = threadIdx.x / " + I(NR) + ";");
+  // lane = row group x CW + cell of the warp (CW = 32 / NR cells per warp): the CW lanes that own a row are adjacent,
+  // so their 16-byte publishing stores go out as one shared-memory wavefront (one lane per quarter-warp costs four)
+  const int CW = 32 / NR;
+  E.line("  const int g_ = lane / " + I(CW) + ", cell_ = w * " + I(CW) + " + lane % " + I(CW) + ";");
   E.line("  const double *mr_ = sm_ + " + I(L.oR * 32) + " + g_ * " + I(L.rstr) + " + cell_;");
   E.line("  double *us_ = sm_ + " + I(L.oPB * 32) + " + cell_ * " + I(L.pbs) + ";     // U rows of this cell, row c at uoff(c)");
   for (int t = 0; t < RS; t++) {
@@ -652,7 +697,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     E.line("  for (int c = " + I(chi) + "; c >= " + I(clo) + "; c--) {");
     E.line("    const int go = c - " + I(clo) + ";");
     E.line("    double x_ = Y" + I(to) + " * IP" + I(to) + ";");
-    E.line("    x_ = __shfl_sync(0xffffffffu, x_, (lane & " + I(~(NR - 1) & 31) + ") | go);");
+    E.line("    x_ = __shfl_sync(0xffffffffu, x_, go * " + I(CW) + " + lane % " + I(CW) + ");");
     E.line("    if (g_ == go) XS" + I(to) + " = x_;");
     for (int t = 0; t <= to; t++)                                        // rows of higher slots are all > c
       E.line("    if (r" + I(t) + " < c) Y" + I(t) + " = fma(-p" + I(t) + "[c], x_, Y" + I(t) + ");");

@@ -30,6 +30,8 @@ struct Options {
   int jit_max_unknowns = JANC_JIT_MAX_N1;   // "jit_max_unknowns": largest system of the one-thread-per-cell kernel
   bool jit_big_smem = false;            // "jit_big" = "smem": the shared-memory kernel instead of the role-warp kernel
   int roles = 8;                        // "roles": 8 or 16 role-warps
+  bool roles_lu_rows = true;            // "roles_lu" = "rows": LU with one row per lane | "columns": Gauss-Jordan across the role warps
+  bool roles_newton_prim = true;        // "roles_newton" = "prim": T* from a cons->prim launch before the role-warp kernel | "kernel"
   bool tma = true;                      // "tma": 2-D tiles through cp.async.bulk.tensor (TMA) where the layout allows | cp.async
   bool halo_in_kernel = true;           // "halo" = "auto": 2-D patches <= 16 x 16 / small grids gather their halo in the
                                         //   flux kernel; "ghost": always materialise ghosts with k_ghost
@@ -359,6 +361,8 @@ static void jit_setup(janc_ctx *c) {
   c->jit_chem_mode = 0;
   if (!c->opt.jit) { c->jit_log = "disabled by janc_set_option(\"jit\", \"0\")"; return; }
   chemgen::roles_nr_ref() = c->opt.roles;
+  chemgen::roles_lu_rows_ref() = c->opt.roles_lu_rows;
+  chemgen::roles_newton_ref() = !c->opt.roles_newton_prim;
   const int mode = jit_chem_mode(M, c->opt);
   const bool chem = mode != 0;
   c->jit_chem_mode = mode;
@@ -435,6 +439,8 @@ extern "C" int janc_jit_probe(const janc_mech *m, int ndim, char *src_out, size_
   if (rc) return rc;
   const Options opt;
   chemgen::roles_nr_ref() = opt.roles;
+  chemgen::roles_lu_rows_ref() = opt.roles_lu_rows;
+  chemgen::roles_newton_ref() = !opt.roles_newton_prim;
   const int mode = jit_chem_mode(M, opt);
   std::string src = chemgen::generate_prim(M, ndim);
   if (mode == 3) src += chemgen::generate_roles(M, ndim);
@@ -542,6 +548,14 @@ extern "C" int janc_set_option(janc_ctx *c, const char *key, const char *value) 
   if (k == "roles") {
     if (v != "8" && v != "16") { c->err = "roles: 8 | 16"; return JANC_EINVAL; }
     c->opt.roles = atoi(value); return JANC_OK;
+  }
+  if (k == "roles_lu") {
+    if (v != "rows" && v != "columns") { c->err = "roles_lu: rows | columns"; return JANC_EINVAL; }
+    c->opt.roles_lu_rows = v == "rows"; return JANC_OK;
+  }
+  if (k == "roles_newton") {
+    if (v != "prim" && v != "kernel") { c->err = "roles_newton: prim | kernel"; return JANC_EINVAL; }
+    c->opt.roles_newton_prim = v == "prim"; return JANC_OK;
   }
   c->err = "unknown option '" + k + "'";
   return JANC_EINVAL;
@@ -961,6 +975,8 @@ static void launch_chem_reg(janc_ctx *c, double *U) {
 static void do_chem(janc_ctx *c, double *U, Prof *pf) {
   if (c->jit_kernel) {
     const Params &P = c->P;
+    // role-warp kernel: T* = T(U*) from the bandwidth-bound cons->prim kernel (chemgen_roles.h, roles_newton_ref)
+    if (c->jit_chem_mode == 3 && c->opt.roles_newton_prim) do_prim(c, U, 0, 0, nullptr, nullptr);
     ChemArgs a{U, P.T, P.scal, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc, c->actn, c->act0, P.dt_scale};
     void *args[] = {&a};
     dim3 grid = cell_grid(c, c->jit_chem_cells, c->actn);
