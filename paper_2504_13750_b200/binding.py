@@ -178,11 +178,36 @@ def measure_dfma_peak(device=0, stream=None):
     return out.value
 
 
+def workspace_bytes_for(grid, mech, device=0, options=None):
+    """janc_workspace_bytes of a context for `grid` (n_patches taken from it) and `mech`, without allocating anything:
+    how the AMR driver sizes the workspace for its block capacity."""
+    L = lib()
+    g = _Grid(grid.ndim, (C.c_int * 3)(*grid.n), (C.c_double * 3)(*grid.dx), (C.c_int * 3)(*grid.bc_lo), (C.c_int * 3)(*grid.bc_hi),
+              grid.n_patches, grid.n_levels, grid.ratio)
+    h = C.c_void_p()
+    rc = L.janc_create(C.byref(g), int(device), None, C.byref(h))
+    if rc:
+        raise JancError(rc, "janc_create")
+    try:
+        for k, v in (options or {}).items():
+            if L.janc_set_option(h, str(k).encode(), str(v).encode()):
+                raise JancError(JANC_EINVAL, f"janc_set_option({k})")
+        m, keep = _mech_struct(mech)
+        rc = L.janc_set_mechanism(h, C.byref(m))
+        if rc:
+            raise JancError(rc, "janc_set_mechanism")
+        return int(L.janc_workspace_bytes(h))
+    finally:
+        L.janc_destroy(h)
+
+
 class Solver:
     """janc_* context: create -> set_mechanism -> bind_workspace (torch) -> [set_blocks] -> set_state
     -> step -> get_state -> destroy.  Same call names as the C ABI."""
 
-    def __init__(self, grid, mech, blocks=None, device=0, stream=None, options=None):
+    def __init__(self, grid, mech, blocks=None, device=0, stream=None, options=None, workspace=None):
+        """workspace: a uint8 CUDA tensor to bind instead of allocating one (at least workspace_bytes + 256 bytes; the
+        AMR driver keeps one sized for its block capacity across regrids)."""
         import torch
         if not torch.cuda.is_available():
             raise JancError(JANC_ECUDA, "no CUDA device (libjanc has no CPU fallback)")
@@ -205,7 +230,13 @@ class Solver:
         m, self._keep = _mech_struct(mech)
         self._check(L.janc_set_mechanism(self._h, C.byref(m)), "janc_set_mechanism")
         nbytes = L.janc_workspace_bytes(self._h)
-        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{self.device}")
+        self.workspace_bytes = nbytes
+        if workspace is not None:
+            if not (workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.numel() >= nbytes + 256):
+                raise JancError(JANC_EINVAL, f"workspace tensor too small: {workspace.numel()} < {nbytes + 256}")
+            self.workspace = workspace
+        else:
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{self.device}")
         base = (self.workspace.data_ptr() + 255) // 256 * 256
         self._ws_off = base - self.workspace.data_ptr()
         self._check(L.janc_bind_workspace(self._h, C.c_void_p(base), nbytes), "janc_bind_workspace")
@@ -288,8 +319,9 @@ class Solver:
         a = self._ws_off + off.value
         return self.workspace[a:a + 8 * cnt.value].view(self._torch.int64)
 
-    def regrid(self, thr, nbuf):
-        """janc_regrid_plan + janc_regrid_fill: (level, nbr, parent, U, T) of the regridded two-level list (host arrays)."""
+    def regrid(self, thr, nbuf, device=False):
+        """janc_regrid_plan + janc_regrid_fill: (level, nbr, parent, U, T) of the regridded two-level list (lists: host
+        arrays; U, T: host arrays, or CUDA tensors with device=True)."""
         nd = 1 + (self.shape[3] > 1) + (self.shape[2] > 1)
         cap = self.np_ * (1 + (1 << nd))
         level = np.zeros(cap, np.int32); nbr = np.zeros((cap, 2 * nd), np.int32); parent = np.zeros((cap, 1 + nd), np.int32)
@@ -301,6 +333,8 @@ class Solver:
         U = torch.empty((k,) + self.shape[1:], dtype=torch.float64, device=f"cuda:{self.device}")
         T = torch.empty((k,) + self.shape[2:], dtype=torch.float64, device=f"cuda:{self.device}")
         self._check(lib().janc_regrid_fill(self._h, C.c_void_p(U.data_ptr()), C.c_void_p(T.data_ptr()), 1), "janc_regrid_fill")
+        if device:
+            return level[:k].copy(), nbr[:k].copy(), parent[:k].copy(), U, T
         return level[:k].copy(), nbr[:k].copy(), parent[:k].copy(), U.cpu().numpy(), T.cpu().numpy()
 
     def last_dt(self):

@@ -599,3 +599,46 @@ def test_regrid_matches_the_oracle(B, ref, mech9):
                                                        n_patches=len(lg), n_levels=2, ratio=2),
                      case.mech, Ug, Tg, case.cfl, 2, blocks=I.Blocks(lg, ng, pg))
         check(B, ref, new, 2, TOL1 * 100)
+
+
+def test_amr_run_cycles_against_the_oracle(B, ref, mech9):
+    """amr.AmrRun (advance / regrid cycles, workspace capacity by Algorithm 1 of the paper): four cycles of a driver
+    front sweeping over a two-level list.  Per cycle the oracle advances the same list from the same state (parity within
+    tolerance), then both regrid the GPU's state: identical lists, bitwise identical data.  The workspace is re-allocated
+    only when N_max changes."""
+    from paper_2504_13750_b200 import amr
+    base = I.config2(nx=128, ny=64, mech=mech9)
+    base.grid.bc_hi = (I.BC_REFLECT, I.BC_REFLECT, 0)
+    m0 = np.zeros((8, 16), bool); m0[:, 0] = True
+    case = I.refine_uniform(base, (8, 8), m0)
+    run = amr.AmrRun(case, thr=0.05, nbuf=2, every=10 ** 9, n_max=1)
+    assert run.n_max >= run.n_valid + 1 and run.allocations == 1
+    seen = set()
+    for cycle in range(4):
+        U0, T0 = run.state()
+        grid = I.Grid(2, case.grid.n, case.grid.dx, case.grid.bc_lo, case.grid.bc_hi, n_patches=len(run.blocks.level), n_levels=2, ratio=2)
+        r = ref.RefSolver(grid, case.mech, run.blocks); r.set_state(U0, T0)
+        run.step(3, cfl=case.cfl); r.step(3, cfl=case.cfl)
+        Ug, Tg = run.state(); Ur, _ = r.get_state()
+        assert r.status == 0
+        assert field_errors(case, Ug, Ur).max() <= TOL1 * 100, cycle
+        r.set_state(Ug, Tg)                                   # the criterion is a threshold: decide on the same data
+        lr, nr_, pr, Ur2, Tr2 = r.regrid(0.05, 2)
+        n_max_before, alloc_before = run.n_max, run.allocations
+        run.regrid()
+        assert np.array_equal(run.blocks.level, lr) and np.array_equal(run.blocks.nbr, nr_) and np.array_equal(run.blocks.parent, pr)
+        Ug2, Tg2 = run.state()
+        assert np.array_equal(Ug2, Ur2) and np.array_equal(Tg2, Tr2)
+        assert run.n_max == amr.update_n_max(run.n_valid, n_max_before)
+        assert run.allocations == alloc_before + (run.n_max != n_max_before)
+        seen.add(run.n_valid)
+        r.close()
+    assert len(seen) > 1, "the refined region never changed"
+    # the loop that regrids by itself: same lists as stepping and regridding by hand (deterministic kernels)
+    a = amr.AmrRun(case, thr=0.05, nbuf=2, every=3, n_max=64)
+    a.step(12, cfl=case.cfl)
+    assert a.regrids == 4 and np.array_equal(a.blocks.level, run.blocks.level) and np.array_equal(a.blocks.parent, run.blocks.parent)
+    Ua, _ = a.state(); Ub, _ = run.state()
+    assert np.array_equal(Ua, Ub)
+    assert a.n_max <= 64 and a.n_max >= a.n_valid + 1
+    a.close(); run.close()
