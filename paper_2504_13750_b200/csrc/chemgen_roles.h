@@ -86,13 +86,20 @@ inline RolesDims roles_dims(const MechC &M) {
   }
   return D;
 }
+// The rate loop reads one packed record per (role, slot) instead of tables indexed by the reaction number: the addresses
+// depend on the loop counter only (no load -> index -> load chain) and the record comes in 16-byte loads.
+//   doubles (RC, even): ln A, b, -Ta, the NKB reverse-rate coefficients, 1.0 / 0.0 = reversible
+//   ints    (RX, multiple of 4): reaction index (nr = dummy, -1 = end of list), third-body row + 1, reactants, products
+inline int roles_rc(const MechC &M) { return (3 + roles_dims(M).nkb + 1 + 1) / 2 * 2; }
+inline int roles_rx(const MechC &M) { const RolesDims D = roles_dims(M); return (2 + D.maxof + D.maxob + 3) / 4 * 4; }
 inline size_t roles_table_doubles(const MechC &M) {
   const RolesDims D = roles_dims(M);
-  return (size_t)2 * M.ns + (size_t)M.ns * (D.degh + 1) + (size_t)M.ns * (D.degc + 1) + (size_t)(M.nr + 1) * 3 + (size_t)(M.nr + 1) * D.nkb + (size_t)M.ntb * M.ns;
+  const size_t n = (size_t)roles_nr() * D.nslot * roles_rc(M) + (size_t)2 * M.ns + (size_t)M.ns * (D.degh + 1) + (size_t)M.ns * (D.degc + 1) + (size_t)M.ntb * M.ns;
+  return (n + 1) / 2 * 2;        // the int table behind it stays 16-byte aligned
 }
 inline size_t roles_table_ints(const MechC &M) {
   const RolesDims D = roles_dims(M);
-  return (size_t)roles_nr() * D.nslot + (M.nr + 1) + (size_t)(M.nr + 1) * D.maxof + (size_t)(M.nr + 1) * D.maxob;
+  return (size_t)roles_nr() * D.nslot * roles_rx(M);
 }
 
 inline bool roles_applicable(const MechC &M) {
@@ -198,7 +205,26 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   // warp-uniform, run-time indexed reads of the rate loop are plain broadcast loads.
   std::vector<std::string> td, ti;
   auto addd = [&](const std::string &name, int &off) { off = (int)td.size(); (void)name; };
-  int oiW, oRk, ohc, occ, okf, okb, oeff, ori, ofl, ore, opr;
+  int oiW, oRk, ohc, occ, oeff;
+  const int RC = roles_rc(M), RX = roles_rx(M);
+  // packed records first (16-byte aligned: the tables start on a 256-byte boundary)
+  for (int w = 0; w < NR; w++)
+    for (int q = 0; q < NSLOT; q++) {
+      const int i = ri[(size_t)w * NSLOT + q];
+      const bool real = i >= 0 && i < nr;
+      std::vector<std::string> rec;
+      rec.push_back(num(real ? M.lnA[i] : 0.0)); rec.push_back(num(real ? M.b[i] : 0.0)); rec.push_back(num(real ? -M.Ta[i] : 0.0));
+      for (int e = 0; e < NKB; e++) rec.push_back(num(real ? kbc[(size_t)i * 7 + e] : 0.0));
+      rec.push_back(num(real && M.rev[i] ? 1.0 : 0.0));
+      while ((int)rec.size() < RC) rec.push_back(num(0.0));
+      for (auto &v : rec) td.push_back(v);
+      std::vector<int> rx;
+      rx.push_back(i); rx.push_back(real && M.tb[i] ? M.tbi[i] + 1 : 0);
+      for (int e = 0; e < maxof; e++) rx.push_back(real && e < M.nreac[i] ? M.reac[i][e] : ns);
+      for (int e = 0; e < maxob; e++) rx.push_back(real && e < M.nprod[i] ? M.prod[i][e] : ns);
+      while ((int)rx.size() < RX) rx.push_back(0);
+      for (int v : rx) ti.push_back(I(v));
+    }
   addd("iW", oiW); for (int k = 0; k < ns; k++) td.push_back(num(M.invW[k]));
   addd("Rk", oRk); for (int k = 0; k < ns; k++) td.push_back(num(M.Rk[k]));
   addd("hc", ohc);
@@ -213,16 +239,8 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     const double cc[5] = {c[0] - 1.0, c[1], c[2], c[3], c[4]};
     for (int q = 0; q <= degc; q++) td.push_back(num(cc[q]));
   }
-  addd("kf", okf); for (int i = 0; i < nr; i++) { td.push_back(num(M.lnA[i])); td.push_back(num(M.b[i])); td.push_back(num(-M.Ta[i])); }
-  for (int q = 0; q < 3; q++) td.push_back(num(0.0));
-  addd("kb", okb); for (int i = 0; i < nr; i++) for (int q = 0; q < NKB; q++) td.push_back(num(kbc[(size_t)i * 7 + q]));
-  for (int q = 0; q < NKB; q++) td.push_back(num(0.0));
   addd("eff", oeff); for (int q = 0; q < M.ntb; q++) for (int k = 0; k < ns; k++) td.push_back(num(M.eff[q][k]));
-  ori = (int)ti.size(); for (int v : ri) ti.push_back(I(v));
-  ofl = (int)ti.size(); for (int i = 0; i < nr; i++) ti.push_back(I((M.rev[i] ? 1 : 0) | ((M.tb[i] ? M.tbi[i] + 1 : 0) << 1)));
-  ti.push_back(I(0));
-  ore = (int)ti.size(); for (int i = 0; i <= nr; i++) for (int q = 0; q < maxof; q++) ti.push_back(I(i < nr && q < M.nreac[i] ? M.reac[i][q] : ns));
-  opr = (int)ti.size(); for (int i = 0; i <= nr; i++) for (int q = 0; q < maxob; q++) ti.push_back(I(i < nr && q < M.nprod[i] ? M.prod[i][q] : ns));
+  if (td.size() % 2) td.push_back(num(0.0));
   const int NTD = (int)td.size(), NTI = (int)ti.size();
   if ((size_t)NTD != roles_table_doubles(M) || (size_t)NTI != roles_table_ints(M)) return std::string("#error roles table size\n");
   src += "__constant__ double g_td[" + I(NTD) + "] = {";
@@ -262,8 +280,9 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("for (int q = threadIdx.x; q < " + I(NTD) + "; q += " + I(NR * 32) + ") s_td[q] = g_td[q];");
   E.line("for (int q = threadIdx.x; q < " + I(NTI) + "; q += " + I(NR * 32) + ") s_ti[q] = g_ti[q];");
   E.line("const double *c_iW = s_td + " + I(oiW) + ", *c_Rk = s_td + " + I(oRk) + ", *c_hc = s_td + " + I(ohc) + ", *c_cc = s_td + " + I(occ) +
-         ", *c_kf = s_td + " + I(okf) + ", *c_kb = s_td + " + I(okb) + ", *c_eff = s_td + " + I(oeff) + ";");
-  E.line("const int *c_ri = s_ti + " + I(ori) + ", *c_fl = s_ti + " + I(ofl) + ", *c_re = s_ti + " + I(ore) + ", *c_pr = s_ti + " + I(opr) + ";");
+         ", *c_eff = s_td + " + I(oeff) + ";");
+  E.line("const double2 *c_rc = (const double2 *)s_td + w * " + I(NSLOT * RC / 2) + ";     // this role's records");
+  E.line("const int4 *c_rx = (const int4 *)s_ti + w * " + I(NSLOT * RX / 4) + ";");
   E.line("int *s_flag = (int *)(sm_ + " + I(L.oPIV * 32) + ");");
   E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2, nbp = (ncell + 31) / 32, nbt = nbp * a.np;");
   E.line("const double dt = a.scal[0] * a.dts;");
@@ -342,19 +361,26 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   // / stores: everything lives in one shared-memory array, so the compiler may not move the loads of the next reaction
   // above the stores of the previous one, and a body written reaction by reaction executes them one after the other
   // (two exponential chains in flight instead of eight).
-  auto rate_loads = [&](const std::string &S, const std::string &idx) {
-    E.line("    const int i" + S + " = " + idx + ";");
-    E.line("    const double *f" + S + " = c_kf + 3 * i" + S + ";");
-    E.line("    const double f0" + S + " = f" + S + "[0], f1" + S + " = f" + S + "[1], f2" + S + " = f" + S + "[2];");
+  auto rate_loads = [&](const std::string &S, const std::string &slot) {
+    const int ND2 = RC / 2, NI4 = RX / 4;
+    auto dv = [&](int e) { return "rc" + I(e / 2) + S + (e % 2 ? ".y" : ".x"); };
+    auto iv = [&](int e) { static const char *c[4] = {".x", ".y", ".z", ".w"}; return "rx" + I(e / 4) + S + c[e % 4]; };
+    std::string l = "    const double2 ";
+    for (int e = 0; e < ND2; e++) l += "rc" + I(e) + S + " = c_rc[(" + slot + ") * " + I(ND2) + " + " + I(e) + "]" + (e + 1 < ND2 ? ", " : ";");
+    E.line(l);
+    l = "    const int4 ";
+    for (int e = 0; e < NI4; e++) l += "rx" + I(e) + S + " = c_rx[(" + slot + ") * " + I(NI4) + " + " + I(e) + "]" + (e + 1 < NI4 ? ", " : ";");
+    E.line(l);
+    E.line("    const int i" + S + " = " + iv(0) + ";");
+    E.line("    const double f0" + S + " = " + dv(0) + ", f1" + S + " = " + dv(1) + ", f2" + S + " = " + dv(2) + ";");
     if (any_rev) {
-      E.line("    const double *d" + S + " = c_kb + " + I(NKB) + " * i" + S + ";");
-      std::string l = "    const double ";
-      for (int q = 0; q < NKB; q++) l += "d" + I(q) + S + " = d" + S + "[" + I(q) + "]" + (q + 1 < NKB ? ", " : ";");
+      l = "    const double ";
+      for (int q = 0; q < NKB; q++) l += "d" + I(q) + S + " = " + dv(3 + q) + (q + 1 < NKB ? ", " : ";");
       E.line(l);
-      if (!all_rev) E.line("    const double rv" + S + " = (double)(c_fl[i" + S + "] & 1);");
+      if (!all_rev) E.line("    const double rv" + S + " = " + dv(3 + NKB) + ";");
     }
-    for (int q = 0; q < maxof; q++) E.line("    const double xf" + I(q) + S + " = SM(" + I(L.oX) + " + c_re[i" + S + " * " + I(maxof) + " + " + I(q) + "]);");
-    if (any_rev) for (int q = 0; q < maxob; q++) E.line("    const double xb" + I(q) + S + " = SM(" + I(L.oX) + " + c_pr[i" + S + " * " + I(maxob) + " + " + I(q) + "]);");
+    for (int q = 0; q < maxof; q++) E.line("    const double xf" + I(q) + S + " = SM(" + I(L.oX) + " + " + iv(2 + q) + ");");
+    if (any_rev) for (int q = 0; q < maxob; q++) E.line("    const double xb" + I(q) + S + " = SM(" + I(L.oX) + " + " + iv(2 + maxof + q) + ");");
   };
   auto rate_math = [&](const std::string &S) {
     E.line("    const double kf" + S + " = exp_nb(fma(f2" + S + ", iT, fma(f1" + S + ", lnT, f0" + S + ")));");
@@ -379,15 +405,15 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   auto rate_stores = [&](const std::string &S) {
     E.line("    SM(" + I(L.oR) + " + i" + S + ") = kf" + S + "; SM(" + I(L.oR + nrs) + " + i" + S + ") = kb" + S + "; SM(" + I(L.oR + 2 * nrs) + " + i" + S + ") = rn" + S + ";");
   };
-  const std::string RI = "c_ri[w * " + I(NSLOT) + " + r]";
+  const std::string RI = "c_rx[r * " + I(RX / 4) + "].x", RTB = "c_rx[r * " + I(RX / 4) + "].y";
   E.line("{ const double lnT = log(T), iT = 1.0 / T;");
   E.line("  int r = 0;");
   if (M.ntb > 0) {
     E.line("  #pragma unroll 1");
     E.line("  for (; r < " + I(NSLOT) + "; r++) {");
-    E.line("    if (" + RI + " < 0 || (c_fl[" + RI + "] >> 1) == 0) break;");
-    rate_loads("", RI);
-    E.line("    const int tb_ = (c_fl[i] >> 1) - 1;");
+    E.line("    if (" + RI + " < 0 || " + RTB + " == 0) break;");
+    rate_loads("", "r");
+    E.line("    const int tb_ = rx0.y - 1;");
     E.line("    const double *ef = c_eff + tb_ * " + I(ns) + ";");
     // four partial sums: the ns-term chain of dependent FMAs would be the longest path of the trip
     E.line("    double Mi, Mi1 = 0.0, Mi2 = 0.0, Mi3 = 0.0;");
@@ -405,7 +431,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("  #pragma unroll 1");
   E.line("  for (; r + 3 < " + I(NSLOT) + "; r += 4) {");
   E.line("    if (" + RI + " < 0) break;");
-  for (int q = 0; q < 4; q++) rate_loads(std::string(1, (char)('a' + q)), "c_ri[w * " + I(NSLOT) + " + r + " + I(q) + "]");
+  for (int q = 0; q < 4; q++) rate_loads(std::string(1, (char)('a' + q)), "r + " + I(q));
   for (int q = 0; q < 4; q++) rate_math(std::string(1, (char)('a' + q)));
   for (int q = 0; q < 4; q++) rate_stores(std::string(1, (char)('a' + q)));
   E.line("  }");
