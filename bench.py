@@ -63,9 +63,9 @@ def chem_ops_per_cell(mech):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (flux: stages 2 and 3; the first stage reads U^n only
 # once) from the committed `ncu --set full` captures named in profiles/*_summary.md; None where no capture exists.
-NCU_TRAFFIC_BYTES = {                                   # profiles/r2_summary.md (captures prof_r2_cfg4 / cfg2 / cfg3)
-    ("cfg4_3d_256cubed", "chem"): 6.12e9,
-    ("cfg4_3d_256cubed", "flux"): 13.33e9,
+NCU_TRAFFIC_BYTES = {                                   # profiles/r2_summary.md (captures prof_r2b_cfg4, prof_r2_cfg2 / cfg3)
+    ("cfg4_3d_256cubed", "chem"): 5.98e9,
+    ("cfg4_3d_256cubed", "flux"): 13.30e9,
     ("cfg2_2d_channel_4096x512", "flux"): 6.31e8,
     ("cfg2_2d_channel_4096x512", "chem"): 3.15e8,
     ("cfg3_amr_8192x16x16", "flux"): 9.65e8,
@@ -326,6 +326,21 @@ def measure_slab(binding, case, K, W, local, rank, world, barrier):
     return out
 
 
+def flux_kernel_name(case):
+    """Which flux kernel janc.cu:do_flux launches for this workload with the default options."""
+    g = case.grid
+    even = (g.n[0] + 6) % 2 == 0                      # TMA needs 16-byte global strides: an even padded width
+    if g.ndim == 1:
+        return "k_flux_rk<1,128,1,1,4>"
+    if g.ndim == 3:
+        return "k_flux_rk3_tma<16,8,8,8>" if even else "k_flux_rk<3,16,8,8,8>"
+    if g.n[0] <= 16 and g.n[1] <= 16 and g.n_patches > 0:
+        return "k_flux_rk2<16,16,4,gather>"
+    if case.cells < 600000:
+        return "k_flux_rk2<32,16,4,gather>"
+    return "k_flux_rk2_tma<64,16,8>" if even else "k_flux_rk2<64,16,8>"
+
+
 def rooflines(case, m, K, dfma, hbm_peak, hbm_src):
     """Per-kernel roofline entries of one measured workload: algorithmic fp64 instructions and
     bytes per launch / the kernel's average launch duration (CUDA events, m["phases"]) against the DFMA rate measured
@@ -339,7 +354,7 @@ def rooflines(case, m, K, dfma, hbm_peak, hbm_src):
         avg = fl_ms / fl_n * 1e-3
         ops = flux_ops_per_cell_stage(nd, nvar) * cells
         byt = flux_bytes_per_cell_stage(nd, nvar) * cells
-        ent["flux"] = {"kernel": "k_flux_rk2" if nd == 2 else "k_flux_rk", "bound": "alu", "achieved": ops / avg / 1e12,
+        ent["flux"] = {"kernel": flux_kernel_name(case), "bound": "alu", "achieved": ops / avg / 1e12,
                        "peak": dfma / 1e12, "unit": "T fp64-instr/s (FMA=1)", "frac": ops / avg / dfma,
                        "traffic": NCU_TRAFFIC_BYTES.get((case.name, "flux")), "avg_launch_ms": avg * 1e3,
                        "launches_timed": fl_n, "ms_per_step": fl_ms / K,

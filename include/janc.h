@@ -94,8 +94,8 @@ int janc_create(const janc_grid *grid, int device, void *cuda_stream, janc_ctx *
 /* Options, as text (key, value); JANC_EINVAL for an unknown key or value.  The product runs the defaults; the other
  * values exist so that tests can reach every kernel and every host path without environment variables.
  *   "graph"            "1" (default) | "0"   replay one captured CUDA graph per step | eager launches
- *   "tma"              "1" (default) | "0"   2-D grids above 600 k cells with an even padded width: tiles staged with
- *                      cp.async.bulk.tensor (TMA) | with 8-byte cp.async
+ *   "tma"              "1" (default) | "0"   2-D grids above 600 k cells and 3-D grids, with an even padded width: tiles
+ *                      staged with cp.async.bulk.tensor (TMA) | with 8-byte cp.async (2-D) / staging loops (3-D)
  *   "halo"             "auto" (default) | "ghost"   auto: 2-D patches of <= 16 x 16 cells and 2-D grids below 600 k cells
  *                      gather their halo inside the flux kernel; ghost: k_ghost always materialises the ghost layers
  * and, only before janc_set_mechanism (JANC_ESTATE afterwards), the kernel selection of that call:
@@ -104,7 +104,9 @@ int janc_create(const janc_grid *grid, int device, void *cuda_stream, janc_ctx *
  *   "jit_big"          "roles" (default) | "smem"   kernel for larger mechanisms
  *   "roles"            "8" (default) | "16"  role-warps per CTA of the role-warp chemistry kernel
  *   "roles_lu"         "rows" (default) | "columns"  its linear solve: LU with one row per lane inside a warp |
- *                      column-distributed Gauss-Jordan across the role warps */
+ *                      column-distributed Gauss-Jordan across the role warps
+ *   "roles_newton"     "prim" (default) | "kernel"  where its T* = T(U*) comes from: a cons->prim launch in front of the
+ *                      kernel | the Newton iteration inside the kernel */
 int janc_set_option(janc_ctx *, const char *key, const char *value);
 
 /* Mechanism must be set before the workspace is sized (nvar depends on ns).  A rejected mechanism (JANC_EINVAL) leaves

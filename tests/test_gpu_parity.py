@@ -331,6 +331,19 @@ def test_role_warp_chemistry_kernel(B, ref, mech9, mech20):
     assert s.chem_kernel() == "jit-smem", s.jit_log()
     s.close()
     check(B, ref, c4, 1, TOL1, options={"jit_big": "smem"})
+    # the variants behind the options: Newton iteration inside the kernel, column-distributed Gauss-Jordan
+    for opt in ({"roles_newton": "kernel"}, {"roles_lu": "columns"}, {"roles_lu": "columns", "roles_newton": "kernel", "roles": 16}):
+        check(B, ref, c4, 2, TOL1 * 10, options=opt)
+        Ug, Tg, Ur, Tr = both(B, ref, case, 1, cfl=0.0, dt=1e-7, options=opt)
+        assert field_errors(case, Ug, Ur).max() <= 1e-8, opt
+    # the default takes T* from a cons->prim launch in front of the kernel: one launch more per step
+    a, b = (B.Solver(c4.grid, c4.mech, options={"graph": 0, **o}) for o in ({}, {"roles_newton": "kernel"}))
+    for s_ in (a, b):
+        s_.set_state(c4.U, c4.T)
+    n0 = (a.launch_count(), b.launch_count())
+    a.step(1, cfl=c4.cfl); b.step(1, cfl=c4.cfl)
+    assert (a.launch_count() - n0[0]) - (b.launch_count() - n0[1]) == 1
+    a.close(); b.close()
 
 
 def test_table_driven_chemistry_fallback_parity(B, ref):
