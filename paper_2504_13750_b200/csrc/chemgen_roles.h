@@ -257,16 +257,18 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   src += "#define AWAIT(id) asm volatile(\"barrier.sync %0, " + I(NR * 32) + ";\" :: \"r\"(id) : \"memory\")\n";
   src += "#define PUBLISH(id) do { asm volatile(\"barrier.arrive %0, " + I(NR * 32) + ";\" :: \"r\"(id) : \"memory\"); } while (0)\n";
   // the next turn's inputs: (nvar + 1) x 32 doubles, one 8-byte cp.async each, spread over the CTA
-  src += "__device__ __forceinline__ void prefetch_turn(const ChemArgs &a, double *sm_, long long bt, long long nbp, long long ncell) {\n"
-         "  for (int q = threadIdx.x; q < " + I((nvar + 1) * 32) + "; q += " + I(NR * 32) + ") {\n"
-         "    const int v = q >> 5, l = q & 31;\n"
-         "    const int patch = (int)(bt / nbp);      // relative to a.patch0\n"
-         "    long long t = (bt - (long long)patch * nbp) * 32 + l;\n"
-         "    if (t >= ncell) t = ncell - 1;\n"
-         "    const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;\n"
-         "    const int cj = (int)(r_ % a.n1), ck = (int)(r_ / a.n1);\n"
-         "    const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;\n"
-         "    const double *src = v < " + I(nvar) + " ? a.U + ((long long)(patch + a.patch0) * " + I(nvar) + " + v) * a.pc + id : a.T + (long long)(patch + a.patch0) * a.pc + id;\n"
+  // (32-bit index arithmetic, once per thread: a patch holds fewer than 2^31 cells; the 64-bit divisions this replaces
+  //  were ~1500 instructions per thread and turn)
+  src += "__device__ __forceinline__ void prefetch_turn(const ChemArgs &a, double *sm_, int prel, unsigned lt, unsigned ncell) {\n"
+         "  const int l = threadIdx.x & 31;\n"
+         "  unsigned t = lt * 32u + l;\n"
+         "  if (t >= ncell) t = ncell - 1u;\n"
+         "  const unsigned ci = t % (unsigned)a.n0, r_ = t / (unsigned)a.n0;\n"
+         "  const unsigned cj = r_ % (unsigned)a.n1, ck = r_ / (unsigned)a.n1;\n"
+         "  const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;\n"
+         "  const long long pb = prel + a.patch0;      // prel: patch relative to a.patch0, lt: turn within the patch\n"
+         "  for (int v = threadIdx.x >> 5; v < " + I(nvar + 1) + "; v += " + I(NR) + ") {\n"
+         "    const double *src = v < " + I(nvar) + " ? a.U + (pb * " + I(nvar) + " + v) * a.pc + id : a.T + pb * a.pc + id;\n"
          "    const unsigned dst = (unsigned)__cvta_generic_to_shared(sm_ + (" + I(L.oNX) + " + v) * 32 + l);\n"
          "    asm volatile(\"cp.async.ca.shared.global [%0], [%1], 8;\" :: \"r\"(dst), \"l\"(src) : \"memory\");\n"
          "  }\n"
@@ -284,19 +286,21 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("const double2 *c_rc = (const double2 *)s_td + w * " + I(NSLOT * RC / 2) + ";     // this role's records");
   E.line("const int4 *c_rx = (const int4 *)s_ti + w * " + I(NSLOT * RX / 4) + ";");
   E.line("int *s_flag = (int *)(sm_ + " + I(L.oPIV * 32) + ");");
-  E.line("const long long ncell = (long long)a.n0 * a.n1 * a.n2, nbp = (ncell + 31) / 32, nbt = nbp * a.np;");
+  E.line("const unsigned ncell = (unsigned)a.n0 * (unsigned)a.n1 * (unsigned)a.n2, nbp = (ncell + 31u) / 32u;");
+  E.line("const long long nbt = (long long)nbp * a.np;");
   E.line("const double dt = a.scal[0] * a.dts;");
-  E.line("if ((long long)blockIdx.x < nbt) prefetch_turn(a, sm_, blockIdx.x, nbp, ncell);");
+  E.line("int prel = (int)(blockIdx.x / nbp); unsigned lt = blockIdx.x % nbp;     // patch (relative) and turn within it, advanced without divisions");
+  E.line("if ((long long)blockIdx.x < nbt) prefetch_turn(a, sm_, prel, lt, ncell);");
   E.line("asm volatile(\"cp.async.wait_all;\" ::: \"memory\");");
   E.line("BAR();");
   E.line("#pragma unroll 1");
   E.line("for (long long bt = blockIdx.x; bt < nbt; bt += gridDim.x) {   // persistent CTA: 32 cells per turn");
-  E.line("const int patch = (int)(bt / nbp) + a.patch0;");
-  E.line("long long t = (bt - (long long)(patch - a.patch0) * nbp) * 32 + lane;");
+  E.line("const int patch = prel + a.patch0;");
+  E.line("unsigned t = lt * 32u + lane;");
   E.line("const bool live = t < ncell;");
-  E.line("if (!live) t = ncell - 1;   // idle lanes recompute the last cell and store nothing");
-  E.line("const int ci = (int)(t % a.n0); const long long r_ = t / a.n0;");
-  E.line("const int cj = (int)(r_ % a.n1), ck = (int)(r_ / a.n1);");
+  E.line("if (!live) t = ncell - 1u;   // idle lanes recompute the last cell and store nothing");
+  E.line("const unsigned ci = t % (unsigned)a.n0, r_ = t / (unsigned)a.n0;");
+  E.line("const unsigned cj = r_ % (unsigned)a.n1, ck = r_ / (unsigned)a.n1;");
   E.line("const long long id = (ci + a.G0) * a.st0 + (cj + a.G1) * a.st1 + (ck + a.G2) * a.st2;");
   E.line("double *Up = a.U + (long long)patch * " + I(nvar) + " * a.pc + id;");
   E.line("const long long pid = (long long)patch * a.pc + id;");
@@ -319,7 +323,9 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("SM(" + I(L.oP) + " + w) = pr_; SM(" + I(L.oP + NR) + " + w) = py_;");
   E.line("if (w == 0) SM(" + I(L.oX + ns) + ") = 1.0;");
   E.line("BAR();");
-  E.line("if (bt + gridDim.x < nbt) prefetch_turn(a, sm_, bt + gridDim.x, nbp, ncell);   // lands during this turn");
+  E.line("unsigned nlt = lt + gridDim.x; int nprel = prel;");
+  E.line("while (nlt >= nbp) { nlt -= nbp; nprel++; }");
+  E.line("if (bt + gridDim.x < nbt) prefetch_turn(a, sm_, nprel, nlt, ncell);   // lands during this turn");
   E.line("{ double rsum = 0.0, ysum = 0.0;");
   E.line("  #pragma unroll");
   E.line("  for (int q = 0; q < " + I(NR) + "; q++) { rsum += SM(" + I(L.oP) + " + q); ysum += SM(" + I(L.oP + NR) + " + q); }");
@@ -864,6 +870,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("if (!ok && live) *a.flag = 1;");
   E.line("asm volatile(\"cp.async.wait_all;\" ::: \"memory\");");
   E.line("BAR();   // shared rows are reused by the next turn; the prefetched inputs are visible to every role");
+  E.line("lt = nlt; prel = nprel;");
   E.line("}");
   src += "}\n#undef PST2\n#undef PST1\n#undef SM\n#undef BAR\n#undef AWAIT\n#undef PUBLISH\n";
   return src;
