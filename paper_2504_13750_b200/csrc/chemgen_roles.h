@@ -248,7 +248,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   src += "};\n__constant__ int g_ti[" + I(NTI) + "] = {";
   for (int q = 0; q < NTI; q++) src += (q ? ", " : "") + ti[q];
   src += "};\n";
-  emit_math(src, true);
+  emit_math(src, 2);
   // =========================================================================== kernel
   src += "#define SM(r) sm_[(r) * 32 + lane]\n";
   src += "#define BAR() asm volatile(\"bar.sync 0;\" ::: \"memory\")\n";
