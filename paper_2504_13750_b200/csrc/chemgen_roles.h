@@ -656,7 +656,9 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     E.line(ind + "}");
   };
   auto update_slot = [&](const std::string &cx, int t, int b, int ncols, const std::string &ind) {
-    E.line(ind + "{ const bool act = g_ + " + I(NR * t) + " > " + cx + "; const double l_ = act ? " + R(t, 0) + " * " + IPB(b) + " : 0.0;");
+    // rows <= c are dead values from here on (their U row is frozen in shared memory): they are updated like live rows,
+    // unmasked -- only the pivot check has to leave them out
+    E.line(ind + "{ const bool act = g_ + " + I(NR * t) + " > " + cx + "; const double l_ = " + R(t, 0) + " * " + IPB(b) + ";");
     E.line(ind + "  bad |= (int)(act & (fabs(" + R(t, 0) + ") > fabs(" + Q(b, 0) + ")));");
     for (int j = 1; j < ncols; j++) E.line(ind + "  " + R(t, j - 1) + " = fma(-l_, " + Q(b, j) + ", " + R(t, j) + ");");
     E.line(ind + "}");
