@@ -976,7 +976,7 @@ static void do_chem(janc_ctx *c, double *U, Prof *pf) {
   if (c->jit_kernel) {
     const Params &P = c->P;
     // role-warp kernel: T* = T(U*) from the bandwidth-bound cons->prim kernel (chemgen_roles.h, roles_newton_ref)
-    if (c->jit_chem_mode == 3 && c->opt.roles_newton_prim) do_prim(c, U, 0, 0, nullptr, nullptr);
+    if (c->jit_chem_mode == 3 && c->opt.roles_newton_prim) do_prim(c, U, 0, 0, nullptr, pf);   // timed as cons->prim (phase 0)
     ChemArgs a{U, P.T, P.scal, P.flag, P.n[0], P.n[1], P.n[2], P.G[0], P.G[1], P.G[2], P.st[0], P.st[1], P.st[2], P.pc, c->actn, c->act0, P.dt_scale};
     void *args[] = {&a};
     dim3 grid = cell_grid(c, c->jit_chem_cells, c->actn);
