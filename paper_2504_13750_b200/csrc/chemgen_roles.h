@@ -329,7 +329,11 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("{ double rsum = 0.0, ysum = 0.0;");
   E.line("  #pragma unroll");
   E.line("  for (int q = 0; q < " + I(NR) + "; q++) { rsum += SM(" + I(L.oP) + " + q); ysum += SM(" + I(L.oP + NR) + " + q); }");
-  E.line("  if (w == " + I(wN) + ") { ry" + I(sN) + " = rho - rsum; Y" + I(sN) + " = 1.0 - ysum; SM(" + I(L.oX + n1) + ") = ry" + I(sN) + " * " + num(M.invW[n1]) + "; } }");
+  // X of the last species: every role forms the same value (same sums, same order) and stores it itself before its own
+  // reads in the rate loop -- no barrier is needed between this store and those reads (with T* from the cons->prim
+  // launch there is no Newton loop, whose barriers used to separate them)
+  E.line("  SM(" + I(L.oX + n1) + ") = (rho - rsum) * " + num(M.invW[n1]) + ";");
+  E.line("  if (w == " + I(wN) + ") { ry" + I(sN) + " = rho - rsum; Y" + I(sN) + " = 1.0 - ysum; } }");
   for (int s = 0; s < NSL; s++)
     E.line("const double yr" + I(s) + " = k" + I(s) + " < " + I(ns) + " ? Y" + I(s) + " * c_Rk[k" + I(s) + " < " + I(ns) + " ? k" + I(s) + " : 0] : 0.0;");
   // ---- Newton on e(T) (eq 4.3-4.4, reading A6): partial sums per role, summed in the same order by everyone
