@@ -319,6 +319,7 @@ def test_role_warp_chemistry_kernel(B, ref, mech9, mech20):
     check(B, ref, c1, 1, TOL1, options=small)
     check(B, ref, c1, 20, TOL100, options=small)
     check(B, ref, I.config3(pcols=8, prows=4, npc=16), 2, TOL1 * 10, options=small)
+    check(B, ref, I.config3(pcols=8, prows=4, npc=16), 3, TOL100, options=small, crossover=True)   # per-level launches (patch0 / dt scale)
     case9 = big_dt_case(mech9, 40, 24, 7)
     Ug, Tg, Ur, Tr = both(B, ref, case9, 1, cfl=0.0, dt=2e-7, options=small)
     assert field_errors(case9, Ug, Ur).max() <= 1e-8
