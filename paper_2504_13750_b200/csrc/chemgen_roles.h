@@ -99,7 +99,7 @@ inline size_t roles_table_doubles(const MechC &M) {
 }
 inline size_t roles_table_ints(const MechC &M) {
   const RolesDims D = roles_dims(M);
-  return (size_t)roles_nr() * D.nslot * roles_rx(M);
+  return (size_t)roles_nr() * D.nslot * roles_rx(M) + (size_t)roles_nr() * 2;      // records + per-role trip counts
 }
 
 inline bool roles_applicable(const MechC &M) {
@@ -241,6 +241,19 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   }
   addd("eff", oeff); for (int q = 0; q < M.ntb; q++) for (int k = 0; k < ns; k++) td.push_back(num(M.eff[q][k]));
   if (td.size() % 2) td.push_back(num(0.0));
+  // per role: where its third-body reactions end and where its (padded) list ends -- the loops run on these counts
+  // instead of testing a table entry they have just loaded
+  const int ocnt = (int)ti.size();
+  for (int w = 0; w < NR; w++) {
+    int ntb_w = 0, nend = 0;
+    for (int q = 0; q < NSLOT; q++) {
+      const int i = ri[(size_t)w * NSLOT + q];
+      if (i < 0) break;
+      nend = q + 1;
+      if (i < nr && M.tb[i]) ntb_w = q + 1;
+    }
+    ti.push_back(I(ntb_w)); ti.push_back(I(nend));
+  }
   const int NTD = (int)td.size(), NTI = (int)ti.size();
   if ((size_t)NTD != roles_table_doubles(M) || (size_t)NTI != roles_table_ints(M)) return std::string("#error roles table size\n");
   src += "__constant__ double g_td[" + I(NTD) + "] = {";
@@ -293,6 +306,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("if ((long long)blockIdx.x < nbt) prefetch_turn(a, sm_, prel, lt, ncell);");
   E.line("asm volatile(\"cp.async.wait_all;\" ::: \"memory\");");
   E.line("BAR();");
+  E.line("const int r_tb = s_ti[" + I(ocnt) + " + 2 * w], r_end = s_ti[" + I(ocnt) + " + 2 * w + 1];     // this role's trip counts");
   E.line("#pragma unroll 1");
   E.line("for (long long bt = blockIdx.x; bt < nbt; bt += gridDim.x) {   // persistent CTA: 32 cells per turn");
   E.line("const int patch = prel + a.patch0;");
@@ -420,8 +434,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
   E.line("  int r = 0;");
   if (M.ntb > 0) {
     E.line("  #pragma unroll 1");
-    E.line("  for (; r < " + I(NSLOT) + "; r++) {");
-    E.line("    if (" + RI + " < 0 || " + RTB + " == 0) break;");
+    E.line("  for (; r < r_tb; r++) {");
     rate_loads("", "r");
     E.line("    const int tb_ = rx0.y - 1;");
     E.line("    const double *ef = c_eff + tb_ * " + I(ns) + ";");
@@ -439,8 +452,7 @@ inline std::string generate_roles(const MechC &M, int ndim) {
     E.line("  }");
   }
   E.line("  #pragma unroll 1");
-  E.line("  for (; r + 3 < " + I(NSLOT) + "; r += 4) {");
-  E.line("    if (" + RI + " < 0) break;");
+  E.line("  for (; r < r_end; r += 4) {");
   for (int q = 0; q < 4; q++) rate_loads(std::string(1, (char)('a' + q)), "r + " + I(q));
   for (int q = 0; q < 4; q++) rate_math(std::string(1, (char)('a' + q)));
   for (int q = 0; q < 4; q++) rate_stores(std::string(1, (char)('a' + q)));
