@@ -5,25 +5,24 @@
 // (3 KB per cell) has to live in shared memory, which leaves room for ~2 warps per SM and the kernel crawls
 // on latency.  Here a persistent CTA of 8 warps (one per SM) advances 32 cells per turn: lane = cell,
 // warp = ROLE.  Role w owns
-//   * species  k = w, w+8, w+16      (Newton partial sums for T, the final rho Y_k update),
-//   * reactions dealt round-robin    (Arrhenius / equilibrium exponentials, rates of progress: shared
-//                                     table-driven code; the tables are copied once per CTA into shared
-//                                     memory and read with warp-uniform indices: broadcast loads, no divergence;
-//                                     four reactions per trip through a branch-free body so their exp chains overlap),
-//   * columns  j = w, w+8, w+16 of the system [I - dt J | rhs], held in REGISTERS (57 doubles for Ns = 20).
+//   * species  k = w, w+8, w+16      (X_k, the final rho Y_k update; T* = T(U*) comes from a cons->prim launch in front of
+//                                     this kernel, or -- option roles_newton = kernel -- from Newton partial sums per role),
+//   * reactions dealt round-robin    (Arrhenius / equilibrium exponentials, rates of progress: shared table-driven code;
+//                                     one packed record per (role, slot), copied once per CTA into shared memory and read
+//                                     with warp-uniform addresses: broadcast loads, no divergence; four reactions per
+//                                     trip, emitted as loads / arithmetic / stores so that their exponential chains overlap),
+//   * columns  j = w, w+8, w+16 of the system [I - dt J | rhs], assembled in REGISTERS (57 doubles for Ns = 20).
 // The Jacobian columns are assembled by role-specific literal code (switch on the warp index: every
 // species / reaction index a literal, every update one register FMA, structural zeros never touched),
-// reading the 2 Nr rate coefficients the roles exchanged through shared memory ([row][cell], conflict-free).
-// The elimination is column-distributed Gauss-Jordan written as a compact loop over columns (warm in the
-// instruction cache; a first, fully unrolled version was bound by instruction fetch): the update writes row
-// p + 1 into row p, so the pivot row is always physical row 0 and register names stay static.  One-column
-// look-ahead: the owner of column c + 1 updates that column first and publishes its multipliers; roles
-// synchronise per column with producer / consumer named barriers (barrier.arrive / barrier.sync, ids 1..15),
-// never with a CTA-wide barrier, and no multiplier row is reused within a turn, so roles may run columns apart.
-// The register path never swaps rows: the owner checks that the diagonal entry IS the partial-pivoting choice
-// (first row of maximal |a_rc|, r >= c); if any of the 32 cells needs a swap the CTA spills the system to
-// shared memory and finishes with a generic, loop-based pivoted elimination (same pivot rule as the oracle).
-// All 8 roles of a cell see bit-identical T (same sums, same order).
+// reading the 2 Nr rate coefficients the roles exchanged through shared memory ([row][cell], conflict-free); the
+// third-body efficiency terms, which touch every column, are code shared by all roles.
+// Linear solve (default, roles_lu = rows): the columns are transposed through shared memory and factorised with one
+// ROW per lane inside a warp -- 8 lanes per cell, no inter-warp synchronisation, pivot rows broadcast through a per-cell
+// U store in shared memory, rolled and software-pipelined column loop (see the emitter below).  Kept as roles_lu =
+// columns: column-distributed Gauss-Jordan across the role warps with producer / consumer named barriers.
+// Neither fast path swaps rows: the owner checks that the diagonal entry IS the partial-pivoting choice
+// (first row of maximal |a_rc|, r >= c); if any of the 32 cells needs a swap the CTA solves the system in
+// shared memory with a generic, loop-based pivoted elimination (same pivot rule as the oracle).
 #pragma once
 #include <algorithm>
 
