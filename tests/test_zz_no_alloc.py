@@ -144,3 +144,35 @@ def test_static_scratch_rejects_sizes_beyond_the_maximum(B):
     ok = BareCtx(B, I.Grid(2, (64, 48, 1), (1e-3, 1e-3, 1.0), (2, 2, 0), (2, 2, 0)), I.inert_gas())
     assert ok.call(dummy, None, 0.0, dummy) == B.JANC_EINVAL and "cfl" in ok.error()
     ctx.close(); ok.close()
+
+
+def test_static_scratch_inside_cuda_graph_capture(B, mech9):
+    """The use case the entry point exists for: after one call outside capture (symbol address, species tables), calls
+    are captured into a CUDA graph -- where cudaMalloc and synchronisation are not allowed -- and the replay gives the
+    result of the workspace path for whatever state is in the caller's buffers at replay time."""
+    import torch
+    cs = I.config1(nx=96, ny=40, mech=mech9)
+    cs2 = evolved(B, cs, 6)
+    ref1, ref2 = existing_path(B, cs, cs.cfl), existing_path(B, cs2, cs2.cfl)
+    side = torch.cuda.Stream()
+    U = torch.from_numpy(np.ascontiguousarray(cs.U)).cuda()
+    T = torch.from_numpy(np.ascontiguousarray(cs.T)).cuda()
+    out = torch.zeros(4, dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        ctx = BareCtx(B, cs.grid, cs.mech)                       # bound to the side stream
+        assert ctx.call(U, T, cs.cfl, out) == 0, ctx.error()      # set-up call, outside capture
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            assert ctx.call(U, T, cs.cfl, out) == 0, ctx.error()
+    out.zero_()
+    g.replay(); torch.cuda.synchronize()
+    got1 = out.cpu().numpy().copy()
+    U.copy_(torch.from_numpy(np.ascontiguousarray(cs2.U))); T.copy_(torch.from_numpy(np.ascontiguousarray(cs2.T)))
+    g.replay(); torch.cuda.synchronize()
+    got2 = out.cpu().numpy().copy()
+    assert abs(got1[0] - ref1[0]) <= TOL * ref1[0] and np.abs(got1[1:] - ref1[1]).max() <= TOL * ref1[1].max()
+    assert abs(got2[0] - ref2[0]) <= TOL * ref2[0] and np.abs(got2[1:] - ref2[1]).max() <= TOL * ref2[1].max()
+    assert got1[0] != got2[0]
+    ctx.close()
