@@ -668,3 +668,35 @@ def test_amr_run_cycles_against_the_oracle(B, ref, mech9):
     assert np.array_equal(Ua, Ub)
     assert a.n_max <= 64 and a.n_max >= a.n_valid + 1
     a.close(); run.close()
+
+
+def test_amr_run_in_3d_and_1d(B, ref):
+    """The same cycle check on a 3-D two-level list (8^3 patches: TMA flux boxes that stick out of the patch, k_ghost with
+    coarse parents, 3-D regridding) and on a 1-D one."""
+    from paper_2504_13750_b200 import amr
+    b3 = I.config4(n=16, nspheres=2, radius=4)
+    m3 = np.zeros((2, 2, 2), bool); m3[0, 1, 0] = True
+    c3 = I.refine_uniform(b3, (8, 8, 8), m3)
+    b1 = I.config0(n=192)
+    b1.grid.bc_lo, b1.grid.bc_hi = (I.BC_REFLECT, 0, 0), (I.BC_OUTFLOW, 0, 0)
+    m1 = np.zeros(12, bool); m1[2] = True
+    c1 = I.refine_uniform(b1, (16,), m1)
+    for case, thr, nbuf in ((c3, 0.05, 1), (c1, 0.02, 2)):
+        run = amr.AmrRun(case, thr=thr, nbuf=nbuf, every=10 ** 9)
+        for cycle in range(2):
+            U0, T0 = run.state()
+            g = case.grid
+            grid = I.Grid(g.ndim, g.n, g.dx, g.bc_lo, g.bc_hi, n_patches=len(run.blocks.level), n_levels=2, ratio=2)
+            r = ref.RefSolver(grid, case.mech, run.blocks); r.set_state(U0, T0)
+            run.step(2, cfl=case.cfl); r.step(2, cfl=case.cfl)
+            Ug, Tg = run.state(); Ur, _ = r.get_state()
+            assert field_errors(case, Ug, Ur).max() <= TOL1 * 100, (case.name, cycle)
+            r.set_state(Ug, Tg)
+            lr, nr_, pr, Ur2, Tr2 = r.regrid(thr, nbuf)
+            run.regrid()
+            assert np.array_equal(run.blocks.level, lr) and np.array_equal(run.blocks.nbr, nr_) and np.array_equal(run.blocks.parent, pr), case.name
+            Ug2, Tg2 = run.state()
+            assert np.array_equal(Ug2, Ur2) and np.array_equal(Tg2, Tr2), case.name
+            r.close()
+        assert run.n_max >= run.n_valid + 1
+        run.close()
